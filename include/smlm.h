@@ -1,0 +1,180 @@
+/*
+ * smlm.h -- C ABI of libsmlm_b200: the data-parallel hot path of arXiv 2410.02314
+ * ("An efficient inference frame for single molecule localization microscopy") for one
+ * NVIDIA B200 (sm_100a).
+ *
+ * What the calls compute (PAPER.md = the paper text; "P:nn" = its line nn):
+ *   "the image is copied into GPU memory, where the model performs inference ...
+ *    post-processing is consolidated within GPU memory ... images are loaded into memory
+ *    in advance, allowing the network to directly access them from specified memory
+ *    locations during inference" (section 2.2, Fig. 1b);
+ *   the network is a stack of dilated convolutions whose per-pixel
+ *   outputs are "the probability of a fluorescent molecule, along with the offset ... of
+ *   the fluorescent molecule's position relative to that pixel"; post-processing
+ *   turns "these offsets into absolute coordinates" (P:192 item 3).
+ * The paper gives no layer table or detection rule; sizes, activations and the rule are
+ * BASELINE.json `north_star` / `configs` under the readings listed in DESIGN.md:
+ *
+ *   xhat = ((adu - offset) / gain) / norm_scale                              (per pixel)
+ *   a0   = act(conv3x3(xhat; W0) + b0), zero padding 1, act = ReLU iff stem_relu
+ *   a_{l+1} = a_l + ReLU(conv3x3 dilation d_l, zero padding d_l (a_l; W_l) + b_l)
+ *   o    = Wh a_L + bh                                                       (1x1 heads)
+ *   pixel q is an emitter iff sigmoid(o_p[q]) > threshold and o_p[q] beats each in-frame
+ *   8-neighbour (greater, or equal with the lower linear index iy*W+ix);
+ *   x_nm = (ix + xy_scale tanh(o_dx)) pixel_size, y likewise, z = z_scale tanh(o_z),
+ *   photons = photon_scale softplus(o_N), bg = bg_scale softplus(o_bg), p = sigmoid(o_p).
+ *
+ * Every step runs in hand-written CUDA kernels; there is no CPU fallback: on a machine
+ * without an sm_100 device smlm_create fails with SMLM_ERR_UNSUPPORTED_DEVICE.
+ *
+ * Conventions
+ *   - All structs are plain data, caller-owned, copied by the callee where noted.
+ *   - Status codes, never exceptions or abort().  smlm_last_error gives a message.
+ *   - One smlm_ctx per host thread; calls on one ctx must not overlap.
+ *   - "host" / "device" is stated for every pointer.
+ */
+#ifndef SMLM_H_
+#define SMLM_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SMLM_ABI_VERSION 1
+#define SMLM_MAX_LAYERS 32
+
+typedef struct smlm_ctx smlm_ctx; /* opaque; owns device weights, activations, staging slots, events */
+
+typedef enum {
+  SMLM_OK = 0,
+  SMLM_ERR_INVALID_ARG = -1,
+  SMLM_ERR_UNSUPPORTED_DEVICE = -2, /* current device is not sm_100 */
+  SMLM_ERR_CUDA = -3,
+  SMLM_ERR_OOM = -4,
+  SMLM_ERR_OVERFLOW = -5 /* more emitters found than capacity (reported by smlm_check) */
+} smlm_status;
+
+enum { SMLM_FP32 = 0, SMLM_BF16 = 1 };
+
+/* Trunk convolution kernel choice for SMLM_BF16 (fp32 mode always uses the CUDA-core kernel). */
+enum {
+  SMLM_CONV_AUTO = 0,   /* tcgen05 implicit GEMM */
+  SMLM_CONV_TCGEN05 = 1,
+  SMLM_CONV_DIRECT = 2  /* CUDA-core kernel with the same rounding points (cross-check) */
+};
+
+typedef struct {
+  uint32_t struct_size; /* sizeof(smlm_net_desc) */
+  uint32_t version;     /* SMLM_ABI_VERSION */
+  int32_t channels;     /* C: multiple of 16, 16..64 */
+  int32_t n_layers;     /* L: 0..SMLM_MAX_LAYERS dilated layers */
+  int32_t dilations[SMLM_MAX_LAYERS]; /* d_l in 1..8 */
+  int32_t head_channels; /* 5: p,dx,dy,N,bg    6: p,dx,dy,z,N,bg */
+  int32_t precision;     /* SMLM_FP32 | SMLM_BF16 (bf16 storage + bf16 tensor-core trunk, fp32 accumulate) */
+  int32_t stem_relu;     /* 1: ReLU after the stem conv */
+  float norm_scale;      /* 1000 */
+  float xy_scale;        /* 0.5 */
+  float z_scale_nm;      /* 700 */
+  float photon_scale;    /* multiplies softplus(o_N) */
+  float bg_scale;        /* multiplies softplus(o_bg) */
+  int32_t tile;          /* 0: whole frame; else frames are processed as tile x tile cores with a
+                            halo of (receptive-field radius + 1) and detections are owned by
+                            the tile whose core contains the pixel (no duplicates) */
+  int32_t micro_batch;   /* frames (or tiles) per kernel launch; 0 = auto */
+  int32_t conv_impl;     /* SMLM_CONV_* */
+  int32_t writeback_frames; /* flush the compacted emitter list to a HOST out_emitters once
+                               per this many frames (0 = once at the end of the call) */
+} smlm_net_desc;
+
+/* Camera model.  Scalars are used where a map pointer is NULL.  Maps are [H][W] float32,
+ * HOST or DEVICE memory, read during the call (copied to the device if on the host). */
+typedef struct {
+  float pixel_size_nm;
+  float offset; /* ADU */
+  float gain;   /* ADU per photon */
+  const float* offset_map;
+  const float* gain_map;
+} smlm_camera_params;
+
+/* One detection, 32 bytes.  `frame` is the index within the call, `pix` = iy*W + ix in
+ * full-frame coordinates. */
+typedef struct {
+  int32_t frame;
+  int32_t pix;
+  float x_nm, y_nm, z_nm; /* z_nm = 0 when head_channels == 5 */
+  float photons, bg, p;
+} smlm_emitter;
+
+/*
+ * smlm_create: validate `desc`, copy `weights` to the device, pre-pack the trunk weights
+ * for the tensor cores.  `weights` is a HOST pointer to one little-endian fp32 blob:
+ *     stem W[C][1][3][3], b[C];  for l < L: W_l[C][C][3][3] (OIHW), b_l[C];  head W[n_h][C], b[n_h]
+ * (cross-correlation).  Both inputs may be freed when the call returns.  Synchronous.
+ * Errors: INVALID_ARG (NULL, bad sizes), UNSUPPORTED_DEVICE, CUDA, OOM.  *out_ctx = NULL on error.
+ */
+smlm_status smlm_create(const smlm_net_desc* desc, const void* weights, smlm_ctx** out_ctx);
+
+/*
+ * smlm_localize: the whole hot path for n_frames frames of H x W uint16.
+ *   frames_u16   [n_frames][H][W], PINNED HOST memory (the preloaded ring: copied
+ *                host-to-device in micro-batches on an internal copy stream, overlapped with
+ *                compute) or DEVICE memory (no copy).  Pageable host memory is refused
+ *                (INVALID_ARG).  Must stay valid until `cuda_stream` has finished the call.
+ *   camera       HOST struct, copied.
+ *   threshold    detection threshold on p (strict >).  <= 0: every local maximum; >= 1: none.
+ *   out_emitters DEVICE or PINNED HOST array with room for `*out_count` records.  Order of
+ *                records is unspecified (atomic compaction); compare as a set.
+ *   out_count    HOST pointer.  In: capacity of out_emitters in records.  Out: number of
+ *                emitters found (may exceed the capacity; only the first `capacity` in arrival
+ *                order are stored).  Written asynchronously: valid after the stream finished.
+ *   cuda_stream  a cudaStream_t (NULL = legacy default stream).  The call only enqueues work;
+ *                it is ordered after earlier work on that stream; results are valid once the
+ *                stream has been synchronised.
+ * Errors: INVALID_ARG, CUDA, OOM synchronously; overflow via smlm_check after the sync.
+ */
+smlm_status smlm_localize(smlm_ctx* ctx, const uint16_t* frames_u16, int64_t n_frames, int32_t H,
+                          int32_t W, const smlm_camera_params* camera, float threshold,
+                          smlm_emitter* out_emitters, int64_t* out_count, void* cuda_stream);
+
+/* After the stream of the last smlm_localize has been synchronised: SMLM_ERR_OVERFLOW if it
+ * found more emitters than the capacity, SMLM_ERR_CUDA if an asynchronous error is pending. */
+smlm_status smlm_check(smlm_ctx* ctx);
+
+/* Synchronise, free everything the ctx owns.  NULL is allowed. */
+void smlm_destroy(smlm_ctx* ctx);
+
+/* Message of the last error on this ctx (or of the last failed smlm_create when ctx is NULL).
+ * The pointer stays valid until the next call on the ctx. */
+const char* smlm_last_error(const smlm_ctx* ctx);
+
+/* Number of kernel launches this ctx has enqueued so far (bench.py's `gpu_launches`). */
+int64_t smlm_launch_count(const smlm_ctx* ctx);
+
+/* Timing of the dominant kernel: when enabled, every trunk-convolution launch is bracketed
+ * by CUDA events on the launching stream; smlm_conv_time_ms sums them (after a stream
+ * sync) and reports the number of launches.  Disabled by default (events cost ~1 us). */
+smlm_status smlm_conv_timing(smlm_ctx* ctx, int32_t enable);
+smlm_status smlm_conv_time_ms(smlm_ctx* ctx, double* total_ms, int64_t* launches);
+
+/*
+ * Test/debug exports.  BASELINE.json asks for parity on the raw output maps, which the
+ * production path never writes to memory; these two calls expose them.
+ *   smlm_debug_forward_maps: `maps` is DEVICE float32 [n][n_h][H][W], the PRE-activation
+ *     head outputs o.  `trunk` (may be NULL) is DEVICE float32 [n][L+1][H][W][C], a_0..a_L.
+ *     frames_u16 as in smlm_localize.  Whole frames only (tile is ignored).
+ *   smlm_debug_postprocess: runs detection + decode + compaction on caller-supplied
+ *     DEVICE float32 maps o [n][n_h][H][W].
+ */
+smlm_status smlm_debug_forward_maps(smlm_ctx* ctx, const uint16_t* frames_u16, int64_t n_frames,
+                                    int32_t H, int32_t W, const smlm_camera_params* camera,
+                                    float* maps, float* trunk, void* cuda_stream);
+smlm_status smlm_debug_postprocess(smlm_ctx* ctx, const float* maps, int64_t n_frames, int32_t H,
+                                   int32_t W, const smlm_camera_params* camera, float threshold,
+                                   smlm_emitter* out_emitters, int64_t* out_count, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SMLM_H_ */
