@@ -1,0 +1,286 @@
+#!/usr/bin/env python
+"""Benchmark of the hot path (BASELINE.json metric: frames/s and emitters/s at 256x256 on one
+B200, device-timed; % of tensor / HBM peak).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1]
+
+One "step" = one smlm_localize call over the whole synthetic stack of the config (every row
+of the hot path: preload ring -> K1 stem -> K2 x L dilated convs -> K3 heads + post).
+Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from smlm_synth import get_config, make_frames, make_weights  # noqa: E402
+
+METRIC = "frames_per_s_256x256"
+UNIT = "frames/s"
+DISTINCT_FRAMES = 128       # generated once, cycled to the config's frame count (throughput is data-independent)
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p, "r", encoding="utf-8") as fh:
+            d = json.load(fh)
+        return d, "measured"
+    return dict(FALLBACK_PEAKS), "fallback"
+
+
+def workload(cfg, n_frames=None):
+    n = cfg.frames.n_frames if n_frames is None else n_frames
+    k = min(DISTINCT_FRAMES, n)
+    fs = make_frames(cfg, k)
+    reps = (n + k - 1) // k
+    frames = np.concatenate([fs.frames] * reps)[:n]
+    return fs, np.ascontiguousarray(frames)
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index = index
+        self.rows = []
+        self.stop_flag = threading.Event()
+
+    def run(self):
+        while not self.stop_flag.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                      "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout
+                parts = [p.strip() for p in out.strip().split(",")]
+                if len(parts) >= 7:
+                    self.rows.append(parts)
+            except Exception:
+                pass
+            self.stop_flag.wait(0.1)
+
+    def summary(self):
+        if not self.rows:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unsampled"]}
+        sm = sorted(float(r[0]) for r in self.rows)
+        reasons = []
+        for i, name in enumerate(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")):
+            if any(r[3 + i].lower().startswith("active") for r in self.rows):
+                reasons.append(name)
+        pw = max(float(r[2]) for r in self.rows if r[2].replace(".", "", 1).isdigit())
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.rows[0][1]), "power_w_max": pw,
+                "samples": len(self.rows), "reasons": reasons}
+
+
+def oracle_sample(cfg, fs, weights, n_sample):
+    """The oracle as it stands, timed on this host's cores on the first n_sample frames."""
+    from oracle import oracle as O
+    net = O.net_from_spec(cfg.net)
+    cam = O.make_camera(fs.pixel_size_nm, fs.offset, fs.gain, fs.offset_map, fs.gain_map)
+    O.lib()
+    t0 = time.perf_counter()
+    em = O.localize(net, weights, fs.frames[:n_sample], cam, cfg.threshold)
+    dt = time.perf_counter() - t0
+    return n_sample / dt, len(em) / dt, O.threads(), dt
+
+
+def run_reference(args, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    fs, _ = workload(cfg, n_frames=8)
+    w = make_weights(cfg)
+    n_sample = 2 if args.steps * 1 <= 12 else 1
+    for _ in range(args.warmup):
+        oracle_sample(cfg, fs, w, 1)
+    t_tot, frames = 0.0, 0
+    cores = 1
+    for _ in range(args.steps):
+        fps, eps, cores, dt = oracle_sample(cfg, fs, w, n_sample)
+        t_tot += dt
+        frames += n_sample
+    value = frames / t_tot
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_tot / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": cfg.name, "H": cfg.frames.height, "W": cfg.frames.width,
+                       "channels": cfg.net.channels, "layers": cfg.net.n_layers,
+                       "frames_per_step": n_sample, "note": "fp64 CPU oracle on host cores, bounded sample"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": f"{n_sample} frame(s) of {cfg.name} per step"},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=1)
+    ap.add_argument("--frames", type=int, default=0, help="override the number of frames per step")
+    ap.add_argument("--conv-impl", default="auto", choices=["auto", "tcgen05", "direct"])
+    ap.add_argument("--micro-batch", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    cfg = get_config(args.config)
+    if args.impl == "reference":
+        return run_reference(args, cfg)
+    args.warmup = max(args.warmup, 3)
+
+    import torch
+    import paper_2410_02314_b200 as P
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    n_frames = args.frames or cfg.frames.n_frames
+    fs, frames = workload(cfg, n_frames)
+    weights = make_weights(cfg)
+    H, W = frames.shape[1:]
+    conv_impl = {"auto": P.CONV_AUTO, "tcgen05": P.CONV_TCGEN05, "direct": P.CONV_DIRECT}[args.conv_impl]
+    desc = P.desc_from_spec(cfg.net, tile=cfg.tile, micro_batch=args.micro_batch, conv_impl=conv_impl,
+                            writeback_frames=cfg.writeback_batch)
+    loc = P.Localizer(desc, weights)
+    cap = int(n_frames * max(4 * cfg.frames.emitters_per_frame, 1024))
+    cap = min(cap, n_frames * ((H + 1) // 2) * ((W + 1) // 2))
+    off_map = torch.from_numpy(fs.offset_map).cuda() if fs.offset_map is not None else None
+    gain_map = torch.from_numpy(fs.gain_map).cuda() if fs.gain_map is not None else None
+    cam = loc.camera(fs.pixel_size_nm, fs.offset, fs.gain, off_map, gain_map)
+    frames_host = torch.from_numpy(frames).pin_memory()
+    frames_dev = frames_host.cuda()
+    out_dev = torch.zeros(cap * 32, dtype=torch.uint8, device="cuda")
+    out_host = torch.zeros(cap * 32, dtype=torch.uint8).pin_memory()
+    stream = torch.cuda.Stream()
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(frames_t, out_t, steps, conv_timing=False):
+        loc.conv_timing(conv_timing)
+        barrier()
+        l0 = loc.launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        counts = []
+        with torch.cuda.stream(stream):
+            e0.record(stream)
+            for _ in range(steps):
+                counts.append(loc.localize(frames_t, cam, cfg.threshold, out_t, cap, stream=stream))
+            e1.record(stream)
+        barrier()
+        ms = e0.elapsed_time(e1)
+        st = loc.check()
+        if st != P.OK:
+            raise SystemExit(f"smlm_check: {st} {loc.last_error()}")
+        conv_ms, conv_n = loc.conv_time_ms() if conv_timing else (0.0, 0)
+        loc.conv_timing(False)
+        return ms, [int(c.value) for c in counts], loc.launch_count() - l0, conv_ms, conv_n
+
+    # warm-up (device-resident and end-to-end paths)
+    timed(frames_dev, out_dev, args.warmup)
+    timed(frames_host, out_host, 1)
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    ms, counts, launches, conv_ms, conv_n = timed(frames_dev, out_dev, args.steps, conv_timing=True)
+    ms_e2e, counts_e2e, _, _, _ = timed(frames_host, out_host, args.steps)
+    sampler.stop_flag.set()
+    sampler.join(timeout=2)
+
+    t = torch.tensor([ms, ms_e2e], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max, ms_e2e_max = (float(v) for v in t.cpu())
+    total_frames = world * n_frames * args.steps
+    value = total_frames / (ms_max * 1e-3)
+    e2e_value = total_frames / (ms_e2e_max * 1e-3)
+    emitters = sum(counts)
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    peaks, peak_kind = load_peaks()
+    C, L = cfg.net.channels, cfg.net.n_layers
+    # dominant kernel: the dilated 3x3 conv layer (K2).  Algorithmic work per launch =
+    # 18 C^2 FLOP per pixel per layer x the pixels one launch processes.
+    flop_total = 18.0 * C * C * H * W * n_frames * L * args.steps
+    roofline = None
+    if conv_n > 0 and conv_ms > 0 and cfg.tile == 0:
+        achieved = flop_total / (conv_ms * 1e-3) / 1e12
+        peak = float(peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]))
+        bound = "tensor"
+        if cfg.net.precision != "bf16" or args.conv_impl == "direct":
+            bound = "alu"
+        roofline = {"bound": bound, "kernel": "conv3x3_dilated (K2)", "achieved": achieved, "peak": peak,
+                    "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+                    "peak_source": f"{peak_kind} bf16_tflops_sustained (kernel timed inside a long step)",
+                    "frac_of_burst": achieved / float(peaks["bf16_tflops"]),
+                    "launches": conv_n, "avg_launch_ms": conv_ms / conv_n,
+                    "share_of_step": conv_ms / ms}
+    cpu = None
+    if not args.no_cpu_baseline:
+        ns = 4 if H * W <= 256 * 256 else 1
+        fps, eps, cores, dt = oracle_sample(cfg, fs, weights, ns)
+        cpu = {"value": fps, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"first {ns} frame(s) of {cfg.name}, {dt:.1f} s", "emitters_per_s": eps}
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None,
+        "dtype": "bf16" if cfg.net.precision == "bf16" else "f32", "data": "synthetic",
+        "config": {"workload": cfg.name, "frames_per_step": n_frames, "H": H, "W": W, "channels": C,
+                   "layers": L, "head_channels": cfg.net.head_channels, "tile": cfg.tile,
+                   "distinct_frames": min(DISTINCT_FRAMES, n_frames), "conv_impl": args.conv_impl,
+                   "l2": "inputs larger than L2 (u16 stack + activation stream per step > 126 MB)",
+                   "parallelism": f"replicas x{world}"},
+        "emitters_per_s": world * emitters / (ms_max * 1e-3),
+        "emitters_per_frame": emitters / (n_frames * args.steps),
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(frames.nbytes),
+                "d2h_bytes_per_step": int(counts_e2e[-1] * 32 + 8), "ms_per_step": ms_e2e_max / args.steps,
+                "exposed_copy_ms_per_step": (ms_e2e_max - ms_max) / args.steps},
+        "gpu_launches": launches,
+        "clocks": sampler.summary(),
+        "roofline": roofline,
+        "cpu_baseline": cpu,
+        "tensor_frac_whole_step": (cfg.net.flop_per_px() * H * W * n_frames * args.steps / (ms_max * 1e-3) / 1e12)
+                                  / float(peaks["bf16_tflops"]),
+    }
+    print(json.dumps(line), flush=True)
+    loc.close()
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

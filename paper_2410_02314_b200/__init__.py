@@ -1,0 +1,12 @@
+"""B200-native (sm_100a) hot path of arXiv 2410.02314: DilatedLoc-style inference over stacks
+of single-molecule frames plus on-GPU post-processing, as a C-ABI library
+(include/smlm.h) with a thin ctypes binding.  See DESIGN.md."""
+from .binding import (ABI_VERSION, BF16, CONV_AUTO, CONV_DIRECT, CONV_TCGEN05, EMITTER_DTYPE,
+                      ERR_CUDA, ERR_INVALID_ARG, ERR_OOM, ERR_OVERFLOW, ERR_UNSUPPORTED_DEVICE,
+                      EXPORTS, FP32, OK, CameraParams, Localizer, NetDesc, SmlmError,
+                      desc_from_spec, emitters_to_numpy, lib, make_desc)
+
+__all__ = ["ABI_VERSION", "BF16", "CONV_AUTO", "CONV_DIRECT", "CONV_TCGEN05", "EMITTER_DTYPE",
+           "ERR_CUDA", "ERR_INVALID_ARG", "ERR_OOM", "ERR_OVERFLOW", "ERR_UNSUPPORTED_DEVICE",
+           "EXPORTS", "FP32", "OK", "CameraParams", "Localizer", "NetDesc", "SmlmError",
+           "desc_from_spec", "emitters_to_numpy", "lib", "make_desc"]

@@ -1,0 +1,723 @@
+// C ABI of libsmlm_b200 (include/smlm.h) and the pipeline around the kernels:
+// pinned host ring -> copy stream -> staging slots -> compute stream (K1, K2 x L, K3) ->
+// write-back stream.  Enqueue only: no host synchronisation inside smlm_localize.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "smlm_internal.cuh"
+
+using namespace smlm;
+
+namespace {
+
+constexpr int kSlots = 3;  // staging slots of the preload ring (copy k+1, k+2 while k computes)
+
+thread_local std::string g_create_error;
+
+uint16_t f32_to_bf16_bits(float f) {  // round to nearest even
+  uint32_t u;
+  std::memcpy(&u, &f, 4);
+  if ((u & 0x7fffffffu) > 0x7f800000u) return (uint16_t)((u >> 16) | 0x40);
+  u += 0x7fffu + ((u >> 16) & 1u);
+  return (uint16_t)(u >> 16);
+}
+float bf16_round(float f) {
+  uint32_t u = (uint32_t)f32_to_bf16_bits(f) << 16;
+  float r;
+  std::memcpy(&r, &u, 4);
+  return r;
+}
+
+struct Layer {
+  float* w_direct = nullptr;  // [9][C][C] (tap, ci, co)
+  void* w_umma = nullptr;     // packed bf16 image for conv_umma
+  float* bias = nullptr;
+  int dil = 1;
+};
+
+struct PlanEntry {
+  const void* b0;
+  const void* b1;
+  ActShape s;
+  UmmaPlan* plan;
+};
+
+}  // namespace
+
+struct smlm_ctx {
+  smlm_net_desc d{};
+  bool bf16 = false;
+  bool use_umma = false;
+  int n_sm = 0;
+  int radius = 0;  // receptive-field radius of the maps: 1 + sum(dilations)
+  size_t l2_bytes = 0;
+
+  float *w_stem = nullptr, *b_stem = nullptr, *w_head = nullptr, *b_head = nullptr;
+  std::vector<Layer> layers;
+
+  void* act[2] = {nullptr, nullptr};
+  size_t act_bytes = 0;
+  std::vector<PlanEntry> plans;
+
+  uint16_t* slots = nullptr;  // kSlots x slot_elems
+  size_t slot_elems = 0;
+  bool slot_used[kSlots] = {false, false, false};
+  cudaEvent_t ev_copied[kSlots]{}, ev_consumed[kSlots]{};
+  cudaEvent_t ev_start = nullptr, ev_batch = nullptr, ev_wb = nullptr;
+  cudaStream_t copy_stream = nullptr, wb_stream = nullptr;
+
+  smlm_emitter* em_dev = nullptr;
+  size_t em_cap = 0;
+  unsigned long long* counters = nullptr;  // [0] count, [1] snapshot, [2] flushed
+  unsigned long long* h_count = nullptr;   // pinned, for smlm_check
+  unsigned long long last_capacity = 0;
+
+  float *cam_off = nullptr, *cam_gain = nullptr;
+  size_t cam_elems = 0;
+
+  int64_t launches = 0;
+  bool conv_timing = false;
+  std::vector<cudaEvent_t> tev;  // pairs
+  size_t tev_used = 0;
+
+  std::string err;
+};
+
+namespace {
+
+smlm_status fail(smlm_ctx* c, smlm_status st, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof buf, fmt, ap);
+  va_end(ap);
+  if (c) c->err = buf;
+  else g_create_error = buf;
+  return st;
+}
+
+#define CK(c, call)                                                                          \
+  do {                                                                                       \
+    cudaError_t e_ = (call);                                                                 \
+    if (e_ != cudaSuccess)                                                                   \
+      return fail(c, e_ == cudaErrorMemoryAllocation ? SMLM_ERR_OOM : SMLM_ERR_CUDA,          \
+                  "%s: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__);      \
+  } while (0)
+
+enum PtrKind { PTR_DEVICE, PTR_HOST_PINNED, PTR_OTHER };
+PtrKind classify(const void* p) {
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, p) != cudaSuccess) {
+    cudaGetLastError();
+    return PTR_OTHER;
+  }
+  if (a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged) return PTR_DEVICE;
+  if (a.type == cudaMemoryTypeHost) return PTR_HOST_PINNED;
+  return PTR_OTHER;
+}
+
+void free_plans(smlm_ctx* c) {
+  for (auto& p : c->plans) umma_plan_destroy(p.plan);
+  c->plans.clear();
+}
+
+smlm_status ensure_act(smlm_ctx* c, size_t bytes) {
+  if (bytes <= c->act_bytes) return SMLM_OK;
+  free_plans(c);
+  for (int i = 0; i < 2; ++i) {
+    if (c->act[i]) cudaFree(c->act[i]);
+    c->act[i] = nullptr;
+  }
+  c->act_bytes = 0;
+  for (int i = 0; i < 2; ++i) CK(c, cudaMalloc(&c->act[i], bytes));
+  c->act_bytes = bytes;
+  return SMLM_OK;
+}
+
+smlm_status get_plan(smlm_ctx* c, ActShape s, UmmaPlan** out) {
+  for (auto& p : c->plans)
+    if (p.b0 == c->act[0] && p.b1 == c->act[1] && p.s.B == s.B && p.s.C == s.C && p.s.H == s.H &&
+        p.s.W == s.W) {
+      *out = p.plan;
+      return SMLM_OK;
+    }
+  char err[256] = {0};
+  UmmaPlan* pl = umma_plan_create(c->act[0], c->act[1], s, c->n_sm, err, sizeof err);
+  if (!pl) return fail(c, SMLM_ERR_CUDA, "tcgen05 plan: %s", err);
+  if (c->plans.size() > 64) free_plans(c);
+  c->plans.push_back({c->act[0], c->act[1], s, pl});
+  *out = pl;
+  return SMLM_OK;
+}
+
+// K1 -> K2 x L for one launch set; the result is in act[*result_buf].
+smlm_status run_trunk(smlm_ctx* c, const uint16_t* dev_frames, int frame_base, const ViewSet& vs,
+                      ActShape s, const NormParams& np, cudaStream_t st, int* result_buf,
+                      float* trunk_dump, size_t dump_view_stride, size_t dump_level_stride,
+                      cudaEvent_t after_stem) {
+  CK(c, launch_stem(c->bf16, dev_frames, frame_base, vs, s, np, c->w_stem, c->b_stem,
+                    c->d.stem_relu, c->act[0], st));
+  c->launches++;
+  if (after_stem) CK(c, cudaEventRecord(after_stem, st));
+  int cur = 0;
+  if (trunk_dump) {
+    CK(c, launch_dump_act(c->bf16, c->act[0], s, trunk_dump, dump_view_stride, st));
+    c->launches++;
+  }
+  UmmaPlan* plan = nullptr;
+  if (c->use_umma && !c->layers.empty()) {
+    smlm_status r = get_plan(c, s, &plan);
+    if (r != SMLM_OK) return r;
+  }
+  for (size_t l = 0; l < c->layers.size(); ++l) {
+    const Layer& L = c->layers[l];
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    if (c->conv_timing) {
+      if (c->tev_used + 2 > c->tev.size()) {
+        for (int i = 0; i < 2; ++i) {
+          cudaEvent_t e;
+          CK(c, cudaEventCreate(&e));
+          c->tev.push_back(e);
+        }
+      }
+      e0 = c->tev[c->tev_used++];
+      e1 = c->tev[c->tev_used++];
+      CK(c, cudaEventRecord(e0, st));
+    }
+    if (c->use_umma) {
+      char err[256] = {0};
+      cudaError_t e = launch_conv_umma(plan, cur, L.dil, L.w_umma, L.bias, 0, st, err, sizeof err);
+      if (e != cudaSuccess)
+        return fail(c, SMLM_ERR_CUDA, "conv_umma: %s %s", cudaGetErrorString(e), err);
+    } else {
+      CK(c, launch_conv_direct(c->bf16, c->act[cur], c->act[cur ^ 1], s, L.dil, L.w_direct, L.bias, st));
+    }
+    c->launches++;
+    if (e1) CK(c, cudaEventRecord(e1, st));
+    cur ^= 1;
+    if (trunk_dump) {
+      CK(c, launch_dump_act(c->bf16, c->act[cur], s, trunk_dump + (l + 1) * dump_level_stride,
+                            dump_view_stride, st));
+      c->launches++;
+    }
+  }
+  *result_buf = cur;
+  return SMLM_OK;
+}
+
+smlm_status setup_camera(smlm_ctx* c, const smlm_camera_params* cam, int H, int W, cudaStream_t st,
+                         NormParams* np) {
+  np->offset = cam->offset;
+  np->gain = cam->gain;
+  np->norm_scale = c->d.norm_scale;
+  np->offset_map = nullptr;
+  np->gain_map = nullptr;
+  if ((cam->offset_map == nullptr) != (cam->gain_map == nullptr))
+    return fail(c, SMLM_ERR_INVALID_ARG, "offset_map and gain_map must both be given or both be NULL");
+  if (!cam->offset_map) {
+    if (!(cam->gain > 0.0f)) return fail(c, SMLM_ERR_INVALID_ARG, "camera gain must be > 0");
+    return SMLM_OK;
+  }
+  size_t n = (size_t)H * W;
+  const float* src[2] = {cam->offset_map, cam->gain_map};
+  const float* dst[2] = {nullptr, nullptr};
+  bool need_copy = classify(src[0]) != PTR_DEVICE || classify(src[1]) != PTR_DEVICE;
+  if (need_copy) {
+    if (n > c->cam_elems) {
+      if (c->cam_off) cudaFree(c->cam_off);
+      if (c->cam_gain) cudaFree(c->cam_gain);
+      c->cam_off = c->cam_gain = nullptr;
+      c->cam_elems = 0;
+      CK(c, cudaMalloc(&c->cam_off, n * sizeof(float)));
+      CK(c, cudaMalloc(&c->cam_gain, n * sizeof(float)));
+      c->cam_elems = n;
+    }
+    CK(c, cudaMemcpyAsync(c->cam_off, src[0], n * sizeof(float), cudaMemcpyDefault, st));
+    CK(c, cudaMemcpyAsync(c->cam_gain, src[1], n * sizeof(float), cudaMemcpyDefault, st));
+    dst[0] = c->cam_off;
+    dst[1] = c->cam_gain;
+  } else {
+    dst[0] = src[0];
+    dst[1] = src[1];
+  }
+  np->offset_map = dst[0];
+  np->gain_map = dst[1];
+  return SMLM_OK;
+}
+
+HeadParams head_params(const smlm_ctx* c, const smlm_camera_params* cam, float threshold) {
+  HeadParams hp;
+  hp.n_h = c->d.head_channels;
+  if (threshold <= 0.0f) hp.lthr = -INFINITY;
+  else if (threshold >= 1.0f) hp.lthr = INFINITY;
+  else hp.lthr = (float)std::log((double)threshold / (1.0 - (double)threshold));
+  hp.xy_scale = c->d.xy_scale;
+  hp.z_scale_nm = c->d.z_scale_nm;
+  hp.photon_scale = c->d.photon_scale;
+  hp.bg_scale = c->d.bg_scale;
+  hp.pixel_size_nm = cam->pixel_size_nm;
+  return hp;
+}
+
+// contiguous ranges of tile indices whose windows have the same extent
+struct Range { int t0, n, ext; };
+std::vector<Range> tile_classes(int F, int tile, int halo) {
+  std::vector<Range> out;
+  int T = (F + tile - 1) / tile;
+  for (int t = 0; t < T; ++t) {
+    int lo = std::max(0, t * tile - halo), hi = std::min(F, (t + 1) * tile + halo);
+    int ext = hi - lo;
+    if (!out.empty() && out.back().ext == ext) out.back().n++;
+    else out.push_back({t, 1, ext});
+  }
+  return out;
+}
+
+size_t elt_size(const smlm_ctx* c) { return c->bf16 ? 2 : 4; }
+
+// out_count may be pageable host memory: a D2H copy into it would block the host, so the
+// count goes to the ctx's pinned word and a stream-ordered host function forwards it.
+struct CountCopy { int64_t* dst; const unsigned long long* src; };
+void CUDART_CB count_cb(void* p) {
+  CountCopy* cc = static_cast<CountCopy*>(p);
+  *cc->dst = (int64_t)*cc->src;
+  delete cc;
+}
+smlm_status store_count(smlm_ctx* c, const unsigned long long* counter, int64_t* out_count,
+                        cudaStream_t st) {
+  CK(c, cudaMemcpyAsync(c->h_count, counter, sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+  CountCopy* cc = new (std::nothrow) CountCopy{out_count, c->h_count};
+  if (!cc) return fail(c, SMLM_ERR_OOM, "host allocation failed");
+  cudaError_t e = cudaLaunchHostFunc(st, count_cb, cc);
+  if (e != cudaSuccess) {
+    delete cc;
+    return fail(c, SMLM_ERR_CUDA, "cudaLaunchHostFunc: %s", cudaGetErrorString(e));
+  }
+  return SMLM_OK;
+}
+
+int auto_micro_batch(const smlm_ctx* c, int Hw, int Ww) {
+  if (c->d.micro_batch > 0) return c->d.micro_batch;
+  // keep the two ping-pong maps of a micro-batch inside ~3/4 of L2 (bf16: 2C B/px each)
+  size_t per_view = (size_t)Hw * Ww * c->d.channels * elt_size(c);
+  size_t budget = c->l2_bytes ? c->l2_bytes * 3 / 8 : (size_t)48 << 20;
+  size_t b = budget / std::max<size_t>(per_view, 1);
+  return (int)std::min<size_t>(std::max<size_t>(b, 1), 64);
+}
+
+}  // namespace
+
+extern "C" {
+
+smlm_status smlm_create(const smlm_net_desc* desc, const void* weights, smlm_ctx** out_ctx) {
+  if (out_ctx) *out_ctx = nullptr;
+  if (!desc || !weights || !out_ctx) return fail(nullptr, SMLM_ERR_INVALID_ARG, "NULL argument");
+  if (desc->struct_size != sizeof(smlm_net_desc) || desc->version != SMLM_ABI_VERSION)
+    return fail(nullptr, SMLM_ERR_INVALID_ARG, "smlm_net_desc size/version mismatch");
+  const int C = desc->channels, L = desc->n_layers, nh = desc->head_channels;
+  if (C < 16 || C > 64 || C % 16) return fail(nullptr, SMLM_ERR_INVALID_ARG, "channels must be 16, 32, 48 or 64");
+  if (L < 0 || L > SMLM_MAX_LAYERS) return fail(nullptr, SMLM_ERR_INVALID_ARG, "n_layers out of range");
+  if (nh != 5 && nh != 6) return fail(nullptr, SMLM_ERR_INVALID_ARG, "head_channels must be 5 or 6");
+  if (desc->precision != SMLM_FP32 && desc->precision != SMLM_BF16)
+    return fail(nullptr, SMLM_ERR_INVALID_ARG, "bad precision");
+  if (desc->conv_impl < SMLM_CONV_AUTO || desc->conv_impl > SMLM_CONV_DIRECT)
+    return fail(nullptr, SMLM_ERR_INVALID_ARG, "bad conv_impl");
+  if (desc->precision == SMLM_FP32 && desc->conv_impl == SMLM_CONV_TCGEN05)
+    return fail(nullptr, SMLM_ERR_INVALID_ARG, "the tcgen05 kernel is bf16 only");
+  for (int l = 0; l < L; ++l)
+    if (desc->dilations[l] < 1 || desc->dilations[l] > 8)
+      return fail(nullptr, SMLM_ERR_INVALID_ARG, "dilations must be in 1..8");
+  if (!(desc->norm_scale > 0.0f)) return fail(nullptr, SMLM_ERR_INVALID_ARG, "norm_scale must be > 0");
+  if (desc->tile < 0 || desc->micro_batch < 0 || desc->writeback_frames < 0)
+    return fail(nullptr, SMLM_ERR_INVALID_ARG, "negative tile / micro_batch / writeback_frames");
+
+  int dev = 0;
+  cudaDeviceProp prop;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+    cudaGetLastError();
+    return fail(nullptr, SMLM_ERR_UNSUPPORTED_DEVICE, "no CUDA device");
+  }
+  if (prop.major != 10)
+    return fail(nullptr, SMLM_ERR_UNSUPPORTED_DEVICE, "device %s is sm_%d%d; this library is sm_100a only",
+                prop.name, prop.major, prop.minor);
+
+  smlm_ctx* c = new (std::nothrow) smlm_ctx;
+  if (!c) return fail(nullptr, SMLM_ERR_OOM, "host allocation failed");
+  c->d = *desc;
+  c->bf16 = desc->precision == SMLM_BF16;
+  c->use_umma = c->bf16 && desc->conv_impl != SMLM_CONV_DIRECT;
+  c->n_sm = prop.multiProcessorCount;
+  c->l2_bytes = (size_t)prop.l2CacheSize;
+  c->radius = 1;
+  for (int l = 0; l < L; ++l) c->radius += desc->dilations[l];
+
+  smlm_status st = SMLM_OK;
+  auto upload = [&](const std::vector<float>& h, float** d) -> smlm_status {
+    CK(nullptr, cudaMalloc(d, h.size() * sizeof(float)));
+    CK(nullptr, cudaMemcpy(*d, h.data(), h.size() * sizeof(float), cudaMemcpyHostToDevice));
+    return SMLM_OK;
+  };
+  auto body = [&]() -> smlm_status {
+    const float* w = static_cast<const float*>(weights);
+    std::vector<float> tmp(9 * C);
+    for (int co = 0; co < C; ++co)
+      for (int t = 0; t < 9; ++t) tmp[t * C + co] = w[co * 9 + t];
+    if ((st = upload(tmp, &c->w_stem)) != SMLM_OK) return st;
+    if ((st = upload(std::vector<float>(w + 9 * C, w + 10 * C), &c->b_stem)) != SMLM_OK) return st;
+    w += 10 * C;
+    c->layers.resize(L);
+    std::vector<float> wd((size_t)9 * C * C);
+    std::vector<uint8_t> pack(c->use_umma ? umma_packed_weight_bytes(C) : 0);
+    for (int l = 0; l < L; ++l) {
+      Layer& Ly = c->layers[l];
+      Ly.dil = desc->dilations[l];
+      for (int co = 0; co < C; ++co)
+        for (int ci = 0; ci < C; ++ci)
+          for (int t = 0; t < 9; ++t) {
+            float v = w[((size_t)co * C + ci) * 9 + t];
+            wd[((size_t)t * C + ci) * C + co] = c->bf16 ? bf16_round(v) : v;
+          }
+      if ((st = upload(wd, &Ly.w_direct)) != SMLM_OK) return st;
+      if ((st = upload(std::vector<float>(w + (size_t)9 * C * C, w + (size_t)9 * C * C + C), &Ly.bias)) != SMLM_OK)
+        return st;
+      if (c->use_umma) {
+        umma_pack_weights_host(C, w, pack.data());
+        CK(nullptr, cudaMalloc(&Ly.w_umma, pack.size()));
+        CK(nullptr, cudaMemcpy(Ly.w_umma, pack.data(), pack.size(), cudaMemcpyHostToDevice));
+      }
+      w += (size_t)9 * C * C + C;
+    }
+    if ((st = upload(std::vector<float>(w, w + nh * C), &c->w_head)) != SMLM_OK) return st;
+    if ((st = upload(std::vector<float>(w + nh * C, w + nh * C + nh), &c->b_head)) != SMLM_OK) return st;
+    CK(nullptr, conv_direct_init(C));
+    CK(nullptr, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+    CK(nullptr, cudaStreamCreateWithFlags(&c->wb_stream, cudaStreamNonBlocking));
+    for (int i = 0; i < kSlots; ++i) {
+      CK(nullptr, cudaEventCreateWithFlags(&c->ev_copied[i], cudaEventDisableTiming));
+      CK(nullptr, cudaEventCreateWithFlags(&c->ev_consumed[i], cudaEventDisableTiming));
+    }
+    CK(nullptr, cudaEventCreateWithFlags(&c->ev_start, cudaEventDisableTiming));
+    CK(nullptr, cudaEventCreateWithFlags(&c->ev_batch, cudaEventDisableTiming));
+    CK(nullptr, cudaEventCreateWithFlags(&c->ev_wb, cudaEventDisableTiming));
+    CK(nullptr, cudaMalloc(&c->counters, 4 * sizeof(unsigned long long)));
+    CK(nullptr, cudaMemset(c->counters, 0, 4 * sizeof(unsigned long long)));
+    CK(nullptr, cudaMallocHost(&c->h_count, sizeof(unsigned long long)));
+    *c->h_count = 0;
+    return SMLM_OK;
+  };
+  st = body();
+  if (st != SMLM_OK) {
+    smlm_destroy(c);
+    return st;
+  }
+  *out_ctx = c;
+  return SMLM_OK;
+}
+
+void smlm_destroy(smlm_ctx* c) {
+  if (!c) return;
+  cudaDeviceSynchronize();
+  free_plans(c);
+  cudaFree(c->w_stem); cudaFree(c->b_stem); cudaFree(c->w_head); cudaFree(c->b_head);
+  for (auto& L : c->layers) { cudaFree(L.w_direct); cudaFree(L.w_umma); cudaFree(L.bias); }
+  cudaFree(c->act[0]); cudaFree(c->act[1]); cudaFree(c->slots); cudaFree(c->em_dev);
+  cudaFree(c->counters); cudaFree(c->cam_off); cudaFree(c->cam_gain);
+  if (c->h_count) cudaFreeHost(c->h_count);
+  for (int i = 0; i < kSlots; ++i) {
+    if (c->ev_copied[i]) cudaEventDestroy(c->ev_copied[i]);
+    if (c->ev_consumed[i]) cudaEventDestroy(c->ev_consumed[i]);
+  }
+  if (c->ev_start) cudaEventDestroy(c->ev_start);
+  if (c->ev_batch) cudaEventDestroy(c->ev_batch);
+  if (c->ev_wb) cudaEventDestroy(c->ev_wb);
+  for (auto e : c->tev) cudaEventDestroy(e);
+  if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+  if (c->wb_stream) cudaStreamDestroy(c->wb_stream);
+  cudaGetLastError();
+  delete c;
+}
+
+const char* smlm_last_error(const smlm_ctx* c) { return c ? c->err.c_str() : g_create_error.c_str(); }
+
+int64_t smlm_launch_count(const smlm_ctx* c) { return c ? c->launches : 0; }
+
+smlm_status smlm_conv_timing(smlm_ctx* c, int32_t enable) {
+  if (!c) return SMLM_ERR_INVALID_ARG;
+  c->conv_timing = enable != 0;
+  c->tev_used = 0;
+  return SMLM_OK;
+}
+
+smlm_status smlm_conv_time_ms(smlm_ctx* c, double* total_ms, int64_t* launches) {
+  if (!c || !total_ms || !launches) return SMLM_ERR_INVALID_ARG;
+  double tot = 0.0;
+  for (size_t i = 0; i + 1 < c->tev_used; i += 2) {
+    CK(c, cudaEventSynchronize(c->tev[i + 1]));
+    float ms = 0.f;
+    CK(c, cudaEventElapsedTime(&ms, c->tev[i], c->tev[i + 1]));
+    tot += ms;
+  }
+  *total_ms = tot;
+  *launches = (int64_t)(c->tev_used / 2);
+  c->tev_used = 0;
+  return SMLM_OK;
+}
+
+smlm_status smlm_check(smlm_ctx* c) {
+  if (!c) return SMLM_ERR_INVALID_ARG;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(c, SMLM_ERR_CUDA, "pending CUDA error: %s", cudaGetErrorString(e));
+  if (*c->h_count > c->last_capacity)
+    return fail(c, SMLM_ERR_OVERFLOW, "found %llu emitters, capacity %llu", *c->h_count, c->last_capacity);
+  return SMLM_OK;
+}
+
+smlm_status smlm_localize(smlm_ctx* c, const uint16_t* frames, int64_t n, int32_t H, int32_t W,
+                          const smlm_camera_params* cam, float threshold, smlm_emitter* out,
+                          int64_t* out_count, void* cuda_stream) {
+  if (!c) return SMLM_ERR_INVALID_ARG;
+  if (!cam || !out_count) return fail(c, SMLM_ERR_INVALID_ARG, "NULL camera / out_count");
+  if (n < 0 || H < 1 || W < 1 || (int64_t)H * W > (int64_t)1 << 30 || n > INT32_MAX)
+    return fail(c, SMLM_ERR_INVALID_ARG, "bad n_frames / H / W");
+  if (*out_count < 0) return fail(c, SMLM_ERR_INVALID_ARG, "negative capacity");
+  if (!(threshold == threshold)) return fail(c, SMLM_ERR_INVALID_ARG, "threshold is NaN");
+  if (!(cam->pixel_size_nm > 0.0f)) return fail(c, SMLM_ERR_INVALID_ARG, "pixel_size_nm must be > 0");
+  const unsigned long long capacity = (unsigned long long)*out_count;
+  if (capacity > 0 && !out) return fail(c, SMLM_ERR_INVALID_ARG, "NULL out_emitters with capacity > 0");
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+
+  PtrKind fk = PTR_DEVICE;
+  if (n > 0) {
+    if (!frames) return fail(c, SMLM_ERR_INVALID_ARG, "NULL frames");
+    fk = classify(frames);
+    if (fk == PTR_OTHER)
+      return fail(c, SMLM_ERR_INVALID_ARG,
+                  "frames_u16 must be pinned host memory (the preload ring) or device memory");
+  }
+  PtrKind ok = PTR_DEVICE;
+  if (capacity > 0) {
+    ok = classify(out);
+    if (ok == PTR_OTHER)
+      return fail(c, SMLM_ERR_INVALID_ARG, "out_emitters must be device or pinned host memory");
+  }
+
+  NormParams np;
+  smlm_status r = setup_camera(c, cam, H, W, st, &np);
+  if (r != SMLM_OK) return r;
+  const HeadParams hp = head_params(c, cam, threshold);
+  const int C = c->d.channels;
+
+  // ---- geometry: launch sets (all views of a set share one window size)
+  const int tile = c->d.tile;
+  const bool tiled = tile > 0 && (tile < H || tile < W);
+  const int halo = c->radius + 1;  // maps need `radius`; the 3x3 test reads one more pixel
+  std::vector<Range> ycls, xcls;
+  if (tiled) {
+    ycls = tile_classes(H, tile, halo);
+    xcls = tile_classes(W, tile, halo);
+  } else {
+    ycls.push_back({0, 1, H});
+    xcls.push_back({0, 1, W});
+  }
+  int maxHw = 0, maxWw = 0;
+  for (auto& a : ycls) maxHw = std::max(maxHw, a.ext);
+  for (auto& a : xcls) maxWw = std::max(maxWw, a.ext);
+  const int mb = auto_micro_batch(c, maxHw, maxWw);   // views per launch
+  const int F = tiled ? 1 : mb;                        // frames per chunk
+  size_t need = 0;
+  for (auto& a : ycls)
+    for (auto& b : xcls) {
+      int nv = tiled ? std::min(mb, a.n * b.n) : (int)std::min<int64_t>(mb, std::max<int64_t>(n, 1));
+      need = std::max(need, (size_t)nv * a.ext * b.ext * C * elt_size(c));
+    }
+  if ((r = ensure_act(c, need)) != SMLM_OK) return r;
+
+  const size_t frame_elems = (size_t)H * W;
+  if (fk == PTR_HOST_PINNED && n > 0) {
+    size_t se = (size_t)std::min<int64_t>(F, n) * frame_elems;
+    if (se > c->slot_elems) {
+      CK(c, cudaDeviceSynchronize());  // a previous call may still read the old slots
+      if (c->slots) cudaFree(c->slots);
+      c->slots = nullptr;
+      c->slot_elems = 0;
+      CK(c, cudaMalloc(&c->slots, kSlots * se * sizeof(uint16_t)));
+      c->slot_elems = se;
+      for (int i = 0; i < kSlots; ++i) c->slot_used[i] = false;
+    }
+  }
+  smlm_emitter* list = out;
+  if (ok == PTR_HOST_PINNED && capacity > 0) {
+    if (capacity > c->em_cap) {
+      CK(c, cudaDeviceSynchronize());
+      if (c->em_dev) cudaFree(c->em_dev);
+      c->em_dev = nullptr;
+      c->em_cap = 0;
+      CK(c, cudaMalloc(&c->em_dev, capacity * sizeof(smlm_emitter)));
+      c->em_cap = capacity;
+    }
+    list = c->em_dev;
+  }
+  unsigned long long* counter = c->counters;
+  unsigned long long* snap = c->counters + 1;
+  unsigned long long* flushed = c->counters + 2;
+  CK(c, cudaMemsetAsync(c->counters, 0, 4 * sizeof(unsigned long long), st));
+  c->last_capacity = capacity;
+
+  if (fk == PTR_HOST_PINNED) {
+    CK(c, cudaEventRecord(c->ev_start, st));
+    CK(c, cudaStreamWaitEvent(c->copy_stream, c->ev_start, 0));
+  }
+  const bool host_out = (ok == PTR_HOST_PINNED && capacity > 0);
+  const int wbf = c->d.writeback_frames;
+  bool wb_pending = false;
+  auto flush = [&]() -> smlm_status {
+    // records below the snapshot are complete: every K3 that wrote them precedes it on `st`
+    CK(c, launch_snapshot(counter, capacity, snap, st));
+    CK(c, cudaEventRecord(c->ev_batch, st));
+    CK(c, cudaStreamWaitEvent(c->wb_stream, c->ev_batch, 0));
+    CK(c, launch_flush_emitters(list, out, snap, flushed, c->wb_stream));
+    CK(c, cudaEventRecord(c->ev_wb, c->wb_stream));
+    c->launches += 3;
+    wb_pending = true;
+    return SMLM_OK;
+  };
+
+  int64_t chunk = 0;
+  for (int64_t f0 = 0; f0 < n; f0 += F, ++chunk) {
+    const int nf = (int)std::min<int64_t>(F, n - f0);
+    const uint16_t* dev_frames = frames;
+    int frame_base = 0;
+    int slot = -1;
+    if (fk == PTR_HOST_PINNED) {
+      // P1: the preload ring.  Copy chunk k into slot k % kSlots on the copy stream as soon
+      // as the stem of chunk k - kSlots has consumed it; compute waits for the copy only.
+      slot = (int)(chunk % kSlots);
+      if (c->slot_used[slot]) CK(c, cudaStreamWaitEvent(c->copy_stream, c->ev_consumed[slot], 0));
+      uint16_t* dst = c->slots + (size_t)slot * c->slot_elems;
+      CK(c, cudaMemcpyAsync(dst, frames + (size_t)f0 * frame_elems, (size_t)nf * frame_elems * 2,
+                            cudaMemcpyHostToDevice, c->copy_stream));
+      CK(c, cudaEventRecord(c->ev_copied[slot], c->copy_stream));
+      CK(c, cudaStreamWaitEvent(st, c->ev_copied[slot], 0));
+      c->slot_used[slot] = true;
+      dev_frames = dst;
+      frame_base = (int)f0;
+    }
+    // launch sets of this chunk
+    struct Set { ViewSet vs; ActShape s; };
+    std::vector<Set> sets;
+    if (!tiled) {
+      ViewSet vs{(int)f0, H, W, 0, 0, 0, 1, 0, 1};
+      sets.push_back({vs, ActShape{nf, C, H, W}});
+    } else {
+      for (auto& a : ycls)
+        for (auto& b : xcls) {
+          // split the class into sub-blocks of at most mb views
+          int bx = std::min(b.n, mb), by = std::max(1, std::min(a.n, mb / bx));
+          for (int ty = a.t0; ty < a.t0 + a.n; ty += by)
+            for (int tx = b.t0; tx < b.t0 + b.n; tx += bx) {
+              int ny = std::min(by, a.t0 + a.n - ty), nx = std::min(bx, b.t0 + b.n - tx);
+              ViewSet vs{(int)f0, H, W, tile, halo, ty, ny, tx, nx};
+              sets.push_back({vs, ActShape{ny * nx, C, a.ext, b.ext}});
+            }
+        }
+    }
+    for (size_t si = 0; si < sets.size(); ++si) {
+      int res = 0;
+      cudaEvent_t after_stem = (slot >= 0 && si + 1 == sets.size()) ? c->ev_consumed[slot] : nullptr;
+      r = run_trunk(c, dev_frames, frame_base, sets[si].vs, sets[si].s, np, st, &res, nullptr, 0, 0,
+                    after_stem);
+      if (r != SMLM_OK) return r;
+      CK(c, launch_head_post(c->bf16, c->act[res], sets[si].s, sets[si].vs, c->w_head, c->b_head, hp,
+                             list, counter, capacity, st));
+      c->launches++;
+    }
+    if (host_out && wbf > 0) {
+      int64_t done = f0 + nf;
+      if (done < n && done / wbf != f0 / wbf) {
+        if ((r = flush()) != SMLM_OK) return r;
+      }
+    }
+  }
+  if (host_out) {
+    if ((r = flush()) != SMLM_OK) return r;
+  }
+  if (wb_pending) CK(c, cudaStreamWaitEvent(st, c->ev_wb, 0));
+  return store_count(c, counter, out_count, st);
+}
+
+smlm_status smlm_debug_forward_maps(smlm_ctx* c, const uint16_t* frames, int64_t n, int32_t H,
+                                    int32_t W, const smlm_camera_params* cam, float* maps,
+                                    float* trunk, void* cuda_stream) {
+  if (!c) return SMLM_ERR_INVALID_ARG;
+  if (!cam || !maps || (n > 0 && !frames) || n < 0 || H < 1 || W < 1 || n > INT32_MAX)
+    return fail(c, SMLM_ERR_INVALID_ARG, "bad argument");
+  if (classify(maps) != PTR_DEVICE || (trunk && classify(trunk) != PTR_DEVICE))
+    return fail(c, SMLM_ERR_INVALID_ARG, "maps / trunk must be device memory");
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  PtrKind fk = n > 0 ? classify(frames) : PTR_DEVICE;
+  if (fk == PTR_OTHER) return fail(c, SMLM_ERR_INVALID_ARG, "frames must be pinned host or device memory");
+  NormParams np;
+  smlm_status r = setup_camera(c, cam, H, W, st, &np);
+  if (r != SMLM_OK) return r;
+  const int C = c->d.channels, L = c->d.n_layers, nh = c->d.head_channels;
+  const int mb = auto_micro_batch(c, H, W);
+  const size_t px = (size_t)H * W;
+  if ((r = ensure_act(c, (size_t)std::min<int64_t>(mb, std::max<int64_t>(n, 1)) * px * C * elt_size(c))) != SMLM_OK)
+    return r;
+  uint16_t* tmp = nullptr;
+  if (fk == PTR_HOST_PINNED && n > 0) {
+    CK(c, cudaMalloc(&tmp, (size_t)n * px * 2));
+    CK(c, cudaMemcpyAsync(tmp, frames, (size_t)n * px * 2, cudaMemcpyHostToDevice, st));
+    frames = tmp;
+  }
+  for (int64_t f0 = 0; f0 < n; f0 += mb) {
+    int nf = (int)std::min<int64_t>(mb, n - f0);
+    ViewSet vs{(int)f0, H, W, 0, 0, 0, 1, 0, 1};
+    ActShape s{nf, C, H, W};
+    int res = 0;
+    float* dump = trunk ? trunk + (size_t)f0 * (L + 1) * px * C : nullptr;
+    r = run_trunk(c, frames, 0, vs, s, np, st, &res, dump, (size_t)(L + 1) * px * C, px * C, nullptr);
+    if (r != SMLM_OK) break;
+    cudaError_t e = launch_head_maps(c->bf16, c->act[res], s, c->w_head, c->b_head, nh,
+                                     maps + (size_t)f0 * nh * px, st);
+    c->launches++;
+    if (e != cudaSuccess) {
+      r = fail(c, SMLM_ERR_CUDA, "head_maps: %s", cudaGetErrorString(e));
+      break;
+    }
+  }
+  if (tmp) {
+    cudaStreamSynchronize(st);
+    cudaFree(tmp);
+  }
+  return r;
+}
+
+smlm_status smlm_debug_postprocess(smlm_ctx* c, const float* maps, int64_t n, int32_t H, int32_t W,
+                                   const smlm_camera_params* cam, float threshold, smlm_emitter* out,
+                                   int64_t* out_count, void* cuda_stream) {
+  if (!c) return SMLM_ERR_INVALID_ARG;
+  if (!cam || !out_count || (n > 0 && !maps) || n < 0 || H < 1 || W < 1 || n > 65535 || *out_count < 0)
+    return fail(c, SMLM_ERR_INVALID_ARG, "bad argument");
+  const unsigned long long capacity = (unsigned long long)*out_count;
+  if (capacity > 0 && (!out || classify(out) != PTR_DEVICE))
+    return fail(c, SMLM_ERR_INVALID_ARG, "out_emitters must be device memory here");
+  if (n > 0 && classify(maps) != PTR_DEVICE) return fail(c, SMLM_ERR_INVALID_ARG, "maps must be device memory");
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const HeadParams hp = head_params(c, cam, threshold);
+  CK(c, cudaMemsetAsync(c->counters, 0, 4 * sizeof(unsigned long long), st));
+  c->last_capacity = capacity;
+  CK(c, launch_post_from_maps(maps, (int)n, H, W, hp, out, c->counters, capacity, st));
+  c->launches++;
+  return store_count(c, c->counters, out_count, st);
+}
+
+}  // extern "C"

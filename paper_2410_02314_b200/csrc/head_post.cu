@@ -1,0 +1,302 @@
+// K3: 1x1 heads fused with the post-processing (BASELINE.json north_star (c); smlm.h):
+//   o = Wh a_L + bh;  pixel q is an emitter iff sigmoid(o_p[q]) > thr (tested in the logit
+//   domain: o_p > logit(thr)) and o_p[q] beats each in-frame 8-neighbour (greater, or equal
+//   with the lower linear index);  x = (ix + xy_scale tanh(o_dx)) px, ... ; records are
+//   appended to one list through a block-aggregated atomic counter.
+// The output maps never reach HBM: the block computes the detection logit of a
+// (TH+2) x (TW+2) patch into shared memory, runs the 3x3 test there, and evaluates the
+// remaining heads (and every transcendental) for the survivors only.
+//
+// HBM/L2-read-bound: 2C B/px of activations (+ ~10 % halo re-read), 32 B per emitter out.
+#include <math_constants.h>
+
+#include "chunk_io.cuh"
+#include "smlm_internal.cuh"
+
+namespace smlm {
+namespace {
+
+constexpr int TW = 64, TH = 32, NT = 256;
+constexpr int MAX_CAND = (TW / 2) * (TH / 2);  // no two detections are 8-adjacent
+
+__device__ inline float sigmoid_f(float v) { return 1.0f / (1.0f + expf(-v)); }
+__device__ inline float softplus_f(float v) { return fmaxf(v, 0.0f) + log1pf(expf(-fabsf(v))); }
+
+// One head of one pixel from the activations: fixed summation order (chunk, channel), so
+// every kernel in this file produces bit-identical values for the same pixel.
+template <typename T, int C>
+struct ActSource {
+  const T* act;
+  ActShape s;
+  const float* wh;  // shared memory [n_h][C]
+  const float* bh;  // shared memory [n_h]
+  __device__ inline float head(int h, int b, int y, int x) const {
+    float acc = bh[h];
+    const float* w = wh + h * C;
+#pragma unroll
+    for (int k = 0; k < C / 8; ++k) {
+      float v[8];
+      Chunk<T>::load(act, s.chunk_index(b, k, y, x), v);
+#pragma unroll
+      for (int c = 0; c < 8; ++c) acc = fmaf(v[c], w[k * 8 + c], acc);
+    }
+    return acc;
+  }
+};
+
+struct MapSource {
+  const float* maps;  // [n][n_h][H][W]
+  int n_h, H, W;
+  __device__ inline float head(int h, int b, int y, int x) const {
+    return maps[(((size_t)b * n_h + h) * H + y) * W + x];
+  }
+};
+
+template <typename Src>
+__device__ inline void detect_tile(const Src& src, int Hw, int Ww, const View& v, int b, int Wf,
+                                   const HeadParams& hp, smlm_emitter* __restrict__ out,
+                                   unsigned long long* __restrict__ counter,
+                                   unsigned long long capacity) {
+  __shared__ float lg[TH + 2][TW + 2];
+  __shared__ int cand[MAX_CAND];
+  __shared__ int ncand;
+  __shared__ unsigned long long base;
+
+  const int tid = threadIdx.x;
+  const int x0 = blockIdx.x * TW, y0 = blockIdx.y * TH;
+  if (tid == 0) ncand = 0;
+
+  // phase 1: detection logit of the patch; outside the window (= outside the frame for
+  // every pixel that neighbours an owned pixel) it is -inf: such neighbours never win.
+  for (int i = tid; i < (TH + 2) * (TW + 2); i += NT) {
+    int ly = i / (TW + 2), lx = i - ly * (TW + 2);
+    int y = y0 + ly - 1, x = x0 + lx - 1;
+    float o = -CUDART_INF_F;
+    if (y >= 0 && y < Hw && x >= 0 && x < Ww) o = src.head(0, b, y, x);
+    lg[ly][lx] = o;
+  }
+  __syncthreads();
+
+  // phase 2: threshold + 3x3 local maximum with the index tie rule.  Neighbours with a
+  // lower linear index (row above, left) must be strictly smaller; the others may be equal.
+  for (int i = tid; i < TH * TW; i += NT) {
+    int ly = i / TW, lx = i - ly * TW;
+    int y = y0 + ly, x = x0 + lx;
+    bool keep = (y >= v.cy0 && y < v.cy1 && x >= v.cx0 && x < v.cx1);
+    if (keep) {
+      float c = lg[ly + 1][lx + 1];
+      keep = (c > hp.lthr) && c > lg[ly][lx] && c > lg[ly][lx + 1] && c > lg[ly][lx + 2] &&
+             c > lg[ly + 1][lx] && c >= lg[ly + 1][lx + 2] && c >= lg[ly + 2][lx] &&
+             c >= lg[ly + 2][lx + 1] && c >= lg[ly + 2][lx + 2];
+    }
+    unsigned m = __ballot_sync(0xffffffffu, keep);
+    if (m) {
+      int lane = tid & 31, leader = __ffs(m) - 1, slot = 0;
+      if (lane == leader) slot = atomicAdd(&ncand, __popc(m));
+      slot = __shfl_sync(0xffffffffu, slot, leader);
+      if (keep) cand[slot + __popc(m & ((1u << lane) - 1u))] = i;
+    }
+  }
+  __syncthreads();
+  const int n = ncand;
+  if (n == 0) return;
+  if (tid == 0) base = atomicAdd(counter, (unsigned long long)n);
+  __syncthreads();
+
+  // phase 3: remaining heads + decode for the survivors only.
+  for (int j = tid; j < n; j += NT) {
+    unsigned long long slot = base + j;
+    if (slot >= capacity) continue;  // counted, not stored (smlm_check reports overflow)
+    int i = cand[j];
+    int ly = i / TW, lx = i - ly * TW;
+    int y = y0 + ly, x = x0 + lx;
+    int fy = v.wy0 + y, fx = v.wx0 + x;
+    const int hN = hp.n_h == 6 ? 4 : 3;
+    float odx = src.head(1, b, y, x), ody = src.head(2, b, y, x);
+    float oN = src.head(hN, b, y, x), obg = src.head(hN + 1, b, y, x);
+    smlm_emitter e;
+    e.frame = v.frame;
+    e.pix = fy * Wf + fx;
+    e.x_nm = ((float)fx + hp.xy_scale * tanhf(odx)) * hp.pixel_size_nm;
+    e.y_nm = ((float)fy + hp.xy_scale * tanhf(ody)) * hp.pixel_size_nm;
+    e.z_nm = hp.n_h == 6 ? hp.z_scale_nm * tanhf(src.head(3, b, y, x)) : 0.0f;
+    e.photons = hp.photon_scale * softplus_f(oN);
+    e.bg = hp.bg_scale * softplus_f(obg);
+    e.p = sigmoid_f(lg[ly + 1][lx + 1]);
+    uint4* dst = reinterpret_cast<uint4*>(out + slot);
+    const uint4* srcv = reinterpret_cast<const uint4*>(&e);
+    dst[0] = srcv[0];
+    dst[1] = srcv[1];
+  }
+}
+
+template <typename T, int C>
+__global__ void __launch_bounds__(NT)
+    head_post_kernel(const T* __restrict__ act, ActShape s, ViewSet vs,
+                     const float* __restrict__ w_head, const float* __restrict__ b_head,
+                     HeadParams hp, smlm_emitter* __restrict__ out,
+                     unsigned long long* __restrict__ counter, unsigned long long capacity) {
+  __shared__ float wh[6 * C];
+  __shared__ float bh[8];
+  for (int i = threadIdx.x; i < hp.n_h * C; i += NT) wh[i] = w_head[i];
+  if (threadIdx.x < hp.n_h) bh[threadIdx.x] = b_head[threadIdx.x];
+  __syncthreads();
+  const int b = blockIdx.z;
+  const View v = view_of(vs, b, s.H, s.W);
+  ActSource<T, C> src{act, s, wh, bh};
+  detect_tile(src, s.H, s.W, v, b, vs.Wf, hp, out, counter, capacity);
+}
+
+__global__ void __launch_bounds__(NT)
+    post_from_maps_kernel(const float* __restrict__ maps, int H, int W, HeadParams hp,
+                          smlm_emitter* __restrict__ out, unsigned long long* __restrict__ counter,
+                          unsigned long long capacity) {
+  const int b = blockIdx.z;
+  View v;
+  v.frame = b;
+  v.wy0 = v.wx0 = 0;
+  v.cy0 = v.cx0 = 0;
+  v.cy1 = H;
+  v.cx1 = W;
+  MapSource src{maps, hp.n_h, H, W};
+  detect_tile(src, H, W, v, b, W, hp, out, counter, capacity);
+}
+
+template <typename T, int C>
+__global__ void __launch_bounds__(NT)
+    head_maps_kernel(const T* __restrict__ act, ActShape s, const float* __restrict__ w_head,
+                     const float* __restrict__ b_head, int n_h, float* __restrict__ maps) {
+  __shared__ float wh[6 * C];
+  __shared__ float bh[8];
+  for (int i = threadIdx.x; i < n_h * C; i += NT) wh[i] = w_head[i];
+  if (threadIdx.x < n_h) bh[threadIdx.x] = b_head[threadIdx.x];
+  __syncthreads();
+  const int b = blockIdx.z, y = blockIdx.y;
+  ActSource<T, C> src{act, s, wh, bh};
+  for (int x = blockIdx.x * NT + threadIdx.x; x < s.W; x += gridDim.x * NT)
+    for (int h = 0; h < n_h; ++h)
+      maps[(((size_t)b * n_h + h) * s.H + y) * s.W + x] = src.head(h, b, y, x);
+}
+
+template <typename T>
+__global__ void __launch_bounds__(NT)
+    dump_act_kernel(const T* __restrict__ act, ActShape s, float* __restrict__ dst,
+                    size_t view_stride) {
+  const int b = blockIdx.z, y = blockIdx.y;
+  for (int x = blockIdx.x * NT + threadIdx.x; x < s.W; x += gridDim.x * NT)
+    for (int k = 0; k < s.C / 8; ++k) {
+      float v[8];
+      Chunk<T>::load(act, s.chunk_index(b, k, y, x), v);
+      float* d = dst + (size_t)b * view_stride + ((size_t)y * s.W + x) * s.C + k * 8;
+      for (int c = 0; c < 8; ++c) d[c] = v[c];
+    }
+}
+
+__global__ void snapshot_kernel(const unsigned long long* counter, unsigned long long capacity,
+                                unsigned long long* snap) {
+  unsigned long long c = *counter;
+  *snap = c < capacity ? c : capacity;
+}
+
+__global__ void __launch_bounds__(NT)
+    flush_kernel(const smlm_emitter* __restrict__ dev, smlm_emitter* __restrict__ host,
+                 const unsigned long long* __restrict__ snap, unsigned long long* flushed) {
+  // 16-byte units; grid-stride.  *flushed is advanced by a second, single-thread launch
+  // (flush_commit_kernel) so that every block of this one reads the same start.
+  const unsigned long long lo = *flushed * 2, hi = *snap * 2;
+  const uint4* s = reinterpret_cast<const uint4*>(dev);
+  uint4* d = reinterpret_cast<uint4*>(host);
+  for (unsigned long long i = lo + (unsigned long long)blockIdx.x * NT + threadIdx.x; i < hi;
+       i += (unsigned long long)gridDim.x * NT)
+    d[i] = s[i];
+}
+__global__ void flush_commit_kernel(const unsigned long long* snap, unsigned long long* flushed) {
+  *flushed = *snap;
+}
+
+template <typename T, int C>
+cudaError_t head_post_tc(const void* act, ActShape s, ViewSet vs, const float* w, const float* b,
+                         HeadParams hp, smlm_emitter* out, unsigned long long* counter,
+                         unsigned long long cap, cudaStream_t st) {
+  dim3 grid((s.W + TW - 1) / TW, (s.H + TH - 1) / TH, s.B);
+  head_post_kernel<T, C><<<grid, NT, 0, st>>>((const T*)act, s, vs, w, b, hp, out, counter, cap);
+  return cudaGetLastError();
+}
+template <typename T, int C>
+cudaError_t head_maps_tc(const void* act, ActShape s, const float* w, const float* b, int n_h,
+                         float* maps, cudaStream_t st) {
+  dim3 grid((s.W + NT - 1) / NT, s.H, s.B);
+  head_maps_kernel<T, C><<<grid, NT, 0, st>>>((const T*)act, s, w, b, n_h, maps);
+  return cudaGetLastError();
+}
+
+#define SMLM_DISPATCH_C(T, FN, ...)                      \
+  switch (s.C) {                                         \
+    case 16: return FN<T, 16>(__VA_ARGS__);              \
+    case 32: return FN<T, 32>(__VA_ARGS__);              \
+    case 48: return FN<T, 48>(__VA_ARGS__);              \
+    case 64: return FN<T, 64>(__VA_ARGS__);              \
+    default: return cudaErrorInvalidValue;               \
+  }
+
+}  // namespace
+
+cudaError_t launch_head_post(bool bf16, const void* act, ActShape s, ViewSet vs,
+                             const float* w_head, const float* b_head, HeadParams hp,
+                             smlm_emitter* out, unsigned long long* counter,
+                             unsigned long long capacity, cudaStream_t st) {
+  if (s.B <= 0) return cudaSuccess;
+  if (bf16) {
+    SMLM_DISPATCH_C(__nv_bfloat16, head_post_tc, act, s, vs, w_head, b_head, hp, out, counter, capacity, st)
+  } else {
+    SMLM_DISPATCH_C(float, head_post_tc, act, s, vs, w_head, b_head, hp, out, counter, capacity, st)
+  }
+}
+
+cudaError_t launch_head_maps(bool bf16, const void* act, ActShape s, const float* w_head,
+                             const float* b_head, int n_h, float* maps, cudaStream_t st) {
+  if (s.B <= 0) return cudaSuccess;
+  if (bf16) {
+    SMLM_DISPATCH_C(__nv_bfloat16, head_maps_tc, act, s, w_head, b_head, n_h, maps, st)
+  } else {
+    SMLM_DISPATCH_C(float, head_maps_tc, act, s, w_head, b_head, n_h, maps, st)
+  }
+}
+
+cudaError_t launch_dump_act(bool bf16, const void* act, ActShape s, float* dst, size_t view_stride,
+                            cudaStream_t st) {
+  if (s.B <= 0) return cudaSuccess;
+  dim3 grid((s.W + NT - 1) / NT, s.H, s.B);
+  if (bf16)
+    dump_act_kernel<__nv_bfloat16><<<grid, NT, 0, st>>>((const __nv_bfloat16*)act, s, dst, view_stride);
+  else
+    dump_act_kernel<float><<<grid, NT, 0, st>>>((const float*)act, s, dst, view_stride);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_post_from_maps(const float* maps, int n, int H, int W, HeadParams hp,
+                                  smlm_emitter* out, unsigned long long* counter,
+                                  unsigned long long capacity, cudaStream_t st) {
+  if (n <= 0) return cudaSuccess;
+  dim3 grid((W + TW - 1) / TW, (H + TH - 1) / TH, n);
+  post_from_maps_kernel<<<grid, NT, 0, st>>>(maps, H, W, hp, out, counter, capacity);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_snapshot(const unsigned long long* counter, unsigned long long capacity,
+                            unsigned long long* snap, cudaStream_t st) {
+  snapshot_kernel<<<1, 1, 0, st>>>(counter, capacity, snap);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_flush_emitters(const smlm_emitter* dev, smlm_emitter* host_mapped,
+                                  const unsigned long long* snap, unsigned long long* flushed,
+                                  cudaStream_t st) {
+  flush_kernel<<<64, NT, 0, st>>>(dev, host_mapped, snap, flushed);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  flush_commit_kernel<<<1, 1, 0, st>>>(snap, flushed);
+  return cudaGetLastError();
+}
+
+}  // namespace smlm

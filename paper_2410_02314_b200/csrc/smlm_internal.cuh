@@ -11,28 +11,65 @@ namespace smlm {
 
 // ---------------------------------------------------------------------------------------
 // Activation layout in HBM ("chunk-planar NHWC8"):
-//     act[b][k][y][x][8]      b < B views, k < C/8 channel chunks, y < H, x < Wp, 8 channels
-// Wp = W rounded up to a multiple of 8; columns W..Wp-1 always hold zeros.
+//     act[b][k][y][x][8]      b < B views, k < C/8 channel chunks, y < H, x < W, 8 channels
 // Why: (1) a pixel's 8-channel chunk is one 16-byte (bf16) vector, and consecutive pixels of
 // one chunk are consecutive in memory, so every warp-wide access is a dense 512 B run;
-// (2) one chunk plane row IS the UMMA "K-major, no swizzle" core-matrix sequence
+// (2) one chunk-plane row IS the UMMA "K-major, no swizzle" core-matrix sequence
 // (8 pixels x 16 B = one 128 B core matrix), so a TMA box lands in shared memory already in
-// the layout tcgen05.mma reads, at any pixel shift (conv_umma.cu).
+// the layout tcgen05.mma reads, at ANY pixel shift (conv_umma.cu) - which is what a dilated
+// convolution needs.
 // ---------------------------------------------------------------------------------------
 struct ActShape {
-  int B, C, H, W, Wp;
-  __host__ __device__ size_t elems() const { return (size_t)B * C * H * Wp; }
+  int B, C, H, W;
+  __host__ __device__ size_t elems() const { return (size_t)B * C * H * W; }
   __host__ __device__ size_t chunk_index(int b, int k, int y, int x) const {
-    return ((((size_t)b * (C >> 3) + k) * H + y) * Wp + x);
+    return ((((size_t)b * (C >> 3) + k) * H + y) * W + x);
   }
 };
 
-// One unit of a micro-batch: a window of a frame (whole frame, or one haloed tile).
+// One unit of a micro-batch is a VIEW: a window of a frame (the whole frame, or one tile plus
+// halo clipped to the frame).  All views of a launch have the same window size (s.H x s.W).
+// They are described parametrically (no table in memory): view v of the set is tile
+// (ty0 + (v / nx) % ny, tx0 + v % nx) of frame frame0 + v / (ny * nx).
+struct ViewSet {
+  int frame0;        // first frame (index within the call)
+  int Hf, Wf;        // frame size
+  int tile;          // 0: whole frames
+  int halo;          // tile mode: window = core +- halo, clipped to the frame
+  int ty0, ny, tx0, nx;
+};
+
 struct View {
-  int frame;           // frame index within the call
-  int wy0, wx0;        // window origin inside the frame
+  int frame;
+  int wy0, wx0;            // window origin inside the frame
   int cy0, cy1, cx0, cx1;  // owned ("core") rectangle in window coordinates, half-open
 };
+
+__host__ __device__ inline View view_of(const ViewSet& vs, int v, int Hw, int Ww) {
+  View r;
+  if (vs.tile <= 0) {
+    r.frame = vs.frame0 + v;
+    r.wy0 = r.wx0 = 0;
+    r.cy0 = r.cx0 = 0;
+    r.cy1 = Hw;
+    r.cx1 = Ww;
+    return r;
+  }
+  int per = vs.ny * vs.nx;
+  int f = v / per, t = v - f * per;
+  int ty = vs.ty0 + t / vs.nx, tx = vs.tx0 + t % vs.nx;
+  int y0 = ty * vs.tile, x0 = tx * vs.tile;
+  int y1 = y0 + vs.tile < vs.Hf ? y0 + vs.tile : vs.Hf;
+  int x1 = x0 + vs.tile < vs.Wf ? x0 + vs.tile : vs.Wf;
+  r.frame = vs.frame0 + f;
+  r.wy0 = y0 - vs.halo > 0 ? y0 - vs.halo : 0;
+  r.wx0 = x0 - vs.halo > 0 ? x0 - vs.halo : 0;
+  r.cy0 = y0 - r.wy0;
+  r.cx0 = x0 - r.wx0;
+  r.cy1 = y1 - r.wy0;
+  r.cx1 = x1 - r.wx0;
+  return r;
+}
 
 struct HeadParams {
   int n_h;
@@ -49,29 +86,33 @@ struct NormParams {
 // ----------------------------------------------------------------------------- launchers
 // (each returns the cudaError_t of the launch; all are asynchronous on `st`)
 
-// K1: uint16 unpack + normalise + 3x3 stem conv (+ReLU) -> act.  T = float | __nv_bfloat16.
-cudaError_t launch_stem(bool bf16, const uint16_t* frames, int Hf, int Wf, const View* views,
-                        ActShape s, NormParams np, const float* w_stem /*[9][C]*/,
-                        const float* b_stem, int relu, void* act, cudaStream_t st);
+// K1: uint16 unpack + normalise + 3x3 stem conv (+ReLU) -> act.
+// frames: device u16, frame f of the call at frames + (f - frame_base) * Hf * Wf.
+cudaError_t launch_stem(bool bf16, const uint16_t* frames, int frame_base, ViewSet vs, ActShape s,
+                        NormParams np, const float* w_stem /*[9][C]*/, const float* b_stem,
+                        int relu, void* act, cudaStream_t st);
 
 // K2' reference trunk layer on CUDA cores (fp32 math; storage float or bf16).
 // w: [9][C_in][C_out] float (already rounded to bf16 values in bf16 mode).
 cudaError_t launch_conv_direct(bool bf16, const void* in, void* out, ActShape s, int dil,
                                const float* w, const float* b, cudaStream_t st);
+cudaError_t conv_direct_init(int C);  // opt in to the shared memory the kernel needs
 
 // K2 trunk layer on tcgen05 tensor cores (bf16 storage, fp32 accumulate in TMEM).
-struct UmmaLayerPlan;  // opaque, conv_umma.cu
-UmmaLayerPlan* umma_plan_create(int C, int n_sm, char* err, size_t errlen);
-void umma_plan_destroy(UmmaLayerPlan*);
-// wpack: device, layout produced by umma_pack_weights_host; bias: device float [C].
+struct UmmaPlan;  // opaque, conv_umma.cu: tensor maps for one (buffer pair, shape)
 size_t umma_packed_weight_bytes(int C);
-void umma_pack_weights_host(int C, const float* w_oihw /*[C][C][3][3]*/, void* dst_bf16);
-cudaError_t launch_conv_umma(UmmaLayerPlan* plan, const void* in, void* out, ActShape s, int dil,
-                             const void* wpack, const float* bias, int band_rows,
-                             cudaStream_t st, char* err, size_t errlen);
+// w_oihw [C][C][3][3] fp32 -> the kernel's shared-memory image (bf16, RNE), host side.
+void umma_pack_weights_host(int C, const float* w_oihw, void* dst);
+UmmaPlan* umma_plan_create(const void* buf0, const void* buf1, ActShape s, int n_sm, char* err,
+                           size_t errlen);
+void umma_plan_destroy(UmmaPlan*);
+// in = plan buffer `src` (0/1), out = the other one.
+cudaError_t launch_conv_umma(UmmaPlan* plan, int src, int dil, const void* wpack,
+                             const float* bias, int band_rows, cudaStream_t st, char* err,
+                             size_t errlen);
 
 // K3: 1x1 heads + threshold + 3x3 NMS + decode + warp-aggregated compaction.
-cudaError_t launch_head_post(bool bf16, const void* act, ActShape s, const View* views, int Wf,
+cudaError_t launch_head_post(bool bf16, const void* act, ActShape s, ViewSet vs,
                              const float* w_head /*[n_h][C]*/, const float* b_head, HeadParams hp,
                              smlm_emitter* out, unsigned long long* counter,
                              unsigned long long capacity, cudaStream_t st);
@@ -79,7 +120,7 @@ cudaError_t launch_head_post(bool bf16, const void* act, ActShape s, const View*
 // debug: heads only -> fp32 maps [B][n_h][H][W] (pre-activation)
 cudaError_t launch_head_maps(bool bf16, const void* act, ActShape s, const float* w_head,
                              const float* b_head, int n_h, float* maps, cudaStream_t st);
-// debug: act -> float [B][slot of L1][H][W][C]
+// debug: act -> float dst[b * view_stride + (y*W + x)*C + c]
 cudaError_t launch_dump_act(bool bf16, const void* act, ActShape s, float* dst, size_t view_stride,
                             cudaStream_t st);
 // debug: detection + decode on caller maps [n][n_h][H][W]
@@ -87,11 +128,13 @@ cudaError_t launch_post_from_maps(const float* maps, int n, int H, int W, HeadPa
                                   smlm_emitter* out, unsigned long long* counter,
                                   unsigned long long capacity, cudaStream_t st);
 
-// copy records [done, min(counter, capacity)) from the device list to a mapped host list
+// snap[0] = min(*counter, capacity)
+cudaError_t launch_snapshot(const unsigned long long* counter, unsigned long long capacity,
+                            unsigned long long* snap, cudaStream_t st);
+// copy records [*flushed, *snap) from the device list to a device-visible host list, then
+// *flushed = *snap
 cudaError_t launch_flush_emitters(const smlm_emitter* dev, smlm_emitter* host_mapped,
-                                  const unsigned long long* counter, unsigned long long* flushed,
-                                  unsigned long long capacity, cudaStream_t st);
-// write min/actual count to a (mapped host or device) int64
-cudaError_t launch_store_count(const unsigned long long* counter, long long* dst, cudaStream_t st);
+                                  const unsigned long long* snap, unsigned long long* flushed,
+                                  cudaStream_t st);
 
 }  // namespace smlm

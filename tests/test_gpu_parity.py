@@ -1,0 +1,321 @@
+"""GPU parity tests: the CUDA library (through its C ABI) against the CPU oracle, element by
+element on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star): raw output maps within 1e-4 (fp32 mode) / 2e-2 (bf16
+mode) absolute; emitter count and pixel indices bit-exact outside the contested set;
+sub-pixel coordinates within 0.02 px.
+"""
+import json
+import math
+import os
+
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from smlm_synth import NetSpec, get_config, make_frames, make_weights
+import paper_2410_02314_b200 as P
+import gpu_util as G
+
+pytestmark = pytest.mark.gpu
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+TOL = {"fp32": 1e-4, "bf16": 2e-2}
+BF16_IMPLS = [pytest.param(P.CONV_DIRECT, id="direct"), pytest.param(P.CONV_TCGEN05, id="tcgen05")]
+
+
+def _rand_blob(spec, seed, scale=0.25):
+    rng = np.random.default_rng(seed)
+    return rng.normal(0, scale, size=spec.n_params()).astype(np.float32)
+
+
+# ------------------------------------------------------------------ cfg 0: fp32 reference mode
+def test_cfg0_fp32_trunk_maps_and_emitters():
+    cfg = get_config(0)
+    fs = make_frames(cfg)
+    w = make_weights(cfg)
+    ck = G.cam_kwargs(fs)
+    net, cam, o, dump = G.oracle_run("cfg0", cfg.net, w, fs.frames, ck, dump_trunk=True)
+    og, tg = G.gpu_forward_maps(cfg.net, w, fs.frames, ck, dump_trunk=True)
+    for l in range(cfg.net.n_layers + 1):
+        assert np.max(np.abs(tg[:, l] - dump[:, l])) < 1e-4, f"trunk level {l}"
+    assert np.max(np.abs(G.activated(cfg.net, og) - G.activated(cfg.net, o))) < 1e-4
+    em_o = O.postprocess(net, o, cam, cfg.threshold)
+    em_g = G.gpu_localize(cfg.net, w, fs.frames, ck, cfg.threshold)
+    st = G.parity_gate(cfg.net, o, em_o, em_g, cfg.threshold, 1e-4, fs.pixel_size_nm, 64, 64)
+    print("cfg0 gate", st)
+    assert st["oracle"] > 50 and st["contested_frac"] < 0.5      # the gate is not vacuous
+    assert st["rel_N"] < 1e-3 and st["rel_bg"] < 1e-3
+
+
+# ------------------------------------------------------------------ post-processing alone
+def _gpu_post(spec, o, threshold, pixel=100.0, capacity=None):
+    torch = G.torch_mod()
+    desc = P.desc_from_spec(spec)
+    n, nh, H, W = o.shape
+    cap = n * ((H + 1) // 2) * ((W + 1) // 2) if capacity is None else capacity
+    with P.Localizer(desc, np.zeros(spec.n_params(), np.float32)) as loc:
+        maps = torch.from_numpy(np.ascontiguousarray(o, dtype=np.float32)).cuda()
+        buf = torch.zeros(max(cap, 1) * 32, dtype=torch.uint8, device="cuda")
+        cnt = loc.postprocess(maps, loc.camera(pixel, 100.0, 1.0), threshold, buf, cap)
+        torch.cuda.synchronize()
+        return P.emitters_to_numpy(buf, min(cnt.value, cap)), int(cnt.value), loc.check()
+
+
+with open(os.path.join(GOLDEN, "delta_maps.json"), "r", encoding="utf-8") as _fh:
+    _DELTA = json.load(_fh)
+
+
+@pytest.mark.parametrize("case", _DELTA["cases"], ids=[c["name"] for c in _DELTA["cases"]])
+def test_postprocess_hand_placed_delta_maps(case):
+    H, W = _DELTA["H"], _DELTA["W"]
+    spec = NetSpec(16, (1,), 5, "fp32")
+    o = np.zeros((1, 5, H, W))
+    o[0, 0] = case["background_logit"]
+    for s in case["spikes"]:
+        logit = s["logit"] if "logit" in s else math.log(s["p"] / (1.0 - s["p"]))
+        o[0, 0, s["y"], s["x"]] = logit
+        for h, key in ((1, "o_dx"), (2, "o_dy"), (3, "o_N"), (4, "o_bg")):
+            if key in s:
+                o[0, h, s["y"], s["x"]] = s[key]
+    em, found, status = _gpu_post(spec, o, case["threshold"], _DELTA["pixel_size_nm"])
+    # fp32 maps: a spike placed within 1e-6 of the threshold in p is not representable
+    exp = sorted(case["expect"], key=lambda e: e["pix"])
+    assert status == P.OK
+    assert [int(p) for p in em["pix"]] == [e["pix"] for e in exp], case["name"]
+    for got, e in zip(em, exp):
+        for key in ("x_nm", "y_nm", "p", "photons", "bg"):
+            if key in e:
+                assert float(got[key]) == pytest.approx(e[key], rel=2e-6, abs=1e-30), (case["name"], key)
+        assert got["z_nm"] == 0.0
+
+
+def test_postprocess_ties_thresholds_and_six_heads_match_oracle():
+    rng = np.random.default_rng(42)
+    H, W = 75, 133                                         # several tiles + ragged tail
+    spec = NetSpec(16, (1,), 6, "fp32")
+    net = O.net_from_spec(spec)
+    cam = O.make_camera(100.0, 100.0, 1.0)
+    o = rng.normal(0, 1.0, size=(3, 6, H, W))
+    o[:, 0] = np.round(rng.normal(0, 1.5, size=(3, H, W)) * 2) / 2      # many exact ties
+    o = o.astype(np.float32).astype(np.float64)
+    for thr in (-1.0, 0.0, 0.3, 0.7, 1.0, 2.0):
+        em_o = O.postprocess(net, o, cam, thr)
+        em_g, found, status = _gpu_post(spec, o, thr)
+        assert status == P.OK and found == len(em_o), thr
+        assert np.array_equal(em_g["frame"], em_o["frame"]) and np.array_equal(em_g["pix"], em_o["pix"])
+        if len(em_o):
+            for k, rel in (("x_nm", 1e-6), ("y_nm", 1e-6), ("z_nm", 1e-5), ("photons", 1e-5), ("bg", 1e-5), ("p", 1e-5)):
+                np.testing.assert_allclose(em_g[k], em_o[k], rtol=rel, atol=1e-4, err_msg=k)
+
+
+def test_postprocess_saturation_and_overflow():
+    spec = NetSpec(16, (1,), 5, "fp32")
+    o = np.zeros((1, 5, 9, 9))
+    o[0, 0] = -40.0
+    o[0, 0, 4, 4] = 40.0
+    o[0, 3, 4, 4] = 40.0
+    o[0, 4, 4, 4] = -40.0
+    em, found, status = _gpu_post(spec, o, 0.3)
+    assert found == 1 and np.isfinite([em[k][0] for k in ("x_nm", "y_nm", "photons", "bg", "p")]).all()
+    assert em["photons"][0] == pytest.approx(40000.0, rel=1e-6) and em["p"][0] == pytest.approx(1.0)
+    # overflow: all-local-maxima on a checkerboard, capacity 3
+    o = np.zeros((1, 5, 8, 8))
+    o[0, 0, ::2, ::2] = 1.0
+    em, found, status = _gpu_post(spec, o, 0.3, capacity=3)
+    assert found == 16 and len(em) == 3 and status == P.ERR_OVERFLOW
+
+
+# ------------------------------------------------------------------ ragged sizes, maps, 6 heads
+@pytest.mark.parametrize("C,nh,H,W,dil", [(16, 5, 37, 41, (1, 2)), (32, 6, 70, 131, (1, 2, 4, 8)),
+                                          (64, 6, 33, 200, (8, 4)), (48, 5, 130, 66, (2, 8, 1))])
+def test_fp32_ragged_sizes_camera_maps(C, nh, H, W, dil):
+    spec = NetSpec(C, dil, nh, "fp32")
+    w = _rand_blob(spec, C + H, scale=0.12)
+    rng = np.random.default_rng(H * W)
+    frames = rng.integers(50, 4000, size=(3, H, W)).astype(np.uint16)
+    offm = rng.normal(100, 2, size=(H, W)).astype(np.float32)
+    gm = np.clip(rng.normal(2.0, 0.1, size=(H, W)), 0.5, None).astype(np.float32)
+    ck = dict(pixel_size_nm=100.0, offset=0.0, gain=1.0, offset_map=offm, gain_map=gm)
+    net, cam, o, dump = G.oracle_run(("ragged", C, H), spec, w, frames, ck, dump_trunk=True)
+    og, tg = G.gpu_forward_maps(spec, w, frames, ck, dump_trunk=True)
+    scale = max(1.0, float(np.abs(dump).max()))
+    for l in range(spec.n_layers + 1):
+        assert np.max(np.abs(tg[:, l] - dump[:, l])) < 1e-5 * scale, f"level {l}"
+    assert np.max(np.abs(og - o)) < 2e-5 * scale
+    em_o = O.postprocess(net, o, cam, 0.5)
+    em_g = G.gpu_localize(spec, w, frames, ck, 0.5)
+    st = G.parity_gate(spec, o, em_o, em_g, 0.5, 1e-4, 100.0, H, W)
+    print("ragged gate", (C, nh, H, W), st)
+
+
+# ------------------------------------------------------------------ cfg 1: hc (fp32 mode) and lc (bf16)
+def test_cfg1_hc_weights_fp32_mode_index_gate():
+    cfg = get_config(1)
+    fs = make_frames(cfg, 2)
+    w = make_weights(cfg, "hc")
+    ck = G.cam_kwargs(fs)
+    net, cam, o, _ = G.oracle_run("cfg1hc", cfg.net, w, fs.frames, ck)
+    import dataclasses
+    spec32 = dataclasses.replace(cfg.net, precision="fp32")
+    og = G.gpu_forward_maps(spec32, w, fs.frames, ck)
+    assert np.max(np.abs(G.activated(cfg.net, og) - G.activated(cfg.net, o))) < 1e-4
+    em_o = O.postprocess(net, o, cam, cfg.threshold)
+    em_g = G.gpu_localize(spec32, w, fs.frames, ck, cfg.threshold)
+    st = G.parity_gate(cfg.net, o, em_o, em_g, cfg.threshold, 1e-4, fs.pixel_size_nm, 256, 256)
+    print("cfg1 hc fp32 gate", st)
+    assert st["oracle"] > 800 and st["contested_frac"] < 0.25 and st["flipped"] <= 4
+
+
+@pytest.mark.parametrize("impl", BF16_IMPLS)
+def test_cfg1_lc_weights_bf16_maps_and_gate(impl):
+    cfg = get_config(1)
+    fs = make_frames(cfg, 2)
+    w = make_weights(cfg, "lc")
+    ck = G.cam_kwargs(fs)
+    net, cam, o, _ = G.oracle_run("cfg1lc", cfg.net, w, fs.frames, ck)
+    og = G.gpu_forward_maps(cfg.net, w, fs.frames, ck, conv_impl=impl)
+    err = np.abs(G.activated(cfg.net, og) - G.activated(cfg.net, o)).reshape(2, 5, -1).max(axis=(0, 2))
+    print("cfg1 lc bf16 map errors per head", err)
+    assert err.max() < 2e-2
+    em_o = O.postprocess(net, o, cam, cfg.threshold)
+    em_g = G.gpu_localize(cfg.net, w, fs.frames, ck, cfg.threshold, conv_impl=impl)
+    st = G.parity_gate(cfg.net, o, em_o, em_g, cfg.threshold, 2e-2, fs.pixel_size_nm, 256, 256)
+    print("cfg1 lc bf16 gate", st)
+
+
+@pytest.mark.parametrize("impl", BF16_IMPLS)
+def test_cfg2_crop_bf16_six_heads(impl):
+    cfg = get_config(2)
+    fs = make_frames(cfg, 2, height=136, width=200)
+    w = make_weights(cfg, "lc")
+    ck = G.cam_kwargs(fs)
+    net, cam, o, _ = G.oracle_run("cfg2crop", cfg.net, w, fs.frames, ck)
+    og = G.gpu_forward_maps(cfg.net, w, fs.frames, ck, conv_impl=impl)
+    err = np.abs(G.activated(cfg.net, og) - G.activated(cfg.net, o)).reshape(2, 6, -1).max(axis=(0, 2))
+    print("cfg2 crop bf16 map errors per head", err)
+    assert err.max() < 2e-2
+    em_o = O.postprocess(net, o, cam, cfg.threshold)
+    em_g = G.gpu_localize(cfg.net, w, fs.frames, ck, cfg.threshold, conv_impl=impl)
+    st = G.parity_gate(cfg.net, o, em_o, em_g, cfg.threshold, 2e-2, fs.pixel_size_nm, 136, 200)
+    print("cfg2 crop gate", st)
+
+
+@pytest.mark.parametrize("impl", BF16_IMPLS)
+def test_cfg4_dense_bf16(impl):
+    cfg = get_config(4)
+    fs = make_frames(cfg, 1)
+    w = make_weights(cfg, "lc")
+    ck = G.cam_kwargs(fs)
+    net, cam, o, _ = G.oracle_run("cfg4", cfg.net, w, fs.frames, ck)
+    og = G.gpu_forward_maps(cfg.net, w, fs.frames, ck, conv_impl=impl)
+    assert np.max(np.abs(G.activated(cfg.net, og) - G.activated(cfg.net, o))) < 2e-2
+    em_o = O.postprocess(net, o, cam, cfg.threshold)
+    em_g = G.gpu_localize(cfg.net, w, fs.frames, ck, cfg.threshold, conv_impl=impl)
+    st = G.parity_gate(cfg.net, o, em_o, em_g, cfg.threshold, 2e-2, fs.pixel_size_nm, 256, 256)
+    print("cfg4 gate", st)
+
+
+# ------------------------------------------------------------------ bf16: tensor-core kernel vs CUDA-core kernel
+@pytest.mark.parametrize("C,H,W,dil", [(48, 70, 300, (1, 2, 4, 8)), (64, 40, 129, (8, 1)),
+                                       (16, 64, 64, (1, 2, 4, 8)), (32, 19, 517, (4, 2))])
+def test_tcgen05_matches_direct_bf16(C, H, W, dil):
+    """Same rounding points (bf16 inputs and weights, fp32 accumulate, one RNE store), only the
+    summation order differs: the stored bf16 maps may differ by an ulp here and there."""
+    spec = NetSpec(C, dil, 5, "bf16")
+    w = _rand_blob(spec, 100 + C, scale=(2.0 / (9 * C)) ** 0.5 * 0.6)
+    rng = np.random.default_rng(W)
+    frames = rng.integers(80, 3000, size=(3, H, W)).astype(np.uint16)
+    ck = dict(pixel_size_nm=100.0, offset=100.0, gain=1.0)
+    _, ta = G.gpu_forward_maps(spec, w, frames, ck, dump_trunk=True, conv_impl=P.CONV_DIRECT)
+    _, tb = G.gpu_forward_maps(spec, w, frames, ck, dump_trunk=True, conv_impl=P.CONV_TCGEN05)
+    assert np.array_equal(ta[:, 0], tb[:, 0])
+    for l in range(1, spec.n_layers + 1):
+        d = np.abs(ta[:, l] - tb[:, l])
+        scale = np.maximum(np.abs(ta[:, l]), 1.0)
+        assert np.max(d / scale) < 2.0 ** -6, f"level {l}: {np.max(d / scale)}"
+        assert np.mean(d > 0) < 0.05, f"level {l}: {np.mean(d > 0)} of values differ"
+
+
+# ------------------------------------------------------------------ tiling (cfg 3 mechanics)
+@pytest.mark.parametrize("precision,impl", [("fp32", P.CONV_AUTO), ("bf16", P.CONV_DIRECT),
+                                            ("bf16", P.CONV_TCGEN05)])
+def test_tiled_equals_whole_frame(precision, impl):
+    """cfg 3: tiles with a halo of radius+1, detections owned by the core tile.  The tiled
+    result must equal whole-frame processing (bit-exact: the kernels' summation order does
+    not depend on position) and hence the oracle, which never tiles."""
+    spec = NetSpec(16, (1, 2, 4), 5, precision)                 # radius 8 -> halo 9
+    w = _rand_blob(spec, 5, scale=0.2)
+    rng = np.random.default_rng(77)
+    H, W = 150, 173
+    frames = rng.integers(80, 3000, size=(2, H, W)).astype(np.uint16)
+    offm = rng.normal(100, 2, size=(H, W)).astype(np.float32)
+    gm = np.clip(rng.normal(2.0, 0.1, size=(H, W)), 0.5, None).astype(np.float32)
+    ck = dict(pixel_size_nm=100.0, offset=0.0, gain=1.0, offset_map=offm, gain_map=gm)
+    whole = G.gpu_localize(spec, w, frames, ck, 0.5, conv_impl=impl)
+    assert len(whole) > 100
+    for tile, mb in ((64, 0), (64, 2), (40, 3), (128, 0)):
+        tiled = G.gpu_localize(spec, w, frames, ck, 0.5, conv_impl=impl, tile=tile, micro_batch=mb)
+        assert np.array_equal(tiled["frame"], whole["frame"]) and np.array_equal(tiled["pix"], whole["pix"]), tile
+        for k in ("x_nm", "y_nm", "photons", "bg", "p"):
+            assert np.array_equal(tiled[k], whole[k]), (tile, k)
+    if precision == "fp32":
+        net, cam, o, _ = G.oracle_run("tiled", spec, w, frames, ck)
+        em_o = O.postprocess(net, o, cam, 0.5)
+        G.parity_gate(spec, o, em_o, whole, 0.5, 1e-4, 100.0, H, W)
+
+
+# ------------------------------------------------------------------ pipeline: ring, write-back, edge cases
+def test_pinned_ring_and_writeback_batches_equal_device_path():
+    cfg = get_config(0)
+    fs = make_frames(cfg, 8)
+    frames = np.concatenate([fs.frames] * 5)[:37]               # 37 frames, micro-batch 4 -> ragged tail
+    w = make_weights(cfg)
+    ck = G.cam_kwargs(fs)
+    ref = G.gpu_localize(cfg.net, w, frames, ck, cfg.threshold, micro_batch=4)
+    for kw in (dict(host_frames=True), dict(host_frames=True, host_out=True, writeback_frames=8),
+               dict(host_out=True), dict(host_frames=True, host_out=True, writeback_frames=5, micro_batch=3)):
+        kw.setdefault("micro_batch", 4)
+        em = G.gpu_localize(cfg.net, w, frames, ck, cfg.threshold, **kw)
+        assert np.array_equal(em, ref), kw
+    # frames 8.. repeat frames 0..: same detections, shifted frame index
+    a = ref[ref["frame"] < 8]
+    b = ref[(ref["frame"] >= 8) & (ref["frame"] < 16)]
+    assert np.array_equal(a["pix"], b["pix"]) and np.array_equal(a["frame"] + 8, b["frame"])
+
+
+def test_edge_cases_empty_overflow_pageable_threshold():
+    torch = G.torch_mod()
+    cfg = get_config(0)
+    fs = make_frames(cfg, 2)
+    w = make_weights(cfg)
+    ck = G.cam_kwargs(fs)
+    em, found, status, _ = G.gpu_localize(cfg.net, w, fs.frames[:0], ck, 0.3, return_status=True)
+    assert found == 0 and status == P.OK
+    em, found, status, _ = G.gpu_localize(cfg.net, w, fs.frames, ck, 1.0, return_status=True)
+    assert found == 0 and status == P.OK
+    full = G.gpu_localize(cfg.net, w, fs.frames, ck, 0.3)
+    em, found, status, _ = G.gpu_localize(cfg.net, w, fs.frames, ck, 0.3, capacity=5, return_status=True)
+    assert found == len(full) and len(em) == 5 and status == P.ERR_OVERFLOW
+    em, found, status, _ = G.gpu_localize(cfg.net, w, fs.frames, ck, 0.3, capacity=5, host_out=True,
+                                          return_status=True)
+    assert found == len(full) and len(em) == 5 and status == P.ERR_OVERFLOW
+    allmax, n_all, status, _ = G.gpu_localize(cfg.net, w, fs.frames, ck, 0.0, return_status=True)
+    assert status == P.OK and n_all >= len(full)
+    assert {(int(f), int(q)) for f, q in zip(full["frame"], full["pix"])} <= \
+           {(int(f), int(q)) for f, q in zip(allmax["frame"], allmax["pix"])}
+    # pageable host frames are refused (they would silently serialise the copy)
+    desc = P.desc_from_spec(cfg.net)
+    with P.Localizer(desc, w) as loc:
+        buf = torch.zeros(32 * 10, dtype=torch.uint8, device="cuda")
+        with pytest.raises(P.SmlmError) as ei:
+            loc.localize(torch.from_numpy(fs.frames.copy()), loc.camera(), 0.3, buf, 10)
+        assert ei.value.status == P.ERR_INVALID_ARG
+    # bad descriptors
+    for kw in (dict(channels=24), dict(head_channels=4), dict(dilations=(9,)), dict(precision=7)):
+        base = dict(channels=16, dilations=(1,), head_channels=5, precision=P.FP32)
+        base.update(kw)
+        d = P.make_desc(**base)
+        with pytest.raises(P.SmlmError) as ei:
+            P.Localizer(d, np.zeros((d.channels * 10) + d.n_layers * (d.channels ** 2 * 9 + d.channels)
+                                    + d.head_channels * (d.channels + 1), np.float32))
+        assert ei.value.status == P.ERR_INVALID_ARG
