@@ -29,7 +29,6 @@
 // The activation layout act[b][C/8][y][x][8] makes a TMA box land in shared memory as the
 // UMMA "K-major, no swizzle" operand: core matrix = 8 pixels x 16 B, contiguous, so a
 // horizontal tap is a 16-byte-granular shift of the descriptor start address.
-#include <cuda.h>
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 
@@ -42,15 +41,55 @@
 namespace smlm {
 namespace {
 
-constexpr int kThreads = 384;  // warp 0 TMA, 1 MMA, 2 TMEM alloc, 3 idle, 4-7 / 8-11 epilogue lane 0 / 1
+constexpr int kThreads = 384;  // warps 0 / 2: TMA lane 0 / 1 (2 also owns TMEM alloc), 1 / 3: MMA lane 0 / 1, 4-7 / 8-11: epilogue
 constexpr int kTileM = 128;
 constexpr int kMaxStages = 4;
 constexpr int kTmemCols = 512;
 constexpr int kLaneCols = 256;  // TMEM columns reserved per lane (3C <= 192)
 
+// zero source for the padded parts of a row segment: at most (127 + 8) pixels x 16 B
+__device__ __align__(16) uint4 g_zeros[160];
+
+// Optional per-CTA cycle accounting (-DSMLM_PROF, used by ad-hoc probes only): slot i of CTA b
+// is g_prof[b * 16 + i].
+#ifdef SMLM_PROF
+__device__ unsigned long long g_prof[1024 * 16];
+#define PROF_DECL long long prof_acc[16] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}
+#define PROF_T(var) const long long var = clock64()
+#define PROF_ADD(i, v) prof_acc[i] += (long long)(v)
+#define PROF_WAIT(i, stmt)          \
+  do {                              \
+    long long t0_ = clock64();      \
+    stmt;                           \
+    prof_acc[i] += clock64() - t0_; \
+  } while (0)
+#define PROF_FLUSH(cond)                                                             \
+  if (cond) {                                                                        \
+    for (int i_ = 0; i_ < 16; ++i_)                                                  \
+      if (prof_acc[i_]) g_prof[blockIdx.x * 16 + i_] += (unsigned long long)prof_acc[i_]; \
+  }
+#else
+#define PROF_DECL
+#define PROF_T(var)
+#define PROF_ADD(i, v)
+#define PROF_WAIT(i, stmt) stmt
+#define PROF_FLUSH(cond)
+#endif
+
 // ------------------------------------------------------------------------------ PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return static_cast<uint32_t>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "elect.sync _|p, 0xffffffff;\n"
+      "selp.u32 %0, 1, 0, p;\n"
+      "}\n"
+      : "=r"(pred));
+  return pred != 0;
 }
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
@@ -74,14 +113,6 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
 }
 __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void tma_load_5d(uint32_t dst, const CUtensorMap* map, uint32_t bar, int c0,
-                                            int c1, int c2, int c3, int c4) {
-  asm volatile(
-      "cp.async.bulk.tensor.5d.shared::cluster.global.tile.mbarrier::complete_tx::bytes "
-      "[%0], [%1, {%3, %4, %5, %6, %7}], [%2];" ::"r"(dst),
-      "l"(reinterpret_cast<uint64_t>(map)), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(c4)
-      : "memory");
 }
 __device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
   asm volatile(
@@ -145,49 +176,31 @@ struct Geo {
   long long total;  // B * nseg * d * Lmax row-tiles
 };
 
-struct Step {
-  int b, x0;
-  int in_row, out_row;
-  bool in_valid, out_valid;
+// A lane owns the contiguous range [g, g1) of row-tiles and walks it as RUNS: n consecutive
+// rows i0 .. i0+n-1 of one chain (view b, segment x0, residue r).  A run takes n + 2 steps
+// j = 0 .. n+1: step j brings in chain row q = i0-1+j (image row r + q d, skipped when it is
+// outside the image) and completes the output whose centre was the previous step's row
+// (valid for j >= 2).  All roles of a lane walk the same deterministic sequence.
+struct Run {
+  int b, x0, r, i0, n;
 };
-
-// All roles of a lane walk the same deterministic sequence of steps.  A lane owns the
-// contiguous range [g, g1) of row-tiles; inside one chain a run of n rows takes n + 2 steps
-// (inputs i0-1 .. i0+n; the output of chain index o is complete after the step of input o+1).
-struct LaneIter {
+struct LaneRuns {
   long long g, g1;
-  int i0, n, j, r, b, x0;
-  bool active;
   __device__ void init(const Geo& geo, int lane_id, int nlanes) {
     g = geo.total * lane_id / nlanes;
     g1 = geo.total * (lane_id + 1) / nlanes;
-    active = false;
   }
-  __device__ bool next(const Geo& geo, Step& s) {
-    if (!active) {
-      if (g >= g1) return false;
-      long long chain = g / geo.Lmax;
-      i0 = (int)(g - chain * geo.Lmax);
-      long long rem = g1 - g;
-      n = geo.Lmax - i0 < rem ? geo.Lmax - i0 : (int)rem;
-      r = (int)(chain % geo.d);
-      long long t = chain / geo.d;
-      x0 = (int)(t % geo.nseg) * kTileM;
-      b = (int)(t / geo.nseg);
-      j = 0;
-      active = true;
-    }
-    const int q = i0 - 1 + j;
-    s.b = b;
-    s.x0 = x0;
-    s.in_row = r + q * geo.d;
-    s.in_valid = q >= 0 && s.in_row < geo.H;
-    s.out_row = r + (q - 1) * geo.d;
-    s.out_valid = j >= 2 && s.out_row < geo.H;
-    if (++j == n + 2) {
-      active = false;
-      g += n;
-    }
+  __device__ bool next(const Geo& geo, Run& run) {
+    if (g >= g1) return false;
+    const long long chain = g / geo.Lmax;
+    run.i0 = (int)(g - chain * geo.Lmax);
+    const long long rem = g1 - g;
+    run.n = geo.Lmax - run.i0 < rem ? geo.Lmax - run.i0 : (int)rem;
+    run.r = (int)(chain % geo.d);
+    const long long t = chain / geo.d;
+    run.x0 = (int)(t % geo.nseg) * kTileM;
+    run.b = (int)(t / geo.nseg);
+    g += run.n;
     return true;
   }
 };
@@ -219,9 +232,8 @@ __host__ __device__ inline SmemLayout smem_layout(int C, int d, int nstage) {
 
 template <int C>
 __global__ void __launch_bounds__(kThreads, 1)
-    conv_umma_kernel(const __grid_constant__ CUtensorMap tmap, const __nv_bfloat16* __restrict__ in,
-                     __nv_bfloat16* __restrict__ out, Geo geo, const uint8_t* __restrict__ wpack,
-                     const float* __restrict__ bias, int nstage) {
+    conv_umma_kernel(const __nv_bfloat16* __restrict__ in, __nv_bfloat16* __restrict__ out, Geo geo,
+                     const uint8_t* __restrict__ wpack, const float* __restrict__ bias, int nstage) {
   extern __shared__ uint8_t smem_raw[];
   const SmemLayout L = smem_layout(C, geo.d, nstage);
   const uint32_t sraw = smem_u32(smem_raw);
@@ -229,6 +241,8 @@ __global__ void __launch_bounds__(kThreads, 1)
   uint8_t* smem = smem_raw + (sbase - sraw);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int d = geo.d;
+  PROF_T(t_begin);
+  PROF_DECL;
 
   const uint32_t wbar = sbase + L.bar_off;
   auto full_bar = [&](int ln, int s) { return sbase + L.bar_off + 8u * (1 + ln * (2 * kMaxStages + 2) + s); };
@@ -245,7 +259,7 @@ __global__ void __launch_bounds__(kThreads, 1)
     for (int ln = 0; ln < 2; ++ln) {
       for (int s = 0; s < kMaxStages; ++s) {
         mbar_init(full_bar(ln, s), 1);
-        mbar_init(empty_bar(ln, s), 1);
+        mbar_init(empty_bar(ln, s), 5);  // MMA commit + one arrival per epilogue warp
       }
       mbar_init(acc_full_bar(ln), 1);
       mbar_init(acc_free_bar(ln), 4);  // one arrival per epilogue warp
@@ -264,93 +278,151 @@ __global__ void __launch_bounds__(kThreads, 1)
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
+  // Programmatic dependent launch: everything above (barriers, TMEM, bias) and the weight
+  // load below touch nothing the previous layer's kernel writes, so they overlap its tail.
+  // Let the next layer's kernel start its own prologue as soon as SMs free up ...
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
   const int nlanes = 2 * gridDim.x;
 
-  if (warp == 0) {
-    // =========================== TMA producer ===========================
-    if (lane == 0) {
+  // The two single-thread roles run with the whole warp converged and one elected lane
+  // issuing: every operand below is warp-uniform, so the compiler keeps descriptors and
+  // addresses in uniform registers (inside an `if (lane == 0)` region it falls back to a
+  // per-instruction R2UR broadcast loop, ~19 instructions per MMA: the issue thread, not
+  // the tensor pipe, was then the limiter - profiles/conv_umma_r1_full.md).
+  if (warp == 0 || warp == 2) {
+    // =========================== TMA producers: warp 0 -> lane 0, warp 2 -> lane 1 ========
+    const int ln = warp >> 1;
+    if (warp == 0 && elect_one()) {
       // the layer's weights: one bulk copy stream into shared memory, resident for the launch
       mbar_expect_tx(wbar, L.w_bytes);
       for (uint32_t off = 0; off < L.w_bytes; off += 16384u) {
         uint32_t n = L.w_bytes - off < 16384u ? L.w_bytes - off : 16384u;
         bulk_load(sbase + L.w_off + off, wpack + off, n, wbar);
       }
-      LaneIter it[2];
-      it[0].init(geo, 2 * blockIdx.x, nlanes);
-      it[1].init(geo, 2 * blockIdx.x + 1, nlanes);
-      uint32_t cnt[2] = {0, 0};
-      bool more[2] = {true, true};
-      const uint32_t box_bytes = (uint32_t)(C / 8) * (kTileM + 2 * d) * 16u;
-      while (more[0] || more[1]) {
+    }
+    __syncwarp();
+    // ... and wait for the previous layer's kernel to have finished (it wrote `in` and was
+    // still reading `out`) before the first activation access.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    // One input row segment = C/8 contiguous runs of (128 + 2d) pixels x 16 B in the
+    // chunk-planar layout: one 1-D bulk copy each (a tensor-map box with a 16-byte inner
+    // dimension costs one 32-byte sector request per pixel-chunk, twice the L2 traffic).
+    // The parts of the segment outside the row are the convolution's zero padding (and the
+    // ragged right edge): they are bulk-copied from a block of zeros, for the first `nstage`
+    // loads after the segment changes - after that every stage already holds them.
+    const uint32_t plane = (uint32_t)(kTileM + 2 * d) * 16u;
+    const size_t plane_bytes = (size_t)geo.H * geo.W * 16u;
+    const size_t row_step = (size_t)d * geo.W * 16u;
+    const uint8_t* in_b = reinterpret_cast<const uint8_t*>(in);
+    LaneRuns runs;
+    runs.init(geo, 2 * blockIdx.x + ln, nlanes);
+    Run run;
+    uint32_t st = 0, empty_par = 1;
+    int last_x0 = -1, fills_left = 0;
+    while (runs.next(geo, run)) {
+      const int xl = run.x0 - d, xr = run.x0 + kTileM + d;
+      const int lo = xl > 0 ? xl : 0, hi = xr < geo.W ? xr : geo.W;
+      const uint32_t pre = (uint32_t)(lo - xl) * 16u, mid = (uint32_t)(hi - lo) * 16u,
+                     post = (uint32_t)(xr - hi) * 16u;
+      if (run.x0 != last_x0) {
+        last_x0 = run.x0;
+        fills_left = (pre | post) ? nstage : 0;
+      }
+      int row = run.r + (run.i0 - 1) * d;
+      const uint8_t* src = in_b + ((size_t)run.b * (C / 8) * geo.H * geo.W + (long long)row * geo.W + lo) * 16;
+      for (int j = 0; j < run.n + 2; ++j, row += d, src += row_step) {
+        if (row < 0 || row >= geo.H) continue;
+        const uint32_t dst = stage_addr(ln, st);
+        const uint32_t bar = full_bar(ln, st);
+        const bool fill = fills_left > 0;
+        PROF_WAIT(1, mbar_wait(empty_bar(ln, st), empty_par));
+        if (elect_one()) {
+          mbar_expect_tx(bar, (uint32_t)(C / 8) * (fill ? plane : mid));
 #pragma unroll
-        for (int ln = 0; ln < 2; ++ln) {
-          if (!more[ln]) continue;
-          Step s;
-          more[ln] = it[ln].next(geo, s);
-          if (!more[ln] || !s.in_valid) continue;
-          const int st = cnt[ln] % nstage;
-          mbar_wait(empty_bar(ln, st), ((cnt[ln] / nstage) & 1) ^ 1);
-          mbar_expect_tx(full_bar(ln, st), box_bytes);
-          tma_load_5d(stage_addr(ln, st), &tmap, full_bar(ln, st), 0, s.x0 - d, s.in_row, 0, s.b);
-          cnt[ln]++;
+          for (int k = 0; k < C / 8; ++k)
+            bulk_load(dst + (uint32_t)k * plane + pre, src + (size_t)k * plane_bytes, mid, bar);
+          if (fill) {
+#pragma unroll
+            for (int k = 0; k < C / 8; ++k) {
+              if (pre) bulk_load(dst + (uint32_t)k * plane, g_zeros, pre, bar);
+              if (post) bulk_load(dst + (uint32_t)k * plane + pre + mid, g_zeros, post, bar);
+            }
+          }
+        }
+        __syncwarp();
+        fills_left -= fill ? 1 : 0;
+        if (++st == (uint32_t)nstage) {
+          st = 0;
+          empty_par ^= 1u;
         }
       }
     }
-  } else if (warp == 1) {
-    // =========================== MMA issuer ===========================
-    if (lane == 0) {
-      mbar_wait(wbar, 0);
-      LaneIter it[2];
-      it[0].init(geo, 2 * blockIdx.x, nlanes);
-      it[1].init(geo, 2 * blockIdx.x + 1, nlanes);
-      uint32_t cnt[2] = {0, 0}, u[2] = {0, 0};
-      bool more[2] = {true, true};
-      constexpr uint32_t idesc = umma_idesc(kTileM, 3 * C);
-      const uint32_t plane = (uint32_t)(kTileM + 2 * d) * 16u;  // bytes between channel chunks (A)
-      constexpr uint32_t wplane = 5u * C * 16u;                 // bytes between channel chunks (B)
-      while (more[0] || more[1]) {
-#pragma unroll
-        for (int ln = 0; ln < 2; ++ln) {
-          if (!more[ln]) continue;
-          Step s;
-          more[ln] = it[ln].next(geo, s);
-          if (!more[ln]) continue;
-          const uint32_t uu = u[ln]++;
-          int st = 0;
-          if (s.in_valid) {
-            st = cnt[ln] % nstage;
-            mbar_wait(full_bar(ln, st), (cnt[ln] / nstage) & 1);
-            cnt[ln]++;
-          }
-          mbar_wait(acc_free_bar(ln), uu & 1);  // slot (uu+2)%3 re-initialised by the epilogue
-          tc_fence_after();
-          if (s.in_valid) {
-            // rows stored as ky = (1,0,2,1,0): window start for uu%3 = 0,1,2 is block 0,2,1
-            const uint32_t m = uu % 3u;
-            const uint32_t win = m == 0 ? 0u : (m == 1 ? 2u : 1u);
-            const uint32_t a0 = stage_addr(ln, st);
-            const uint32_t b0 = sbase + L.w_off + win * C * 16u;
-            const uint32_t dcol = tmem_base + (uint32_t)ln * kLaneCols;
+  } else if (warp == 1 || warp == 3) {
+    // =========================== MMA issuers: warp 1 -> lane 0, warp 3 -> lane 1 ==========
+    // One issuing warp per lane: the tensor pipe's instruction queue is short, so while one
+    // warp is busy with barriers and bookkeeping between two steps the other one's MMAs keep
+    // the pipe fed (the lanes are independent: own TMEM columns, own stages).
+    const int ln = warp >> 1;
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    PROF_ADD(0, clock64() - t_begin);
+    PROF_WAIT(2, mbar_wait(wbar, 0));
+    constexpr uint32_t idesc = umma_idesc(kTileM, 3 * C);
+    const uint32_t plane16 = (uint32_t)(kTileM + 2 * d);  // (bytes between channel chunks of A) / 16
+    constexpr uint32_t wplane16 = 5u * C;                 // same for B
+    // descriptor = {hi: SBO = 128 B, version 1; lo: LBO << 16 | start address >> 4}
+    constexpr uint32_t desc_hi = (128u >> 4) | (1u << 14);
+    const uint32_t a_lo_base = (plane16 << 16) | (((sbase + L.stage_off) >> 4) & 0x3FFFu);
+    const uint32_t b_lo_base = (wplane16 << 16) | (((sbase + L.w_off) >> 4) & 0x3FFFu);
+    const uint32_t stage16 = L.stage_bytes >> 4;
+    const uint32_t dcol = __shfl_sync(0xffffffffu, tmem_base, 0) + (uint32_t)ln * kLaneCols;
+    LaneRuns runs;
+    runs.init(geo, 2 * blockIdx.x + ln, nlanes);
+    Run run;
+    uint32_t st = 0, full_par = 0, free_par = 0, m = 0;
+    while (runs.next(geo, run)) {
+      int row = run.r + (run.i0 - 1) * d;
+      for (int j = 0; j < run.n + 2; ++j, row += d) {
+        const bool in_valid = row >= 0 && row < geo.H;
+        if (in_valid) PROF_WAIT(3, mbar_wait(full_bar(ln, st), full_par));
+        PROF_WAIT(4, mbar_wait(acc_free_bar(ln), free_par));  // slot (u+2)%3 re-initialised by the epilogue
+        free_par ^= 1u;
+        tc_fence_after();
+        // rows stored as ky = (1,0,2,1,0): window start for u%3 = 0,1,2 is block 0,2,1
+        const uint32_t win = m == 0 ? 0u : (m == 1 ? 2u : 1u);
+        const uint32_t a_lo = a_lo_base + ((uint32_t)ln * nstage + st) * stage16;
+        const uint32_t b_lo = b_lo_base + win * C;
+        PROF_T(t_issue);
+        if (elect_one()) {
+          if (in_valid) {
 #pragma unroll
             for (int kx = 0; kx < 3; ++kx) {
 #pragma unroll
               for (int ks = 0; ks < C / 16; ++ks) {
-                const uint64_t ad = umma_desc(a0 + (uint32_t)(2 * ks) * plane + (uint32_t)(kx * d) * 16u, plane, 128u);
-                const uint64_t bd = umma_desc(b0 + (uint32_t)(kx * (C / 8) + 2 * ks) * wplane, wplane, 128u);
-                tc_mma(dcol, ad, bd, idesc, 1u);
+                const uint32_t al = a_lo + (uint32_t)(2 * ks) * plane16 + (uint32_t)(kx * d);
+                const uint32_t bl = b_lo + (uint32_t)(kx * (C / 8) + 2 * ks) * wplane16;
+                tc_mma(dcol, ((uint64_t)desc_hi << 32) | al, ((uint64_t)desc_hi << 32) | bl, idesc, 1u);
               }
             }
             tc_commit(empty_bar(ln, st));
           }
           tc_commit(acc_full_bar(ln));
         }
+        __syncwarp();
+        PROF_ADD(8, clock64() - t_issue);
+        if (in_valid && ++st == (uint32_t)nstage) {
+          st = 0;
+          full_par ^= 1u;
+        }
+        m = m == 2 ? 0u : m + 1u;
       }
     }
+    PROF_ADD(5, clock64() - t_begin);
   } else if (warp >= 4) {
     // =========================== epilogue ===========================
     const int ln = (warp - 4) >> 2;
     const int qd = warp & 3;  // TMEM lane quadrant this warp may access
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     const int px = qd * 32 + lane;
     const uint32_t tlane = tmem_base + ((uint32_t)(qd * 32) << 16) + (uint32_t)ln * kLaneCols;
     auto init_slot = [&](uint32_t slot) {
@@ -370,55 +442,76 @@ __global__ void __launch_bounds__(kThreads, 1)
     __syncwarp();
     if (lane == 0) mbar_arrive(acc_free_bar(ln));
 
-    LaneIter it;
-    it.init(geo, 2 * blockIdx.x + ln, nlanes);
-    Step s;
-    uint32_t u = 0;
     const size_t plane_px = (size_t)geo.H * geo.W;
-    while (it.next(geo, s)) {
-      const uint32_t uu = u++;
-      const uint32_t slot = (uu + 2u) % 3u;  // output whose centre input was step uu-1
-      const int x = s.x0 + px;
-      const bool store = s.out_valid && x < geo.W;
-      uint4 res[C / 8];
-      size_t pix = 0;
-      if (store) {
-        pix = ((size_t)s.b * (C / 8) * geo.H + s.out_row) * geo.W + x;
-        const uint4* rp = reinterpret_cast<const uint4*>(in);
+    const uint32_t plane = (uint32_t)(kTileM + 2 * d) * 16u;
+    // The residual operand of an output row is its own centre input row, which the previous
+    // step of this lane loaded into a stage: it is read from shared memory (no second trip
+    // to L2), and that stage is handed back to the producer only afterwards (the empty
+    // barrier counts the MMA commit plus one arrival per epilogue warp).
+    LaneRuns runs;
+    runs.init(geo, 2 * blockIdx.x + ln, nlanes);
+    Run run;
+    uint32_t slot = 2, acc_par = 0, st = 0, full_par = 0;
+    uint32_t prev_st = 0, prev_par = 0;
+    bool prev_valid = false;
+    while (runs.next(geo, run)) {
+      const int x = run.x0 + px;
+      int row = run.r + (run.i0 - 1) * d;  // input row of the step; the output row is row - d
+      uint4* orow = reinterpret_cast<uint4*>(out) +
+                    ((size_t)run.b * (C / 8) * geo.H * geo.W + (long long)(row - d) * geo.W + x);
+      for (int j = 0; j < run.n + 2; ++j, row += d, orow += (size_t)d * geo.W) {
+        const bool in_valid = row >= 0 && row < geo.H;
+        const bool out_valid = j >= 2 && row - d < geo.H;
+        const bool store = out_valid && x < geo.W;
+        PROF_WAIT(6, mbar_wait(acc_full_bar(ln), acc_par));
+        acc_par ^= 1u;
+        tc_fence_after();
+        uint32_t acc[C];
+        if (out_valid) {
 #pragma unroll
-        for (int k = 0; k < C / 8; ++k) res[k] = __ldg(rp + pix + (size_t)k * plane_px);
-      }
-      __syncwarp();  // the tcgen05 ld/st below are warp-collective (.sync.aligned)
-      mbar_wait(acc_full_bar(ln), uu & 1);
-      tc_fence_after();
-      uint32_t acc[C];
-      if (s.out_valid) {
-#pragma unroll
-        for (int g16 = 0; g16 < C / 16; ++g16)
-          tc_ld16(tlane + slot * C + g16 * 16, *reinterpret_cast<uint32_t(*)[16]>(&acc[g16 * 16]));
-        tc_wait_ld();
-      }
-      init_slot(slot);
-      tc_wait_st();
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(acc_free_bar(ln));
-      if (store) {
-        uint4* op = reinterpret_cast<uint4*>(out);
-#pragma unroll
-        for (int k = 0; k < C / 8; ++k) {
-          const uint32_t rw[4] = {res[k].x, res[k].y, res[k].z, res[k].w};
-          uint32_t ow[4];
-#pragma unroll
-          for (int i = 0; i < 4; ++i) {
-            float r0 = __uint_as_float(rw[i] << 16), r1 = __uint_as_float(rw[i] & 0xffff0000u);
-            float v0 = r0 + fmaxf(__uint_as_float(acc[k * 8 + 2 * i]), 0.0f);
-            float v1 = r1 + fmaxf(__uint_as_float(acc[k * 8 + 2 * i + 1]), 0.0f);
-            __nv_bfloat162 h = __floats2bfloat162_rn(v0, v1);
-            ow[i] = *reinterpret_cast<uint32_t*>(&h);
-          }
-          op[pix + (size_t)k * plane_px] = make_uint4(ow[0], ow[1], ow[2], ow[3]);
+          for (int g16 = 0; g16 < C / 16; ++g16)
+            tc_ld16(tlane + slot * C + g16 * 16, *reinterpret_cast<uint32_t(*)[16]>(&acc[g16 * 16]));
+          tc_wait_ld();
         }
+        init_slot(slot);
+        tc_wait_st();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(acc_free_bar(ln));
+        if (prev_valid) {
+          if (store) {
+            mbar_wait(full_bar(ln, prev_st), prev_par);  // complete long ago: makes the TMA writes visible
+            const uint4* rp = reinterpret_cast<const uint4*>(smem + (stage_addr(ln, prev_st) - sbase) +
+                                                             (uint32_t)(d + px) * 16u);
+#pragma unroll
+            for (int k = 0; k < C / 8; ++k) {
+              const uint4 res = rp[(size_t)k * (plane / 16u)];
+              const uint32_t rw[4] = {res.x, res.y, res.z, res.w};
+              uint32_t ow[4];
+#pragma unroll
+              for (int i = 0; i < 4; ++i) {
+                float r0 = __uint_as_float(rw[i] << 16), r1 = __uint_as_float(rw[i] & 0xffff0000u);
+                float v0 = r0 + fmaxf(__uint_as_float(acc[k * 8 + 2 * i]), 0.0f);
+                float v1 = r1 + fmaxf(__uint_as_float(acc[k * 8 + 2 * i + 1]), 0.0f);
+                __nv_bfloat162 h = __floats2bfloat162_rn(v0, v1);
+                ow[i] = *reinterpret_cast<uint32_t*>(&h);
+              }
+              orow[(size_t)k * plane_px] = make_uint4(ow[0], ow[1], ow[2], ow[3]);
+            }
+          }
+          __syncwarp();
+          if (lane == 0) mbar_arrive(empty_bar(ln, prev_st));
+        }
+        prev_valid = in_valid;
+        if (in_valid) {
+          prev_st = st;
+          prev_par = full_par;
+          if (++st == (uint32_t)nstage) {
+            st = 0;
+            full_par ^= 1u;
+          }
+        }
+        slot = slot == 2 ? 0u : slot + 1u;
       }
     }
   }
@@ -426,6 +519,8 @@ __global__ void __launch_bounds__(kThreads, 1)
   // ---- teardown
   tc_fence_before();
   __syncthreads();
+  if (threadIdx.x == 0) PROF_ADD(7, clock64() - t_begin);
+  PROF_FLUSH(threadIdx.x == 0 || threadIdx.x == 32 || threadIdx.x == 128)
   if (warp == 2) {
     tc_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(kTmemCols) : "memory");
@@ -433,23 +528,6 @@ __global__ void __launch_bounds__(kThreads, 1)
 }
 
 // ------------------------------------------------------------------------------ host side
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*,
-                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
-                                  CUtensorMapFloatOOBfill);
-
-EncodeTiledFn get_encode() {
-  static EncodeTiledFn fn = nullptr;
-  if (!fn) {
-    void* p = nullptr;
-    cudaDriverEntryPointQueryResult q;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
-        q == cudaDriverEntryPointSuccess)
-      fn = reinterpret_cast<EncodeTiledFn>(p);
-  }
-  return fn;
-}
-
 uint16_t bf16_bits(float f) {
   uint32_t u;
   std::memcpy(&u, &f, 4);
@@ -459,17 +537,26 @@ uint16_t bf16_bits(float f) {
 }
 
 template <int C>
-cudaError_t launch_c(const CUtensorMap& map, const void* in, void* out, Geo geo, const void* wpack,
-                     const float* bias, int nstage, int grid, size_t smem, cudaStream_t st) {
+cudaError_t launch_c(const void* in, void* out, Geo geo, const void* wpack, const float* bias, int nstage,
+                     int grid, size_t smem, cudaStream_t st) {
   static bool attr_done = false;
   if (!attr_done) {
     cudaError_t e = cudaFuncSetAttribute(conv_umma_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) return e;
     attr_done = true;
   }
-  conv_umma_kernel<C><<<grid, kThreads, smem, st>>>(map, (const __nv_bfloat16*)in, (__nv_bfloat16*)out, geo,
-                                                    (const uint8_t*)wpack, bias, nstage);
-  return cudaGetLastError();
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3((unsigned)grid);
+  cfg.blockDim = dim3(kThreads);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, conv_umma_kernel<C>, (const __nv_bfloat16*)in, (__nv_bfloat16*)out, geo,
+                            (const uint8_t*)wpack, bias, nstage);
 }
 
 }  // namespace
@@ -478,8 +565,6 @@ struct UmmaPlan {
   const void* buf[2];
   ActShape s;
   int n_sm;
-  CUtensorMap maps[2][9];  // [buffer][dilation]
-  bool have[2][9];
 };
 
 size_t umma_packed_weight_bytes(int C) { return (size_t)30 * C * C; }
@@ -502,10 +587,6 @@ void umma_pack_weights_host(int C, const float* w /*[C][C][3][3]*/, void* dst) {
 }
 
 UmmaPlan* umma_plan_create(const void* buf0, const void* buf1, ActShape s, int n_sm, char* err, size_t errlen) {
-  if (!get_encode()) {
-    snprintf(err, errlen, "cuTensorMapEncodeTiled not available from the driver");
-    return nullptr;
-  }
   if (s.C % 16 || s.C < 16 || s.C > 64) {
     snprintf(err, errlen, "channels must be 16/32/48/64");
     return nullptr;
@@ -515,7 +596,6 @@ UmmaPlan* umma_plan_create(const void* buf0, const void* buf1, ActShape s, int n
   p->buf[1] = buf1;
   p->s = s;
   p->n_sm = n_sm;
-  std::memset(p->have, 0, sizeof p->have);
   return p;
 }
 
@@ -526,24 +606,6 @@ cudaError_t launch_conv_umma(UmmaPlan* p, int src, int dil, const void* wpack, c
   if (!p || dil < 1 || dil > 8 || src < 0 || src > 1) return cudaErrorInvalidValue;
   const ActShape& s = p->s;
   if (s.B <= 0) return cudaSuccess;
-  if (!p->have[src][dil]) {
-    // act[b][k][y][x][8] as a rank-5 tensor (8, W, H, C/8, B); box = one row segment with its
-    // horizontal halo, all channel chunks.  Out-of-bounds elements are zero-filled: that IS the
-    // convolution's zero padding (and the ragged right edge).
-    cuuint64_t gdim[5] = {8, (cuuint64_t)s.W, (cuuint64_t)s.H, (cuuint64_t)(s.C / 8), (cuuint64_t)s.B};
-    cuuint64_t gstr[4] = {16, (cuuint64_t)s.W * 16, (cuuint64_t)s.W * s.H * 16,
-                          (cuuint64_t)s.W * s.H * (s.C / 8) * 16};
-    cuuint32_t box[5] = {8, (cuuint32_t)(kTileM + 2 * dil), 1, (cuuint32_t)(s.C / 8), 1};
-    cuuint32_t estr[5] = {1, 1, 1, 1, 1};
-    CUresult r = get_encode()(&p->maps[src][dil], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 5, const_cast<void*>(p->buf[src]),
-                              gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                              CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (r != CUDA_SUCCESS) {
-      snprintf(err, errlen, "cuTensorMapEncodeTiled failed (%d) for %dx%dx%dx%d d=%d", (int)r, s.B, s.C, s.H, s.W, dil);
-      return cudaErrorInvalidValue;
-    }
-    p->have[src][dil] = true;
-  }
   Geo geo;
   geo.B = s.B;
   geo.H = s.H;
@@ -555,7 +617,8 @@ cudaError_t launch_conv_umma(UmmaPlan* p, int src, int dil, const void* wpack, c
   // stages: as many as fit next to the resident weights (<= kMaxStages)
   int nstage = kMaxStages;
   SmemLayout L = smem_layout(s.C, dil, nstage);
-  while (nstage > 1 && L.total + 1024 > 227u * 1024u) L = smem_layout(s.C, dil, --nstage);
+  // (>= 2: a stage is released only by the epilogue of the following step)
+  while (nstage > 2 && L.total + 1024 > 227u * 1024u) L = smem_layout(s.C, dil, --nstage);
   if (L.total + 1024 > 227u * 1024u) {
     snprintf(err, errlen, "shared memory budget exceeded");
     return cudaErrorInvalidValue;
@@ -567,10 +630,10 @@ cudaError_t launch_conv_umma(UmmaPlan* p, int src, int dil, const void* wpack, c
   const void* in = p->buf[src];
   void* out = const_cast<void*>(p->buf[src ^ 1]);
   switch (s.C) {
-    case 16: return launch_c<16>(p->maps[src][dil], in, out, geo, wpack, bias, nstage, grid, smem, st);
-    case 32: return launch_c<32>(p->maps[src][dil], in, out, geo, wpack, bias, nstage, grid, smem, st);
-    case 48: return launch_c<48>(p->maps[src][dil], in, out, geo, wpack, bias, nstage, grid, smem, st);
-    case 64: return launch_c<64>(p->maps[src][dil], in, out, geo, wpack, bias, nstage, grid, smem, st);
+    case 16: return launch_c<16>(in, out, geo, wpack, bias, nstage, grid, smem, st);
+    case 32: return launch_c<32>(in, out, geo, wpack, bias, nstage, grid, smem, st);
+    case 48: return launch_c<48>(in, out, geo, wpack, bias, nstage, grid, smem, st);
+    case 64: return launch_c<64>(in, out, geo, wpack, bias, nstage, grid, smem, st);
   }
   return cudaErrorInvalidValue;
 }
