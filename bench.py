@@ -185,8 +185,8 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    def timed(frames_t, out_t, steps, conv_timing=False):
-        loc.conv_timing(conv_timing)
+    def timed(frames_t, out_t, steps, kernel_timing=False):
+        loc.kernel_timing(kernel_timing)
         barrier()
         l0 = loc.launch_count()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -201,9 +201,10 @@ def main():
         st = loc.check()
         if st != P.OK:
             raise SystemExit(f"smlm_check: {st} {loc.last_error()}")
-        conv_ms, conv_n = loc.conv_time_ms() if conv_timing else (0.0, 0)
-        loc.conv_timing(False)
-        return ms, [int(c.value) for c in counts], loc.launch_count() - l0, conv_ms, conv_n
+        kt = {k: loc.kernel_time_ms(k) for k in (P.KERNEL_STEM, P.KERNEL_CONV, P.KERNEL_POST)} \
+            if kernel_timing else None
+        loc.kernel_timing(False)
+        return ms, [int(c.value) for c in counts], loc.launch_count() - l0, kt
 
     # warm-up (device-resident and end-to-end paths)
     timed(frames_dev, out_dev, args.warmup)
@@ -211,11 +212,12 @@ def main():
 
     sampler = ClockSampler(local)
     sampler.start()
-    ms, counts, launches, _, _ = timed(frames_dev, out_dev, args.steps)
-    ms_e2e, counts_e2e, _, _, _ = timed(frames_host, out_host, args.steps)
+    ms, counts, launches, _ = timed(frames_dev, out_dev, args.steps)
+    ms_e2e, counts_e2e, _, _ = timed(frames_host, out_host, args.steps)
     # roofline pass: the same steps with every K2 launch bracketed by CUDA events on the
     # launching stream (the events serialise a little, so `value` is not taken from this pass)
-    ms_rf, _, _, conv_ms, conv_n = timed(frames_dev, out_dev, args.steps, conv_timing=True)
+    ms_rf, _, _, kt = timed(frames_dev, out_dev, args.steps, kernel_timing=True)
+    conv_ms, conv_n = kt[P.KERNEL_CONV]
     sampler.stop_flag.set()
     sampler.join(timeout=2)
 
@@ -250,6 +252,21 @@ def main():
                     "frac_of_burst": achieved / float(peaks["bf16_tflops"]),
                     "launches": conv_n, "avg_launch_ms": conv_ms / conv_n,
                     "share_of_step": conv_ms / ms_rf}
+    # K1 / K3: bytes moved per launch / CUDA-event time, against the
+    # measured HBM copy bandwidth (the maps they touch are L2-resident in this pipeline, so
+    # this is "bytes moved", not DRAM traffic).
+    io_kernels = {}
+    if kt is not None:
+        px = float(H) * W * n_frames * args.steps
+        emit_bytes = 32.0 * sum(counts)
+        for name, kind, nbytes in (("stem (K1)", P.KERNEL_STEM, px * (2 + 2 * C)),
+                                   ("heads+post (K3)", P.KERNEL_POST, px * 4 + emit_bytes)):
+            k_ms, k_n = kt[kind]
+            if k_n > 0 and k_ms > 0:
+                gbs = nbytes / (k_ms * 1e-3) / 1e9
+                io_kernels[name] = {"achieved_GBs": gbs, "frac_of_hbm": gbs / float(peaks["hbm_gbs"]),
+                                    "launches": k_n, "avg_launch_ms": k_ms / k_n,
+                                    "share_of_step": k_ms / ms_rf}
     cpu = None
     if not args.no_cpu_baseline:
         ns = 4 if H * W <= 256 * 256 else 1
@@ -274,6 +291,7 @@ def main():
         "gpu_launches": launches,
         "clocks": sampler.summary(),
         "roofline": roofline,
+        "io_kernels": io_kernels,
         "cpu_baseline": cpu,
         "tensor_frac_whole_step": (cfg.net.flop_per_px() * H * W * n_frames * args.steps / (ms_max * 1e-3) / 1e12)
                                   / float(peaks["bf16_tflops"]),

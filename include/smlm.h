@@ -152,11 +152,14 @@ const char* smlm_last_error(const smlm_ctx* ctx);
 /* Number of kernel launches this ctx has enqueued so far (bench.py's `gpu_launches`). */
 int64_t smlm_launch_count(const smlm_ctx* ctx);
 
-/* Timing of the dominant kernel: when enabled, every trunk-convolution launch is bracketed
- * by CUDA events on the launching stream; smlm_conv_time_ms sums them (after a stream
- * sync) and reports the number of launches.  Disabled by default (events cost ~1 us). */
-smlm_status smlm_conv_timing(smlm_ctx* ctx, int32_t enable);
-smlm_status smlm_conv_time_ms(smlm_ctx* ctx, double* total_ms, int64_t* launches);
+/* Per-kernel timing for bench.py's roofline: when enabled, every launch of K1 (stem), K2
+ * (trunk convolution) and K3 (heads + post-processing) is bracketed by CUDA events on the
+ * launching stream; smlm_kernel_time_ms (after a stream sync) sums the launches of one kind
+ * since timing was last enabled.  Disabled by default: the events cost ~1 us each and switch
+ * off the programmatic overlap between consecutive layers. */
+enum { SMLM_KERNEL_STEM = 0, SMLM_KERNEL_CONV = 1, SMLM_KERNEL_POST = 2 };
+smlm_status smlm_kernel_timing(smlm_ctx* ctx, int32_t enable);
+smlm_status smlm_kernel_time_ms(smlm_ctx* ctx, int32_t kind, double* total_ms, int64_t* launches);
 
 /*
  * Test/debug exports.  BASELINE.json asks for parity on the raw output maps, which the

@@ -19,9 +19,10 @@ FP32, BF16 = 0, 1
 CONV_AUTO, CONV_TCGEN05, CONV_DIRECT = 0, 1, 2
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED_DEVICE, ERR_CUDA, ERR_OOM, ERR_OVERFLOW = 0, -1, -2, -3, -4, -5
 ABI_VERSION = 1
+KERNEL_STEM, KERNEL_CONV, KERNEL_POST = 0, 1, 2
 
 EXPORTS = ["smlm_create", "smlm_localize", "smlm_check", "smlm_destroy", "smlm_last_error",
-           "smlm_launch_count", "smlm_conv_timing", "smlm_conv_time_ms",
+           "smlm_launch_count", "smlm_kernel_timing", "smlm_kernel_time_ms",
            "smlm_debug_forward_maps", "smlm_debug_postprocess"]
 
 
@@ -74,10 +75,10 @@ def lib():
         L.smlm_last_error.argtypes = [vp]
         L.smlm_launch_count.restype = i64
         L.smlm_launch_count.argtypes = [vp]
-        L.smlm_conv_timing.restype = C.c_int
-        L.smlm_conv_timing.argtypes = [vp, i32]
-        L.smlm_conv_time_ms.restype = C.c_int
-        L.smlm_conv_time_ms.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(i64)]
+        L.smlm_kernel_timing.restype = C.c_int
+        L.smlm_kernel_timing.argtypes = [vp, i32]
+        L.smlm_kernel_time_ms.restype = C.c_int
+        L.smlm_kernel_time_ms.argtypes = [vp, i32, C.POINTER(C.c_double), C.POINTER(i64)]
         L.smlm_debug_forward_maps.restype = C.c_int
         L.smlm_debug_forward_maps.argtypes = [vp, vp, i64, i32, i32, C.POINTER(CameraParams), vp,
                                               vp, vp]
@@ -192,12 +193,13 @@ class Localizer:
     def launch_count(self) -> int:
         return int(lib().smlm_launch_count(self._h))
 
-    def conv_timing(self, enable: bool):
-        self._check(lib().smlm_conv_timing(self._h, 1 if enable else 0))
+    def kernel_timing(self, enable: bool):
+        self._check(lib().smlm_kernel_timing(self._h, 1 if enable else 0))
 
-    def conv_time_ms(self):
+    def kernel_time_ms(self, kind: int):
+        """(total ms, launches) of KERNEL_STEM / KERNEL_CONV / KERNEL_POST since timing was enabled."""
         ms, k = C.c_double(), C.c_int64()
-        self._check(lib().smlm_conv_time_ms(self._h, C.byref(ms), C.byref(k)))
+        self._check(lib().smlm_kernel_time_ms(self._h, int(kind), C.byref(ms), C.byref(k)))
         return ms.value, k.value
 
     # -- debug exports

@@ -65,6 +65,8 @@ struct smlm_ctx {
 
   void* act[2] = {nullptr, nullptr};
   size_t act_bytes = 0;
+  float* logit = nullptr;  // detection-head map written by the last tcgen05 layer
+  size_t logit_bytes = 0;
   std::vector<PlanEntry> plans;
 
   uint16_t* slots = nullptr;  // kSlots x slot_elems
@@ -84,8 +86,9 @@ struct smlm_ctx {
   size_t cam_elems = 0;
 
   int64_t launches = 0;
-  bool conv_timing = false;
+  bool timing = false;
   std::vector<cudaEvent_t> tev;  // pairs
+  std::vector<int> tev_kind;     // one per pair
   size_t tev_used = 0;
 
   std::string err;
@@ -111,6 +114,29 @@ smlm_status fail(smlm_ctx* c, smlm_status st, const char* fmt, ...) {
       return fail(c, e_ == cudaErrorMemoryAllocation ? SMLM_ERR_OOM : SMLM_ERR_CUDA,          \
                   "%s: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__);      \
   } while (0)
+
+// kernel timing (smlm_kernel_timing): bracket one launch with two events on its stream
+smlm_status time_begin(smlm_ctx* c, int kind, cudaStream_t st, cudaEvent_t* e1) {
+  *e1 = nullptr;
+  if (!c->timing) return SMLM_OK;
+  if (c->tev_used + 2 > c->tev.size()) {
+    for (int i = 0; i < 2; ++i) {
+      cudaEvent_t e;
+      CK(c, cudaEventCreate(&e));
+      c->tev.push_back(e);
+    }
+  }
+  if (c->tev_kind.size() < c->tev.size() / 2) c->tev_kind.resize(c->tev.size() / 2);
+  c->tev_kind[c->tev_used / 2] = kind;
+  cudaEvent_t e0 = c->tev[c->tev_used++];
+  *e1 = c->tev[c->tev_used++];
+  CK(c, cudaEventRecord(e0, st));
+  return SMLM_OK;
+}
+smlm_status time_end(smlm_ctx* c, cudaEvent_t e1, cudaStream_t st) {
+  if (e1) CK(c, cudaEventRecord(e1, st));
+  return SMLM_OK;
+}
 
 enum PtrKind { PTR_DEVICE, PTR_HOST_PINNED, PTR_OTHER };
 PtrKind classify(const void* p) {
@@ -139,6 +165,12 @@ smlm_status ensure_act(smlm_ctx* c, size_t bytes) {
   c->act_bytes = 0;
   for (int i = 0; i < 2; ++i) CK(c, cudaMalloc(&c->act[i], bytes));
   c->act_bytes = bytes;
+  if (c->use_umma) {  // one fp32 per pixel: bytes / (C * 2) pixels
+    if (c->logit) cudaFree(c->logit);
+    c->logit = nullptr;
+    c->logit_bytes = bytes / ((size_t)c->d.channels * 2) * sizeof(float);
+    CK(c, cudaMalloc(&c->logit, c->logit_bytes));
+  }
   return SMLM_OK;
 }
 
@@ -162,10 +194,15 @@ smlm_status get_plan(smlm_ctx* c, ActShape s, UmmaPlan** out) {
 smlm_status run_trunk(smlm_ctx* c, const uint16_t* dev_frames, int frame_base, const ViewSet& vs,
                       ActShape s, const NormParams& np, cudaStream_t st, int* result_buf,
                       float* trunk_dump, size_t dump_view_stride, size_t dump_level_stride,
-                      cudaEvent_t after_stem) {
+                      cudaEvent_t after_stem, bool want_logit, bool* have_logit) {
+  if (have_logit) *have_logit = false;
+  cudaEvent_t te = nullptr;
+  smlm_status tr = time_begin(c, SMLM_KERNEL_STEM, st, &te);
+  if (tr != SMLM_OK) return tr;
   CK(c, launch_stem(c->bf16, dev_frames, frame_base, vs, s, np, c->w_stem, c->b_stem,
                     c->d.stem_relu, c->act[0], st));
   c->launches++;
+  if ((tr = time_end(c, te, st)) != SMLM_OK) return tr;
   if (after_stem) CK(c, cudaEventRecord(after_stem, st));
   int cur = 0;
   if (trunk_dump) {
@@ -179,29 +216,21 @@ smlm_status run_trunk(smlm_ctx* c, const uint16_t* dev_frames, int frame_base, c
   }
   for (size_t l = 0; l < c->layers.size(); ++l) {
     const Layer& L = c->layers[l];
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
-    if (c->conv_timing) {
-      if (c->tev_used + 2 > c->tev.size()) {
-        for (int i = 0; i < 2; ++i) {
-          cudaEvent_t e;
-          CK(c, cudaEventCreate(&e));
-          c->tev.push_back(e);
-        }
-      }
-      e0 = c->tev[c->tev_used++];
-      e1 = c->tev[c->tev_used++];
-      CK(c, cudaEventRecord(e0, st));
-    }
+    cudaEvent_t e1 = nullptr;
+    if ((tr = time_begin(c, SMLM_KERNEL_CONV, st, &e1)) != SMLM_OK) return tr;
     if (c->use_umma) {
       char err[256] = {0};
-      cudaError_t e = launch_conv_umma(plan, cur, L.dil, L.w_umma, L.bias, 0, st, err, sizeof err);
+      const bool head = want_logit && l + 1 == c->layers.size();
+      cudaError_t e = launch_conv_umma(plan, cur, L.dil, L.w_umma, L.bias, c->w_head, c->b_head,
+                                       head ? c->logit : nullptr, st, err, sizeof err);
+      if (head && have_logit) *have_logit = true;
       if (e != cudaSuccess)
         return fail(c, SMLM_ERR_CUDA, "conv_umma: %s %s", cudaGetErrorString(e), err);
     } else {
       CK(c, launch_conv_direct(c->bf16, c->act[cur], c->act[cur ^ 1], s, L.dil, L.w_direct, L.bias, st));
     }
     c->launches++;
-    if (e1) CK(c, cudaEventRecord(e1, st));
+    if ((tr = time_end(c, e1, st)) != SMLM_OK) return tr;
     cur ^= 1;
     if (trunk_dump) {
       CK(c, launch_dump_act(c->bf16, c->act[cur], s, trunk_dump + (l + 1) * dump_level_stride,
@@ -306,10 +335,13 @@ smlm_status store_count(smlm_ctx* c, const unsigned long long* counter, int64_t*
 
 int auto_micro_batch(const smlm_ctx* c, int Hw, int Ww) {
   if (c->d.micro_batch > 0) return c->d.micro_batch;
-  // keep the two ping-pong maps of a micro-batch inside ~3/4 of L2 (bf16: 2C B/px each)
+  // Measured on B200 (profiles/microbatch_sweep_r1.md): keeping the two ping-pong maps
+  // L2-resident (7 frames of 256x256x48) is SLOWER than streaming large micro-batches from
+  // HBM - per-launch overheads and the two halo steps per lane range weigh more than the
+  // DRAM traffic, which stays below 65 % of HBM bandwidth.  So: up to 64 views per launch,
+  // bounded by 1.5 GB per activation buffer.
   size_t per_view = (size_t)Hw * Ww * c->d.channels * elt_size(c);
-  size_t budget = c->l2_bytes ? c->l2_bytes * 3 / 8 : (size_t)48 << 20;
-  size_t b = budget / std::max<size_t>(per_view, 1);
+  size_t b = ((size_t)1536 << 20) / std::max<size_t>(per_view, 1);
   return (int)std::min<size_t>(std::max<size_t>(b, 1), 64);
 }
 
@@ -428,7 +460,7 @@ void smlm_destroy(smlm_ctx* c) {
   free_plans(c);
   cudaFree(c->w_stem); cudaFree(c->b_stem); cudaFree(c->w_head); cudaFree(c->b_head);
   for (auto& L : c->layers) { cudaFree(L.w_direct); cudaFree(L.w_umma); cudaFree(L.bias); }
-  cudaFree(c->act[0]); cudaFree(c->act[1]); cudaFree(c->slots); cudaFree(c->em_dev);
+  cudaFree(c->act[0]); cudaFree(c->act[1]); cudaFree(c->logit); cudaFree(c->slots); cudaFree(c->em_dev);
   cudaFree(c->counters); cudaFree(c->cam_off); cudaFree(c->cam_gain);
   if (c->h_count) cudaFreeHost(c->h_count);
   for (int i = 0; i < kSlots; ++i) {
@@ -449,25 +481,28 @@ const char* smlm_last_error(const smlm_ctx* c) { return c ? c->err.c_str() : g_c
 
 int64_t smlm_launch_count(const smlm_ctx* c) { return c ? c->launches : 0; }
 
-smlm_status smlm_conv_timing(smlm_ctx* c, int32_t enable) {
+smlm_status smlm_kernel_timing(smlm_ctx* c, int32_t enable) {
   if (!c) return SMLM_ERR_INVALID_ARG;
-  c->conv_timing = enable != 0;
+  c->timing = enable != 0;
   c->tev_used = 0;
   return SMLM_OK;
 }
 
-smlm_status smlm_conv_time_ms(smlm_ctx* c, double* total_ms, int64_t* launches) {
-  if (!c || !total_ms || !launches) return SMLM_ERR_INVALID_ARG;
+smlm_status smlm_kernel_time_ms(smlm_ctx* c, int32_t kind, double* total_ms, int64_t* launches) {
+  if (!c || !total_ms || !launches || kind < SMLM_KERNEL_STEM || kind > SMLM_KERNEL_POST)
+    return SMLM_ERR_INVALID_ARG;
   double tot = 0.0;
+  int64_t n = 0;
   for (size_t i = 0; i + 1 < c->tev_used; i += 2) {
+    if (c->tev_kind[i / 2] != kind) continue;
     CK(c, cudaEventSynchronize(c->tev[i + 1]));
     float ms = 0.f;
     CK(c, cudaEventElapsedTime(&ms, c->tev[i], c->tev[i + 1]));
     tot += ms;
+    ++n;
   }
   *total_ms = tot;
-  *launches = (int64_t)(c->tev_used / 2);
-  c->tev_used = 0;
+  *launches = n;
   return SMLM_OK;
 }
 
@@ -632,12 +667,20 @@ smlm_status smlm_localize(smlm_ctx* c, const uint16_t* frames, int64_t n, int32_
     for (size_t si = 0; si < sets.size(); ++si) {
       int res = 0;
       cudaEvent_t after_stem = (slot >= 0 && si + 1 == sets.size()) ? c->ev_consumed[slot] : nullptr;
+      bool have_logit = false;
       r = run_trunk(c, dev_frames, frame_base, sets[si].vs, sets[si].s, np, st, &res, nullptr, 0, 0,
-                    after_stem);
+                    after_stem, true, &have_logit);
       if (r != SMLM_OK) return r;
-      CK(c, launch_head_post(c->bf16, c->act[res], sets[si].s, sets[si].vs, c->w_head, c->b_head, hp,
-                             list, counter, capacity, st));
+      cudaEvent_t te = nullptr;
+      if ((r = time_begin(c, SMLM_KERNEL_POST, st, &te)) != SMLM_OK) return r;
+      if (have_logit)
+        CK(c, launch_post_logits(c->act[res], c->logit, sets[si].s, sets[si].vs, c->w_head, c->b_head, hp,
+                                 list, counter, capacity, st));
+      else
+        CK(c, launch_head_post(c->bf16, c->act[res], sets[si].s, sets[si].vs, c->w_head, c->b_head, hp,
+                               list, counter, capacity, st));
       c->launches++;
+      if ((r = time_end(c, te, st)) != SMLM_OK) return r;
     }
     if (host_out && wbf > 0) {
       int64_t done = f0 + nf;
@@ -684,7 +727,8 @@ smlm_status smlm_debug_forward_maps(smlm_ctx* c, const uint16_t* frames, int64_t
     ActShape s{nf, C, H, W};
     int res = 0;
     float* dump = trunk ? trunk + (size_t)f0 * (L + 1) * px * C : nullptr;
-    r = run_trunk(c, frames, 0, vs, s, np, st, &res, dump, (size_t)(L + 1) * px * C, px * C, nullptr);
+    r = run_trunk(c, frames, 0, vs, s, np, st, &res, dump, (size_t)(L + 1) * px * C, px * C, nullptr, false,
+                  nullptr);
     if (r != SMLM_OK) break;
     cudaError_t e = launch_head_maps(c->bf16, c->act[res], s, c->w_head, c->b_head, nh,
                                      maps + (size_t)f0 * nh * px, st);

@@ -223,17 +223,23 @@ __host__ __device__ inline SmemLayout smem_layout(int C, int d, int nstage) {
   L.stage_off = (L.w_off + L.w_bytes + 127u) & ~127u;
   L.nstage = nstage;
   L.bias_off = L.stage_off + 2u * nstage * L.stage_bytes;
-  L.bar_off = L.bias_off + (uint32_t)C * 4u;
+  L.bar_off = L.bias_off + (uint32_t)(2 * C + 4) * 4u;  // layer bias, detection-head row + its bias
   // barriers: wbar, per lane: full[kMaxStages], empty[kMaxStages], acc_full, acc_free
   L.tmem_off = L.bar_off + 8u * (1 + 2 * (2 * kMaxStages + 2));
   L.total = L.tmem_off + 16u;
   return L;
 }
 
-template <int C>
+// HEAD: the layer is the last one of the trunk; the epilogue additionally evaluates the
+// detection head o_p = b_p + sum_c w_p[c] a[c] on the ROUNDED output values (same order and
+// fmaf chain as head_post.cu, so both produce the same bits) and stores it as an fp32 map:
+// K3 then reads 4 B/px instead of 2C B/px.
+template <int C, bool HEAD>
 __global__ void __launch_bounds__(kThreads, 1)
     conv_umma_kernel(const __nv_bfloat16* __restrict__ in, __nv_bfloat16* __restrict__ out, Geo geo,
-                     const uint8_t* __restrict__ wpack, const float* __restrict__ bias, int nstage) {
+                     const uint8_t* __restrict__ wpack, const float* __restrict__ bias, int nstage,
+                     const float* __restrict__ head_w, const float* __restrict__ head_b,
+                     float* __restrict__ logit) {
   extern __shared__ uint8_t smem_raw[];
   const SmemLayout L = smem_layout(C, geo.d, nstage);
   const uint32_t sraw = smem_u32(smem_raw);
@@ -274,6 +280,10 @@ __global__ void __launch_bounds__(kThreads, 1)
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
   for (int i = threadIdx.x; i < C; i += kThreads) bias_s[i] = bias[i];
+  if (HEAD) {
+    for (int i = threadIdx.x; i < C; i += kThreads) bias_s[C + i] = head_w[i];
+    if (threadIdx.x == 0) bias_s[2 * C] = head_b[0];
+  }
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -483,6 +493,7 @@ __global__ void __launch_bounds__(kThreads, 1)
             mbar_wait(full_bar(ln, prev_st), prev_par);  // complete long ago: makes the TMA writes visible
             const uint4* rp = reinterpret_cast<const uint4*>(smem + (stage_addr(ln, prev_st) - sbase) +
                                                              (uint32_t)(d + px) * 16u);
+            float lg = HEAD ? bias_s[2 * C] : 0.0f;
 #pragma unroll
             for (int k = 0; k < C / 8; ++k) {
               const uint4 res = rp[(size_t)k * (plane / 16u)];
@@ -495,9 +506,14 @@ __global__ void __launch_bounds__(kThreads, 1)
                 float v1 = r1 + fmaxf(__uint_as_float(acc[k * 8 + 2 * i + 1]), 0.0f);
                 __nv_bfloat162 h = __floats2bfloat162_rn(v0, v1);
                 ow[i] = *reinterpret_cast<uint32_t*>(&h);
+                if (HEAD) {
+                  lg = fmaf(__uint_as_float(ow[i] << 16), bias_s[C + k * 8 + 2 * i], lg);
+                  lg = fmaf(__uint_as_float(ow[i] & 0xffff0000u), bias_s[C + k * 8 + 2 * i + 1], lg);
+                }
               }
               orow[(size_t)k * plane_px] = make_uint4(ow[0], ow[1], ow[2], ow[3]);
             }
+            if (HEAD) logit[((size_t)run.b * geo.H + (row - d)) * geo.W + x] = lg;
           }
           __syncwarp();
           if (lane == 0) mbar_arrive(empty_bar(ln, prev_st));
@@ -536,12 +552,14 @@ uint16_t bf16_bits(float f) {
   return (uint16_t)(u >> 16);
 }
 
-template <int C>
-cudaError_t launch_c(const void* in, void* out, Geo geo, const void* wpack, const float* bias, int nstage,
-                     int grid, size_t smem, cudaStream_t st) {
+template <int C, bool HEAD>
+cudaError_t launch_ch(const void* in, void* out, Geo geo, const void* wpack, const float* bias, int nstage,
+                      int grid, size_t smem, const float* head_w, const float* head_b, float* logit,
+                      cudaStream_t st) {
   static bool attr_done = false;
   if (!attr_done) {
-    cudaError_t e = cudaFuncSetAttribute(conv_umma_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    cudaError_t e = cudaFuncSetAttribute(conv_umma_kernel<C, HEAD>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         227 * 1024);
     if (e != cudaSuccess) return e;
     attr_done = true;
   }
@@ -555,8 +573,15 @@ cudaError_t launch_c(const void* in, void* out, Geo geo, const void* wpack, cons
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, conv_umma_kernel<C>, (const __nv_bfloat16*)in, (__nv_bfloat16*)out, geo,
-                            (const uint8_t*)wpack, bias, nstage);
+  return cudaLaunchKernelEx(&cfg, conv_umma_kernel<C, HEAD>, (const __nv_bfloat16*)in, (__nv_bfloat16*)out,
+                            geo, (const uint8_t*)wpack, bias, nstage, head_w, head_b, logit);
+}
+template <int C>
+cudaError_t launch_c(const void* in, void* out, Geo geo, const void* wpack, const float* bias, int nstage,
+                     int grid, size_t smem, const float* head_w, const float* head_b, float* logit,
+                     cudaStream_t st) {
+  return logit ? launch_ch<C, true>(in, out, geo, wpack, bias, nstage, grid, smem, head_w, head_b, logit, st)
+               : launch_ch<C, false>(in, out, geo, wpack, bias, nstage, grid, smem, head_w, head_b, logit, st);
 }
 
 }  // namespace
@@ -602,7 +627,8 @@ UmmaPlan* umma_plan_create(const void* buf0, const void* buf1, ActShape s, int n
 void umma_plan_destroy(UmmaPlan* p) { delete p; }
 
 cudaError_t launch_conv_umma(UmmaPlan* p, int src, int dil, const void* wpack, const float* bias,
-                             int /*band_rows*/, cudaStream_t st, char* err, size_t errlen) {
+                             const float* head_w, const float* head_b, float* logit, cudaStream_t st,
+                             char* err, size_t errlen) {
   if (!p || dil < 1 || dil > 8 || src < 0 || src > 1) return cudaErrorInvalidValue;
   const ActShape& s = p->s;
   if (s.B <= 0) return cudaSuccess;
@@ -630,10 +656,10 @@ cudaError_t launch_conv_umma(UmmaPlan* p, int src, int dil, const void* wpack, c
   const void* in = p->buf[src];
   void* out = const_cast<void*>(p->buf[src ^ 1]);
   switch (s.C) {
-    case 16: return launch_c<16>(in, out, geo, wpack, bias, nstage, grid, smem, st);
-    case 32: return launch_c<32>(in, out, geo, wpack, bias, nstage, grid, smem, st);
-    case 48: return launch_c<48>(in, out, geo, wpack, bias, nstage, grid, smem, st);
-    case 64: return launch_c<64>(in, out, geo, wpack, bias, nstage, grid, smem, st);
+    case 16: return launch_c<16>(in, out, geo, wpack, bias, nstage, grid, smem, head_w, head_b, logit, st);
+    case 32: return launch_c<32>(in, out, geo, wpack, bias, nstage, grid, smem, head_w, head_b, logit, st);
+    case 48: return launch_c<48>(in, out, geo, wpack, bias, nstage, grid, smem, head_w, head_b, logit, st);
+    case 64: return launch_c<64>(in, out, geo, wpack, bias, nstage, grid, smem, head_w, head_b, logit, st);
   }
   return cudaErrorInvalidValue;
 }

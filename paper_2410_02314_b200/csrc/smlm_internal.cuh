@@ -106,16 +106,24 @@ void umma_pack_weights_host(int C, const float* w_oihw, void* dst);
 UmmaPlan* umma_plan_create(const void* buf0, const void* buf1, ActShape s, int n_sm, char* err,
                            size_t errlen);
 void umma_plan_destroy(UmmaPlan*);
-// in = plan buffer `src` (0/1), out = the other one.
+// in = plan buffer `src` (0/1), out = the other one.  logit != nullptr (last layer): also
+// store the detection head o_p = head_b[0] + head_w[0..C) . out as fp32 [B][H][W].
 cudaError_t launch_conv_umma(UmmaPlan* plan, int src, int dil, const void* wpack,
-                             const float* bias, int band_rows, cudaStream_t st, char* err,
-                             size_t errlen);
+                             const float* bias, const float* head_w, const float* head_b,
+                             float* logit, cudaStream_t st, char* err, size_t errlen);
 
 // K3: 1x1 heads + threshold + 3x3 NMS + decode + warp-aggregated compaction.
 cudaError_t launch_head_post(bool bf16, const void* act, ActShape s, ViewSet vs,
                              const float* w_head /*[n_h][C]*/, const float* b_head, HeadParams hp,
                              smlm_emitter* out, unsigned long long* counter,
                              unsigned long long capacity, cudaStream_t st);
+
+// K3 after a HEAD conv layer: the detection logit comes from `logit` [B][H][W], the other
+// heads are evaluated from `act` for the survivors only.
+cudaError_t launch_post_logits(const void* act, const float* logit, ActShape s, ViewSet vs,
+                               const float* w_head, const float* b_head, HeadParams hp,
+                               smlm_emitter* out, unsigned long long* counter,
+                               unsigned long long capacity, cudaStream_t st);
 
 // debug: heads only -> fp32 maps [B][n_h][H][W] (pre-activation)
 cudaError_t launch_head_maps(bool bf16, const void* act, ActShape s, const float* w_head,

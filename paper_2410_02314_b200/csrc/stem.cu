@@ -2,9 +2,9 @@
 // fused (BASELINE.json north_star (a); smlm.h: xhat = ((adu - offset)/gain)/norm_scale,
 // a0 = act(conv3x3(xhat; W0) + b0), zero padding 1 at the FRAME border).
 //
-// HBM-bound: 2 B/px in, 2C B/px out (bf16).  One thread = one pixel, all C channels; a warp
-// covers 32 consecutive pixels of a row, so each of its C/8 stores is one dense 512 B run
-// in the chunk-planar layout.  The normalised (TY+2) x (TX+2) input patch is staged in
+// HBM/L2-write-bound: 2 B/px in, 2C B/px out (bf16).  One thread = four pixels 32 apart, all
+// C channels; a warp covers 32 consecutive pixels of a row per store, so each store is one
+// dense 512 B run in the chunk-planar layout.  The normalised (TY+2) x (TX+2) input patch is staged in
 // shared memory once per block (the divisions happen once per pixel, not once per tap).
 #include "chunk_io.cuh"
 #include "smlm_internal.cuh"
@@ -12,79 +12,130 @@
 namespace smlm {
 namespace {
 
-constexpr int TX = 64, TY = 4;
+constexpr int TX = 128, PX = 4;  // tile = 128 pixels of one row; pixels per thread (x, x+32, x+64, x+96)
+constexpr int NW = 4;            // warps per block, one tile each per round
 
+// Persistent blocks: tile t = (view, row, 128-px segment); warp w of block j takes tiles
+// (j * NW + w), + gridDim.x * NW, ...  With 5 blocks per SM the tail is one row-tile.
 template <typename T, int C>
-__global__ void __launch_bounds__(TX* TY)
+__global__ void __launch_bounds__(32 * NW)
     stem_kernel(const uint16_t* __restrict__ frames, int frame_base, ViewSet vs, ActShape s,
                 NormParams np, const float* __restrict__ w /*[9][C]*/,
                 const float* __restrict__ bias, int relu, T* __restrict__ act) {
-  __shared__ float xs[TY + 2][TX + 2];
+  __shared__ float xs[NW][3][TX + 2];
   __shared__ __align__(16) float ws[9][C];
   __shared__ __align__(16) float bs[C];
 
-  const int b = blockIdx.z;
-  const View v = view_of(vs, b, s.H, s.W);
-  const int tid = threadIdx.y * TX + threadIdx.x;
-  for (int i = tid; i < 9 * C; i += TX * TY) ws[i / C][i % C] = w[i];
-  for (int i = tid; i < C; i += TX * TY) bs[i] = bias[i];
-
-  const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
-  const uint16_t* frame = frames + (size_t)(v.frame - frame_base) * vs.Hf * vs.Wf;
-  const float inv_scalar = 1.0f / (np.gain * np.norm_scale);
-  for (int i = tid; i < (TY + 2) * (TX + 2); i += TX * TY) {
-    int ly = i / (TX + 2), lx = i - ly * (TX + 2);
-    int fy = v.wy0 + y0 + ly - 1, fx = v.wx0 + x0 + lx - 1;  // frame coordinates
-    float xn = 0.0f;
-    if (fy >= 0 && fy < vs.Hf && fx >= 0 && fx < vs.Wf) {
-      size_t q = (size_t)fy * vs.Wf + fx;
-      float adu = (float)frame[q];
-      if (np.offset_map)
-        xn = ((adu - np.offset_map[q]) / np.gain_map[q]) / np.norm_scale;
-      else
-        xn = (adu - np.offset) * inv_scalar;
-    }
-    xs[ly][lx] = xn;
-  }
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  for (int i = tid; i < 9 * C; i += 32 * NW) ws[i / C][i % C] = w[i];
+  for (int i = tid; i < C; i += 32 * NW) bs[i] = bias[i];
   __syncthreads();
 
-  const int x = x0 + threadIdx.x, y = y0 + threadIdx.y;
-  if (x >= s.W || y >= s.H) return;
-  float xn[9];
+  const int nseg = (s.W + TX - 1) / TX;
+  const long long ntiles = (long long)s.B * s.H * nseg;
+  const float inv_scalar = 1.0f / (np.gain * np.norm_scale);
+  constexpr int PATCH = 3 * (TX + 2), NLD = (PATCH + 31) / 32;
+  for (long long t = (long long)blockIdx.x * NW + warp; t < ntiles; t += (long long)gridDim.x * NW) {
+    const int seg = (int)(t % nseg);
+    const long long ty = t / nseg;
+    const int y = (int)(ty % s.H), b = (int)(ty / s.H);
+    const int x0 = seg * TX;
+    const View v = view_of(vs, b, s.H, s.W);
+    const uint16_t* frame = frames + (size_t)(v.frame - frame_base) * vs.Hf * vs.Wf;
+    // all loads of the 3 x 130 patch first (independent, one round trip), then the arithmetic
+    float adu[NLD], om[NLD], gm[NLD];
+    bool ok[NLD];
 #pragma unroll
-  for (int ky = 0; ky < 3; ++ky)
-#pragma unroll
-    for (int kx = 0; kx < 3; ++kx) xn[ky * 3 + kx] = xs[threadIdx.y + ky][threadIdx.x + kx];
-
-#pragma unroll
-  for (int k = 0; k < C / 8; ++k) {
-    float acc[8];
-#pragma unroll
-    for (int c = 0; c < 8; ++c) acc[c] = bs[k * 8 + c];
-#pragma unroll
-    for (int t = 0; t < 9; ++t)
-#pragma unroll
-      for (int c = 0; c < 8; ++c) acc[c] = fmaf(xn[t], ws[t][k * 8 + c], acc[c]);
-    if (relu) {
-#pragma unroll
-      for (int c = 0; c < 8; ++c) acc[c] = fmaxf(acc[c], 0.0f);
+    for (int r = 0; r < NLD; ++r) {
+      const int i = lane + r * 32;
+      const int ly = i / (TX + 2), lx = i - ly * (TX + 2);
+      const int fy = v.wy0 + y + ly - 1, fx = v.wx0 + x0 + lx - 1;  // frame coordinates
+      ok[r] = i < PATCH && fy >= 0 && fy < vs.Hf && fx >= 0 && fx < vs.Wf;
+      const size_t q = ok[r] ? (size_t)fy * vs.Wf + fx : 0;
+      adu[r] = ok[r] ? (float)__ldg(frame + q) : 0.0f;
+      om[r] = (ok[r] && np.offset_map) ? __ldg(np.offset_map + q) : np.offset;
+      gm[r] = (ok[r] && np.offset_map) ? __ldg(np.gain_map + q) : 1.0f;
     }
-    Chunk<T>::store(act, s.chunk_index(b, k, y, x), acc);
+    __syncwarp();  // the previous tile's reads of xs[warp] are done
+#pragma unroll
+    for (int r = 0; r < NLD; ++r) {
+      const int i = lane + r * 32;
+      if (i >= PATCH) continue;
+      float xn = 0.0f;
+      if (ok[r]) xn = np.offset_map ? ((adu[r] - om[r]) / gm[r]) / np.norm_scale : (adu[r] - om[r]) * inv_scalar;
+      xs[warp][i / (TX + 2)][i % (TX + 2)] = xn;
+    }
+    __syncwarp();
+
+    // Each thread owns PX pixels 32 apart in x: a weight read from shared memory feeds PX
+    // FMAs, and every store of the warp is one dense 512-byte run.
+    float xn[PX][9];
+#pragma unroll
+    for (int p = 0; p < PX; ++p)
+#pragma unroll
+      for (int ky = 0; ky < 3; ++ky)
+#pragma unroll
+        for (int kx = 0; kx < 3; ++kx) xn[p][ky * 3 + kx] = xs[warp][ky][lane + 32 * p + kx];
+
+#pragma unroll 1
+    for (int k = 0; k < C / 8; ++k) {  // not unrolled: keeps the loop body inside the instruction cache
+      float acc[PX][8];
+#pragma unroll
+      for (int c = 0; c < 8; ++c) {
+        const float bv = bs[k * 8 + c];
+#pragma unroll
+        for (int p = 0; p < PX; ++p) acc[p][c] = bv;
+      }
+#pragma unroll
+      for (int tp = 0; tp < 9; ++tp)
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+          const float wv = ws[tp][k * 8 + c];
+#pragma unroll
+          for (int p = 0; p < PX; ++p) acc[p][c] = fmaf(xn[p][tp], wv, acc[p][c]);
+        }
+#pragma unroll
+      for (int p = 0; p < PX; ++p) {
+        const int x = x0 + lane + 32 * p;
+        if (x >= s.W) continue;
+        if (relu) {
+#pragma unroll
+          for (int c = 0; c < 8; ++c) acc[p][c] = fmaxf(acc[p][c], 0.0f);
+        }
+        Chunk<T>::store(act, s.chunk_index(b, k, y, x), acc[p]);
+      }
+    }
   }
+}
+
+template <typename T, int C>
+cudaError_t launch_tc(const uint16_t* frames, int frame_base, ViewSet vs, ActShape s, NormParams np,
+                      const float* w, const float* b, int relu, void* act, cudaStream_t st) {
+  static int blocks_per_wave = 0;
+  if (!blocks_per_wave) {
+    int dev = 0, n_sm = 0, per_sm = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, stem_kernel<T, C>, 32 * NW, 0);
+    blocks_per_wave = n_sm * (per_sm > 0 ? per_sm : 1);
+  }
+  const long long ntiles = (long long)s.B * s.H * ((s.W + TX - 1) / TX);
+  const long long want = (ntiles + NW - 1) / NW;
+  const int grid = (int)(want < blocks_per_wave ? want : blocks_per_wave);
+  stem_kernel<T, C><<<grid, 32 * NW, 0, st>>>(frames, frame_base, vs, s, np, w, b, relu, (T*)act);
+  return cudaGetLastError();
 }
 
 template <typename T>
 cudaError_t launch_t(const uint16_t* frames, int frame_base, ViewSet vs, ActShape s, NormParams np,
                      const float* w, const float* b, int relu, void* act, cudaStream_t st) {
-  dim3 grid((s.W + TX - 1) / TX, (s.H + TY - 1) / TY, s.B), block(TX, TY);
   switch (s.C) {
-    case 16: stem_kernel<T, 16><<<grid, block, 0, st>>>(frames, frame_base, vs, s, np, w, b, relu, (T*)act); break;
-    case 32: stem_kernel<T, 32><<<grid, block, 0, st>>>(frames, frame_base, vs, s, np, w, b, relu, (T*)act); break;
-    case 48: stem_kernel<T, 48><<<grid, block, 0, st>>>(frames, frame_base, vs, s, np, w, b, relu, (T*)act); break;
-    case 64: stem_kernel<T, 64><<<grid, block, 0, st>>>(frames, frame_base, vs, s, np, w, b, relu, (T*)act); break;
+    case 16: return launch_tc<T, 16>(frames, frame_base, vs, s, np, w, b, relu, act, st);
+    case 32: return launch_tc<T, 32>(frames, frame_base, vs, s, np, w, b, relu, act, st);
+    case 48: return launch_tc<T, 48>(frames, frame_base, vs, s, np, w, b, relu, act, st);
+    case 64: return launch_tc<T, 64>(frames, frame_base, vs, s, np, w, b, relu, act, st);
     default: return cudaErrorInvalidValue;
   }
-  return cudaGetLastError();
 }
 
 }  // namespace
