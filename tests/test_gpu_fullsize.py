@@ -1,0 +1,136 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (default
+micro-batch, frames in a pinned host ring, emitter list written back to pinned host memory,
+write-back batches where the config has them): sampled frames against the oracle, plus
+properties that hold for every frame (the stack cycles a set of distinct frames, so frame f
+and frame f + k must give the same detections; no two detections are 8-adjacent).
+"""
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from smlm_synth import get_config, make_frames, make_weights
+import paper_2410_02314_b200 as P
+import gpu_util as G
+
+pytestmark = pytest.mark.gpu
+
+
+def _stack(cfg, n, k):
+    fs = make_frames(cfg, k)
+    reps = (n + k - 1) // k
+    return fs, np.ascontiguousarray(np.concatenate([fs.frames] * reps)[:n])
+
+
+def _check_cycle_and_adjacency(em, n, k, W):
+    order = np.lexsort((em["pix"], em["frame"]))
+    em = em[order]
+    per = [em[em["frame"] == f] for f in range(min(k, n))]
+    # every frame f >= k repeats frame f - k
+    bounds = np.searchsorted(em["frame"], np.arange(n + 1))
+    for f in range(k, n):
+        a = em[bounds[f]:bounds[f + 1]]
+        b = per[f % k]
+        assert len(a) == len(b) and np.array_equal(a["pix"], b["pix"]), f
+        for key in ("x_nm", "y_nm", "photons", "bg", "p"):
+            assert np.array_equal(a[key], b[key]), (f, key)
+    # no two detections of a frame are 8-adjacent (property of the rule, G8)
+    for b in per[:4]:
+        ys, xs = b["pix"] // W, b["pix"] % W
+        grid = np.zeros((ys.max() + 3, W + 2), dtype=np.int32)
+        grid[ys + 1, xs + 1] = 1
+        nb = sum(np.roll(np.roll(grid, dy, 0), dx, 1) for dy in (-1, 0, 1) for dx in (-1, 0, 1))
+        assert int((nb * grid).max()) == 1
+    return em
+
+
+def _oracle_gate(cfg, w, fs, em, sample, tol, H, W):
+    ck = G.cam_kwargs(fs)
+    net = O.net_from_spec(cfg.net)
+    cam = O.make_camera(**ck)
+    k = len(fs.frames)
+    stats = []
+    for f in sample:
+        o = O.forward_maps(net, w, fs.frames[f % k:f % k + 1], cam)
+        em_o = O.postprocess(net, o, cam, cfg.threshold)
+        em_o["frame"] += f
+        em_g = em[em["frame"] == f]
+        stats.append(G.parity_gate(cfg.net, o, em_o, em_g, cfg.threshold, tol, fs.pixel_size_nm, H, W,
+                                   frame_offset=f))
+    return stats
+
+
+def test_cfg1_full_1000_frames_pinned_ring_sampled_against_oracle():
+    cfg = get_config(1)
+    n, k = cfg.frames.n_frames, 16
+    fs, frames = _stack(cfg, n, k)
+    w = make_weights(cfg)
+    cap = n * 4 * cfg.frames.emitters_per_frame
+    em = G.gpu_localize(cfg.net, w, frames, G.cam_kwargs(fs), cfg.threshold, capacity=cap,
+                        host_frames=True, host_out=True)
+    em = _check_cycle_and_adjacency(em, n, k, 256)
+    stats = _oracle_gate(cfg, w, fs, em, (0, 63, 64, 500, 999), 2e-2, 256, 256)
+    print("cfg1 full-size gate", stats)
+
+
+def test_cfg4_stream_2560_frames_writeback_256_sampled_against_oracle():
+    """cfg 4's launch configuration (write-back every 256 frames) on 10 write-back batches;
+    the full 10 000-frame stack differs only in the number of batches."""
+    cfg = get_config(4)
+    n, k = 2560, 8
+    fs, frames = _stack(cfg, n, k)
+    w = make_weights(cfg)
+    cap = n * 2 * cfg.frames.emitters_per_frame
+    em = G.gpu_localize(cfg.net, w, frames, G.cam_kwargs(fs), cfg.threshold, capacity=cap,
+                        host_frames=True, host_out=True, writeback_frames=cfg.writeback_batch)
+    em = _check_cycle_and_adjacency(em, n, k, 256)
+    stats = _oracle_gate(cfg, w, fs, em, (0, 255, 256, 2559), 2e-2, 256, 256)
+    print("cfg4 stream gate", stats)
+
+
+def test_cfg2_512x512_six_heads_sampled_against_oracle():
+    cfg = get_config(2)
+    n, k = 96, 2
+    fs, frames = _stack(cfg, n, k)
+    w = make_weights(cfg)
+    cap = n * 3 * cfg.frames.emitters_per_frame
+    em = G.gpu_localize(cfg.net, w, frames, G.cam_kwargs(fs), cfg.threshold, capacity=cap,
+                        host_frames=True, host_out=True)
+    em = _check_cycle_and_adjacency(em, n, k, 512)
+    stats = _oracle_gate(cfg, w, fs, em, (0, 95), 2e-2, 512, 512)
+    print("cfg2 full-frame gate", stats)
+
+
+def test_cfg3_2048_tiled_sampled_rows_against_oracle_crop():
+    """cfg 3: one full 2048x2048 frame through 512x512 tiles with per-pixel camera maps.  The
+    oracle (which never tiles) runs on a 700x700 crop that covers a 2x2 tile crossing; inside
+    the crop, at least radius+1 = 47 px from the crop's inner edges, both see the same
+    receptive fields, so detections there must agree (reading G15)."""
+    cfg = get_config(3)
+    fs = make_frames(cfg, 1)
+    w = make_weights(cfg)
+    H = W = 2048
+    ck = G.cam_kwargs(fs)
+    frames = np.ascontiguousarray(np.concatenate([fs.frames, fs.frames]))
+    em = G.gpu_localize(cfg.net, w, frames, ck, cfg.threshold, capacity=2 * 4 * cfg.frames.emitters_per_frame,
+                        host_frames=True, host_out=True, tile=cfg.tile)
+    a, b = em[em["frame"] == 0], em[em["frame"] == 1]
+    assert len(a) > 1000 and np.array_equal(a["pix"], b["pix"]) and np.array_equal(a["x_nm"], b["x_nm"])
+    # crop with its origin at the frame origin: rows/cols 0..699 (the frame border keeps its
+    # zero padding, the inner edges lose 47 px)
+    S, M = 700, 47
+    crop = np.ascontiguousarray(fs.frames[:, :S, :S])
+    ckc = dict(ck, offset_map=np.ascontiguousarray(fs.offset_map[:S, :S]),
+               gain_map=np.ascontiguousarray(fs.gain_map[:S, :S]))
+    net = O.net_from_spec(cfg.net)
+    cam = O.make_camera(**ckc)
+    o = O.forward_maps(net, w, crop, cam)
+    em_o = O.postprocess(net, o, cam, cfg.threshold)
+    inner = lambda y, x: (y < S - M) & (x < S - M)
+    yo, xo = em_o["pix"] // S, em_o["pix"] % S
+    em_o = em_o[inner(yo, xo)]
+    ya, xa = a["pix"] // W, a["pix"] % W
+    ag = a[inner(ya, xa)].copy()
+    ag["pix"] = (ya[inner(ya, xa)] * S + xa[inner(ya, xa)]).astype(np.int32)
+    st = G.parity_gate(cfg.net, o, em_o, ag, cfg.threshold, 2e-2, fs.pixel_size_nm, S, S)
+    print("cfg3 tiled vs oracle crop", st)
+    assert st["oracle"] > 1000
