@@ -566,11 +566,17 @@ smlm_status smlm_localize(smlm_ctx* c, const uint16_t* frames, int64_t n, int32_
   for (auto& a : ycls) maxHw = std::max(maxHw, a.ext);
   for (auto& a : xcls) maxWw = std::max(maxWw, a.ext);
   const int mb = auto_micro_batch(c, maxHw, maxWw);   // views per launch
-  const int F = tiled ? 1 : mb;                        // frames per chunk
+  // frames per chunk: whole frames -> one view each; tiles -> as many frames as keep the
+  // largest launch set (all tiles of one window class, times the frames) within mb views
+  int tiles_per_frame = 0;
+  for (auto& a : ycls)
+    for (auto& b : xcls) tiles_per_frame = std::max(tiles_per_frame, a.n * b.n);
+  const int F = (int)std::max<int64_t>(1, std::min<int64_t>(tiled ? mb / std::max(tiles_per_frame, 1) : mb,
+                                                           std::max<int64_t>(n, 1)));
   size_t need = 0;
   for (auto& a : ycls)
     for (auto& b : xcls) {
-      int nv = tiled ? std::min(mb, a.n * b.n) : (int)std::min<int64_t>(mb, std::max<int64_t>(n, 1));
+      int nv = tiled ? std::max(1, std::min(mb, F * a.n * b.n)) : F;
       need = std::max(need, (size_t)nv * a.ext * b.ext * C * elt_size(c));
     }
   if ((r = ensure_act(c, need)) != SMLM_OK) return r;
@@ -654,13 +660,15 @@ smlm_status smlm_localize(smlm_ctx* c, const uint16_t* frames, int64_t n, int32_
     } else {
       for (auto& a : ycls)
         for (auto& b : xcls) {
-          // split the class into sub-blocks of at most mb views
-          int bx = std::min(b.n, mb), by = std::max(1, std::min(a.n, mb / bx));
+          // all tiles of the class for the nf frames of the chunk in one set if that is at
+          // most mb views, else sub-blocks of tiles (times the frames) of at most mb views
+          const int per_frame = std::max(1, mb / nf);
+          int bx = std::min(b.n, per_frame), by = std::max(1, std::min(a.n, per_frame / bx));
           for (int ty = a.t0; ty < a.t0 + a.n; ty += by)
             for (int tx = b.t0; tx < b.t0 + b.n; tx += bx) {
               int ny = std::min(by, a.t0 + a.n - ty), nx = std::min(bx, b.t0 + b.n - tx);
               ViewSet vs{(int)f0, H, W, tile, halo, ty, ny, tx, nx};
-              sets.push_back({vs, ActShape{ny * nx, C, a.ext, b.ext}});
+              sets.push_back({vs, ActShape{nf * ny * nx, C, a.ext, b.ext}});
             }
         }
     }

@@ -43,7 +43,7 @@ namespace {
 
 constexpr int kThreads = 384;  // warps 0 / 2: TMA lane 0 / 1 (2 also owns TMEM alloc), 1 / 3: MMA lane 0 / 1, 4-7 / 8-11: epilogue
 constexpr int kTileM = 128;
-constexpr int kMaxStages = 4;
+constexpr int kMaxStages = 6;
 constexpr int kTmemCols = 512;
 constexpr int kLaneCols = 256;  // TMEM columns reserved per lane (3C <= 192)
 
@@ -461,8 +461,8 @@ __global__ void __launch_bounds__(kThreads, 1)
     LaneRuns runs;
     runs.init(geo, 2 * blockIdx.x + ln, nlanes);
     Run run;
-    uint32_t slot = 2, acc_par = 0, st = 0, full_par = 0;
-    uint32_t prev_st = 0, prev_par = 0;
+    uint32_t slot = 2, acc_par = 0, st = 0;
+    uint32_t prev_st = 0;
     bool prev_valid = false;
     while (runs.next(geo, run)) {
       const int x = run.x0 + px;
@@ -476,6 +476,7 @@ __global__ void __launch_bounds__(kThreads, 1)
         PROF_WAIT(6, mbar_wait(acc_full_bar(ln), acc_par));
         acc_par ^= 1u;
         tc_fence_after();
+        PROF_T(t_tm0);
         uint32_t acc[C];
         if (out_valid) {
 #pragma unroll
@@ -488,9 +489,13 @@ __global__ void __launch_bounds__(kThreads, 1)
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(acc_free_bar(ln));
+        PROF_ADD(9, clock64() - t_tm0);
+        PROF_T(t_post0);
         if (prev_valid) {
           if (store) {
-            mbar_wait(full_bar(ln, prev_st), prev_par);  // complete long ago: makes the TMA writes visible
+            // The stage was filled by the async proxy at least one whole step ago; its full
+            // barrier was observed by this lane's MMA warp, whose tcgen05.commit on acc_full
+            // this thread has in turn observed (causality order), so no second wait on it.
             const uint4* rp = reinterpret_cast<const uint4*>(smem + (stage_addr(ln, prev_st) - sbase) +
                                                              (uint32_t)(d + px) * 16u);
             float lg = HEAD ? bias_s[2 * C] : 0.0f;
@@ -518,14 +523,11 @@ __global__ void __launch_bounds__(kThreads, 1)
           __syncwarp();
           if (lane == 0) mbar_arrive(empty_bar(ln, prev_st));
         }
+        PROF_ADD(10, clock64() - t_post0);
         prev_valid = in_valid;
         if (in_valid) {
           prev_st = st;
-          prev_par = full_par;
-          if (++st == (uint32_t)nstage) {
-            st = 0;
-            full_par ^= 1u;
-          }
+          if (++st == (uint32_t)nstage) st = 0;
         }
         slot = slot == 2 ? 0u : slot + 1u;
       }
