@@ -244,8 +244,19 @@ def main():
         bound = "tensor"
         if cfg.net.precision != "bf16" or args.conv_impl == "direct":
             bound = "alu"
+        # DRAM traffic per launch from the ncu --set full capture of this kernel in this launch
+        # configuration (profiles/kernels_r1_final_full.md: cfg 1, 64 frames per launch,
+        # dram__bytes_read.sum + dram__bytes_write.sum = 435 + 354 MB); null for other shapes.
+        traffic = None
+        alg_bytes_per_launch = 4.0 * C * H * W * (n_frames * args.steps * L / conv_n)
+        if cfg.index in (1, 4) and bound == "tensor" and abs(alg_bytes_per_launch - 805.3e6) < 1e6:
+            traffic = 789.0e6
         roofline = {"bound": bound, "kernel": "conv3x3_dilated (K2)", "achieved": achieved, "peak": peak,
-                    "unit": "TFLOP/s", "frac": achieved / peak, "traffic": None,
+                    "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
+                    "algorithmic_bytes_per_launch": alg_bytes_per_launch,
+                    "hbm_GBs_algorithmic": alg_bytes_per_launch * conv_n / (conv_ms * 1e-3) / 1e9,
+                    "hbm_frac_algorithmic": alg_bytes_per_launch * conv_n / (conv_ms * 1e-3) / 1e9
+                                            / float(peaks["hbm_gbs"]),
                     "peak_source": f"{peak_kind} bf16_tflops_sustained (kernel timed inside a long step)",
                     "frac_of_burst": achieved / float(peaks["bf16_tflops"]),
                     "launches": conv_n, "avg_launch_ms": conv_ms / conv_n,

@@ -15,6 +15,16 @@ namespace {
 constexpr int TX = 128, PX = 4;  // tile = 128 pixels of one row; pixels per thread (x, x+32, x+64, x+96)
 constexpr int NW = 4;            // warps per block, one tile each per round
 
+__device__ __forceinline__ unsigned long long pack2(float lo, float hi) {
+  return ((unsigned long long)__float_as_uint(hi) << 32) | __float_as_uint(lo);
+}
+__device__ __forceinline__ unsigned long long ffma2(unsigned long long a, unsigned long long b,
+                                                    unsigned long long c) {
+  unsigned long long d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+
 // Persistent blocks: tile t = (view, row, 128-px segment); warp w of block j takes tiles
 // (j * NW + w), + gridDim.x * NW, ...  With 5 blocks per SM the tail is one row-tile.
 template <typename T, int C>
@@ -23,11 +33,11 @@ __global__ void __launch_bounds__(32 * NW)
                 NormParams np, const float* __restrict__ w /*[9][C]*/,
                 const float* __restrict__ bias, int relu, T* __restrict__ act) {
   __shared__ float xs[NW][3][TX + 2];
-  __shared__ __align__(16) float ws[9][C];
+  __shared__ __align__(16) float2 ws2[9][C];  // every weight twice: the broadcast operand of fma.rn.f32x2
   __shared__ __align__(16) float bs[C];
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  for (int i = tid; i < 9 * C; i += 32 * NW) ws[i / C][i % C] = w[i];
+  for (int i = tid; i < 9 * C; i += 32 * NW) ws2[i / C][i % C] = make_float2(w[i], w[i]);
   for (int i = tid; i < C; i += 32 * NW) bs[i] = bias[i];
   __syncthreads();
 
@@ -67,42 +77,51 @@ __global__ void __launch_bounds__(32 * NW)
     }
     __syncwarp();
 
-    // Each thread owns PX pixels 32 apart in x: a weight read from shared memory feeds PX
-    // FMAs, and every store of the warp is one dense 512-byte run.
-    float xn[PX][9];
+    // Each thread owns PX = 4 pixels 32 apart in x, held as two pixel pairs: one packed
+    // fma.rn.f32x2 (two independent IEEE fp32 FMAs, same bits as fmaf) updates one channel of
+    // a pair, which halves the FMA instruction count of this issue-bound loop; every store of
+    // the warp is one dense 512-byte run.
+    unsigned long long xp[PX / 2][9];
 #pragma unroll
-    for (int p = 0; p < PX; ++p)
+    for (int pp = 0; pp < PX / 2; ++pp)
 #pragma unroll
       for (int ky = 0; ky < 3; ++ky)
 #pragma unroll
-        for (int kx = 0; kx < 3; ++kx) xn[p][ky * 3 + kx] = xs[warp][ky][lane + 32 * p + kx];
+        for (int kx = 0; kx < 3; ++kx)
+          xp[pp][ky * 3 + kx] = pack2(xs[warp][ky][lane + 64 * pp + kx], xs[warp][ky][lane + 64 * pp + 32 + kx]);
 
 #pragma unroll 1
     for (int k = 0; k < C / 8; ++k) {  // not unrolled: keeps the loop body inside the instruction cache
-      float acc[PX][8];
+      unsigned long long acc[PX / 2][8];
 #pragma unroll
       for (int c = 0; c < 8; ++c) {
         const float bv = bs[k * 8 + c];
 #pragma unroll
-        for (int p = 0; p < PX; ++p) acc[p][c] = bv;
+        for (int pp = 0; pp < PX / 2; ++pp) acc[pp][c] = pack2(bv, bv);
       }
 #pragma unroll
       for (int tp = 0; tp < 9; ++tp)
 #pragma unroll
-        for (int c = 0; c < 8; ++c) {
-          const float wv = ws[tp][k * 8 + c];
+        for (int c = 0; c < 8; c += 2) {
+          const ulonglong2 wv = *reinterpret_cast<const ulonglong2*>(&ws2[tp][k * 8 + c]);
 #pragma unroll
-          for (int p = 0; p < PX; ++p) acc[p][c] = fmaf(xn[p][tp], wv, acc[p][c]);
+          for (int pp = 0; pp < PX / 2; ++pp) {
+            acc[pp][c] = ffma2(xp[pp][tp], wv.x, acc[pp][c]);
+            acc[pp][c + 1] = ffma2(xp[pp][tp], wv.y, acc[pp][c + 1]);
+          }
         }
 #pragma unroll
       for (int p = 0; p < PX; ++p) {
-        const int x = x0 + lane + 32 * p;
+        const int x = x0 + lane + 32 * p;  // pair pp = p / 2 holds pixels 64 pp (low) and 64 pp + 32 (high)
         if (x >= s.W) continue;
-        if (relu) {
+        float v[8];
 #pragma unroll
-          for (int c = 0; c < 8; ++c) acc[p][c] = fmaxf(acc[p][c], 0.0f);
+        for (int c = 0; c < 8; ++c) {
+          const unsigned long long a = acc[p >> 1][c];
+          v[c] = __uint_as_float((p & 1) ? (unsigned)(a >> 32) : (unsigned)a);
+          if (relu) v[c] = fmaxf(v[c], 0.0f);
         }
-        Chunk<T>::store(act, s.chunk_index(b, k, y, x), acc[p]);
+        Chunk<T>::store(act, s.chunk_index(b, k, y, x), v);
       }
     }
   }

@@ -319,3 +319,58 @@ def test_edge_cases_empty_overflow_pageable_threshold():
             P.Localizer(d, np.zeros((d.channels * 10) + d.n_layers * (d.channels ** 2 * 9 + d.channels)
                                     + d.head_channels * (d.channels + 1), np.float32))
         assert ei.value.status == P.ERR_INVALID_ARG
+
+
+# ------------------------------------------------------------------ production K3 (logit map from the last
+# tcgen05 layer's epilogue + post_logits_kernel) against the oracle's rule, exactly
+def _exact_post_check(spec, w, frames, ck, thr, **kw):
+    """The production list must equal the ORACLE's post-processing applied to the GPU's own
+    pre-activation maps (fp32 values are exact in fp64, so every comparison of the rule is
+    decided identically): same (frame, pix) set with no contested-set allowance, decoded
+    values to float rounding.  Pins the fused head (same bits as the debug maps), the 3x3
+    test with its tie rule, ownership in tiled mode and the compaction."""
+    net = O.net_from_spec(spec)
+    cam = O.make_camera(**ck)
+    og = G.gpu_forward_maps(spec, w, frames, ck, conv_impl=P.CONV_TCGEN05)
+    em_o = O.postprocess(net, og.astype(np.float64), cam, thr)
+    em_g = G.gpu_localize(spec, w, frames, ck, thr, conv_impl=P.CONV_TCGEN05, **kw)
+    assert len(em_o) == len(em_g)
+    assert np.array_equal(em_o["frame"], em_g["frame"]) and np.array_equal(em_o["pix"], em_g["pix"])
+    for k, tol in (("x_nm", 2e-3), ("y_nm", 2e-3), ("z_nm", 2e-2), ("p", 1e-6)):      # + fp32 ulp of the value
+        assert np.all(np.abs(em_o[k] - em_g[k]) <= tol + 2.4e-7 * np.abs(em_o[k])), k
+    for k in ("photons", "bg"):
+        assert np.max(np.abs(em_o[k] - em_g[k]) / np.maximum(np.abs(em_o[k]), 1.0), initial=0.0) <= 1e-5, k
+    return len(em_o)
+
+
+def test_production_post_equals_oracle_rule_on_gpu_maps_cfg1_and_cfg2_crop():
+    cfg = get_config(1)
+    fs = make_frames(cfg, 3)
+    n = _exact_post_check(cfg.net, make_weights(cfg, "lc"), fs.frames, G.cam_kwargs(fs), cfg.threshold)
+    assert n > 500
+    cfg = get_config(2)
+    fs = make_frames(cfg, 2, height=150, width=333)            # ragged, 6 heads, C = 64
+    n = _exact_post_check(cfg.net, make_weights(cfg, "lc"), fs.frames, G.cam_kwargs(fs), cfg.threshold)
+    assert n > 100
+    n = _exact_post_check(cfg.net, make_weights(cfg, "lc"), fs.frames, G.cam_kwargs(fs), cfg.threshold,
+                          tile=96, micro_batch=5)
+    assert n > 100
+
+
+def test_production_post_tie_rule_on_quantised_logits():
+    """Logit = bf16(relu(xhat)) of a coarse integer image: thousands of exact ties between
+    neighbours, plateaus, and image-border cases in the tcgen05 production path."""
+    spec = NetSpec(16, (1,), 5, "bf16")
+    C = 16
+    w = np.zeros(spec.n_params(), np.float32)
+    w[0 * 9 + 4] = 1.0                                         # stem channel 0 = centre tap
+    off_head = C * 10 + (C * C * 9 + C)
+    w[off_head + 0] = 1.0                                      # p head reads channel 0
+    w[off_head + 1 * C + 1] = 0.3                              # dx head reads channel 1 (zero): dx = 0
+    rng = np.random.default_rng(5)
+    frames = (100 + 250 * rng.integers(0, 4, size=(3, 70, 150))).astype(np.uint16)   # 4 levels
+    frames[1, 10:30, 20:60] = 1100                                                   # plateau
+    ck = dict(pixel_size_nm=100.0, offset=100.0, gain=1.0)
+    for thr in (0.3, 0.55, 0.0):
+        n = _exact_post_check(spec, w, frames, ck, thr)
+        assert n > 50 or thr == 0.55
