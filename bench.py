@@ -104,9 +104,11 @@ def run_reference(args, cfg):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    fs, _ = workload(cfg, n_frames=8)
+    fs, _ = workload(cfg, n_frames=16)
     w = make_weights(cfg)
-    n_sample = 2 if args.steps * 1 <= 12 else 1
+    # one step = a bounded sample: about 5e11 FLOP of oracle work (a few seconds on 16 cores)
+    H, W = cfg.frames.height, cfg.frames.width
+    n_sample = max(1, min(len(fs.frames), int(5e11 / (cfg.net.flop_per_px() * H * W))))
     for _ in range(args.warmup):
         oracle_sample(cfg, fs, w, 1)
     t_tot, frames = 0.0, 0
@@ -278,7 +280,8 @@ def main():
                                     "share_of_step": k_ms / ms_rf}
     cpu = None
     if not args.no_cpu_baseline:
-        ns = 4 if H * W <= 256 * 256 else 1
+        # bounded sample: about 2e12 FLOP of oracle work (10-15 s on 16 host cores)
+        ns = max(1, min(len(fs.frames), int(2e12 / (cfg.net.flop_per_px() * H * W))))
         fps, eps, cores, dt = oracle_sample(cfg, fs, weights, ns)
         cpu = {"value": fps, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": f"first {ns} frame(s) of {cfg.name}, {dt:.1f} s", "emitters_per_s": eps}
