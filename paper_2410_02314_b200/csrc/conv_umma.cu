@@ -455,15 +455,27 @@ __global__ void __launch_bounds__(kThreads, 1)
     const size_t plane_px = (size_t)geo.H * geo.W;
     const uint32_t plane = (uint32_t)(kTileM + 2 * d) * 16u;
     // The residual operand of an output row is its own centre input row, which the previous
-    // step of this lane loaded into a stage: it is read from shared memory (no second trip
-    // to L2), and that stage is handed back to the producer only afterwards (the empty
-    // barrier counts the MMA commit plus one arrival per epilogue warp).
+    // step of this lane staged in shared memory: it is read from there (no second trip to
+    // L2).  Two policies for handing that stage back to the producer (the empty barrier
+    // counts the MMA commit plus one arrival per epilogue warp):
+    //   kEarly (C = 64, where only 2-3 stages per lane fit): the epilogue of step u - whose
+    //     acc_full says MMA(u) is done with stage(u) - copies the 128 centre pixels into
+    //     registers for step u+1 and releases the stage at once; holding it until step u+1
+    //     would cost one stage of prefetch depth (measured: 0.8 -> 1.2 PFLOP/s at C = 64).
+    //     The copy is a generic-proxy read that the TMA refill (async proxy) must not
+    //     overtake: fence.proxy.async before the arrive.  Without it the arrive is issued
+    //     behind loads still in flight and the refill raced with them (measured).
+    //   otherwise (6 stages): step u+1 reads the residual straight from stage(u) and releases
+    //     it after use; no extra registers, no fence (3 % faster at C = 48).
+    constexpr bool kEarly = C >= 64;
     LaneRuns runs;
     runs.init(geo, 2 * blockIdx.x + ln, nlanes);
     Run run;
-    uint32_t slot = 2, acc_par = 0, st = 0;
-    uint32_t prev_st = 0;
+    uint32_t slot = 2, acc_par = 0, st = 0, prev_st = 0;
     bool prev_valid = false;
+    uint4 res[C / 8];
+#pragma unroll
+    for (int k = 0; k < C / 8; ++k) res[k] = make_uint4(0u, 0u, 0u, 0u);
     while (runs.next(geo, run)) {
       const int x = run.x0 + px;
       int row = run.r + (run.i0 - 1) * d;  // input row of the step; the output row is row - d
@@ -491,44 +503,53 @@ __global__ void __launch_bounds__(kThreads, 1)
         if (lane == 0) mbar_arrive(acc_free_bar(ln));
         PROF_ADD(9, clock64() - t_tm0);
         PROF_T(t_post0);
-        if (prev_valid) {
-          if (store) {
-            // The stage was filled by the async proxy at least one whole step ago; its full
-            // barrier was observed by this lane's MMA warp, whose tcgen05.commit on acc_full
-            // this thread has in turn observed (causality order), so no second wait on it.
-            const uint4* rp = reinterpret_cast<const uint4*>(smem + (stage_addr(ln, prev_st) - sbase) +
-                                                             (uint32_t)(d + px) * 16u);
-            float lg = HEAD ? bias_s[2 * C] : 0.0f;
+        // (the stage was filled by the async proxy; its full barrier was observed by this
+        // lane's MMA warp, whose tcgen05.commit on acc_full this thread has observed in turn)
+        const uint4* rprev = reinterpret_cast<const uint4*>(smem + (stage_addr(ln, prev_st) - sbase) +
+                                                            (uint32_t)(d + px) * 16u);
+        if (store) {
+          float lg = HEAD ? bias_s[2 * C] : 0.0f;
 #pragma unroll
-            for (int k = 0; k < C / 8; ++k) {
-              const uint4 res = rp[(size_t)k * (plane / 16u)];
-              const uint32_t rw[4] = {res.x, res.y, res.z, res.w};
-              uint32_t ow[4];
+          for (int k = 0; k < C / 8; ++k) {
+            const uint4 rk = kEarly ? res[k] : rprev[(size_t)k * (plane / 16u)];
+            const uint32_t rw[4] = {rk.x, rk.y, rk.z, rk.w};
+            uint32_t ow[4];
 #pragma unroll
-              for (int i = 0; i < 4; ++i) {
-                float r0 = __uint_as_float(rw[i] << 16), r1 = __uint_as_float(rw[i] & 0xffff0000u);
-                float v0 = r0 + fmaxf(__uint_as_float(acc[k * 8 + 2 * i]), 0.0f);
-                float v1 = r1 + fmaxf(__uint_as_float(acc[k * 8 + 2 * i + 1]), 0.0f);
-                __nv_bfloat162 h = __floats2bfloat162_rn(v0, v1);
-                ow[i] = *reinterpret_cast<uint32_t*>(&h);
-                if (HEAD) {
-                  lg = fmaf(__uint_as_float(ow[i] << 16), bias_s[C + k * 8 + 2 * i], lg);
-                  lg = fmaf(__uint_as_float(ow[i] & 0xffff0000u), bias_s[C + k * 8 + 2 * i + 1], lg);
-                }
+            for (int i = 0; i < 4; ++i) {
+              float r0 = __uint_as_float(rw[i] << 16), r1 = __uint_as_float(rw[i] & 0xffff0000u);
+              float v0 = r0 + fmaxf(__uint_as_float(acc[k * 8 + 2 * i]), 0.0f);
+              float v1 = r1 + fmaxf(__uint_as_float(acc[k * 8 + 2 * i + 1]), 0.0f);
+              __nv_bfloat162 h = __floats2bfloat162_rn(v0, v1);
+              ow[i] = *reinterpret_cast<uint32_t*>(&h);
+              if (HEAD) {
+                lg = fmaf(__uint_as_float(ow[i] << 16), bias_s[C + k * 8 + 2 * i], lg);
+                lg = fmaf(__uint_as_float(ow[i] & 0xffff0000u), bias_s[C + k * 8 + 2 * i + 1], lg);
               }
-              orow[(size_t)k * plane_px] = make_uint4(ow[0], ow[1], ow[2], ow[3]);
             }
-            if (HEAD) logit[((size_t)run.b * geo.H + (row - d)) * geo.W + x] = lg;
+            orow[(size_t)k * plane_px] = make_uint4(ow[0], ow[1], ow[2], ow[3]);
           }
-          __syncwarp();
-          if (lane == 0) mbar_arrive(empty_bar(ln, prev_st));
+          if (HEAD) logit[((size_t)run.b * geo.H + (row - d)) * geo.W + x] = lg;
         }
-        PROF_ADD(10, clock64() - t_post0);
+        if (kEarly) {
+          if (in_valid) {
+            const uint4* rp = reinterpret_cast<const uint4*>(smem + (stage_addr(ln, st) - sbase) +
+                                                             (uint32_t)(d + px) * 16u);
+#pragma unroll
+            for (int k = 0; k < C / 8; ++k) res[k] = rp[(size_t)k * (plane / 16u)];
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty_bar(ln, st));
+          }
+        } else if (prev_valid) {
+          __syncwarp();  // the residual was consumed above (real data dependence), so the
+          if (lane == 0) mbar_arrive(empty_bar(ln, prev_st));  // loads are done before this arrive
+        }
         prev_valid = in_valid;
         if (in_valid) {
           prev_st = st;
           if (++st == (uint32_t)nstage) st = 0;
         }
+        PROF_ADD(10, clock64() - t_post0);
         slot = slot == 2 ? 0u : slot + 1u;
       }
     }
@@ -645,7 +666,7 @@ cudaError_t launch_conv_umma(UmmaPlan* p, int src, int dil, const void* wpack, c
   // stages: as many as fit next to the resident weights (<= kMaxStages)
   int nstage = kMaxStages;
   SmemLayout L = smem_layout(s.C, dil, nstage);
-  // (>= 2: a stage is released only by the epilogue of the following step)
+  // (>= 2 for any overlap of load and MMA)
   while (nstage > 2 && L.total + 1024 > 227u * 1024u) L = smem_layout(s.C, dil, --nstage);
   if (L.total + 1024 > 227u * 1024u) {
     snprintf(err, errlen, "shared memory budget exceeded");
