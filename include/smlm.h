@@ -85,7 +85,8 @@ typedef struct {
   int32_t micro_batch;   /* frames (or tiles) per kernel launch; 0 = auto */
   int32_t conv_impl;     /* SMLM_CONV_* */
   int32_t writeback_frames; /* flush the compacted emitter list to a HOST out_emitters once
-                               per this many frames (0 = once at the end of the call) */
+                               per this many frames, overlapped with compute (0 = library
+                               default, 256; the last flush is at the end of the call) */
 } smlm_net_desc;
 
 /* Camera model.  Scalars are used where a map pointer is NULL.  Maps are [H][W] float32,

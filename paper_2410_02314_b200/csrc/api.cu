@@ -617,7 +617,8 @@ smlm_status smlm_localize(smlm_ctx* c, const uint16_t* frames, int64_t n, int32_
     CK(c, cudaStreamWaitEvent(c->copy_stream, c->ev_start, 0));
   }
   const bool host_out = (ok == PTR_HOST_PINNED && capacity > 0);
-  const int wbf = c->d.writeback_frames;
+  // 0 = library default: flush every 256 frames, so that only the last batch's D2H is exposed
+  const int wbf = c->d.writeback_frames > 0 ? c->d.writeback_frames : 256;
   bool wb_pending = false;
   auto flush = [&]() -> smlm_status {
     // records below the snapshot are complete: every K3 that wrote them precedes it on `st`
