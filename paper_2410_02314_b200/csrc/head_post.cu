@@ -154,7 +154,7 @@ __global__ void __launch_bounds__(NT)
 // one contiguous range of the list with a single global atomicAdd (same-address atomics
 // from every warp serialise in L2), and each survivor evaluates the other heads from the
 // activations and writes its record.
-constexpr int LW = 64, LH = 8;  // NT = 256 threads, two pixels each
+constexpr int LW = 64, LH = 16;  // NT = 256 threads, four pixels each
 constexpr int LCAND = (LW / 2) * (LH / 2);  // no two detections are 8-adjacent
 
 template <typename T, int C>
@@ -183,6 +183,9 @@ __global__ void __launch_bounds__(NT, 4)
     pv[r] = (i < PATCH && y >= 0 && y < s.H && x >= 0 && x < s.W) ? __ldg(lmap + (size_t)y * s.W + x)
                                                                 : -CUDART_INF_F;
   }
+  // head weights for the survivors: fetched now, in the shadow of the patch round trip
+  for (int i = tid; i < hp.n_h * C; i += NT) wh[i] = __ldg(w_head + i);
+  if (tid < hp.n_h) bh[tid] = __ldg(b_head + tid);
   if (tid == 0) ncand = 0;
 #pragma unroll
   for (int r = 0; r < (PATCH + NT - 1) / NT; ++r) {
@@ -218,8 +221,6 @@ __global__ void __launch_bounds__(NT, 4)
   if (n == 0) return;
   // the block's survivors take one contiguous range of the list: one global atomic per block
   if (tid == 0) base = atomicAdd(counter, (unsigned long long)n);
-  for (int i = tid; i < hp.n_h * C; i += NT) wh[i] = w_head[i];
-  if (tid < hp.n_h) bh[tid] = b_head[tid];
   __syncthreads();
   if (tid >= n) return;
   const unsigned long long slot = base + tid;
