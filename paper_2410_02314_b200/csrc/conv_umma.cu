@@ -3,32 +3,35 @@
 // bf16 activations and weights, fp32 accumulation in TMEM, one RNE rounding of the stored
 // result (BASELINE.json north_star (b)).
 //
-// Dataflow ("row-chain walk"):  an implicit GEMM with M = 128 consecutive pixels of
-// one image row, K = C input channels per tap, and - instead of N = C - N = 3C: the three
-// vertical taps of one horizontal tap share their A operand.  Input row q of the chain
-// r, r+d, r+2d, ... contributes
+// Dataflow ("row-chain walk"):  an implicit GEMM with M = 128
+// consecutive pixels of one image row, K = C input channels per tap, and - instead of
+// N = C - N = 3C: the three vertical taps of one horizontal tap share their A operand.
+// Input row q of the chain r, r+d, r+2d, ... contributes
 //     W[ky=0] to output row q+1,  W[ky=1] to output row q,  W[ky=2] to output row q-1
 // (chain indices), so ONE tcgen05.mma  D[128 x 3C] += A[128 x 16] * B[16 x 3C]  feeds three
-// output rows that live in three TMEM slots of C columns each.  Every input row is read from
-// L2 once (one TMA box of (128+2d) pixels x C channels) and is used by 3 x C/16 MMAs of
-// N = 3C, which keeps the tensor pipe - not the shared-memory operand fetch - the limiter
-// (N = C would re-read the 4 KB A tile for every 1.5 KB of B).
+// output rows that live in three TMEM slots of C columns each.  Every input row is fetched
+// once (C/8 bulk copies of (128+2d) pixels x 16 B) and is used by 3 x C/16 MMAs of N = 3C,
+// which keeps the tensor pipe - not the shared-memory operand fetch - the limiter (N = C
+// would re-read the 4 KB A tile for every 1.5 KB of B).
 //   * slot of output o = (step id of its centre input) % 3; the B operand is the window
 //     [m] of the weight rows stored as (ky = 1, 0, 2, 1, 0) so that the rotation is just a
 //     different start address;
 //   * after the MMAs of step u the output whose centre was step u-1 is complete: the
 //     epilogue warps tcgen05.ld its slot, re-initialise the slot with the bias
 //     (tcgen05.st - the next output accumulates on top, so the bias add is free), release
-//     it, then apply ReLU + residual, round to bf16 and store;
-//   * two independent "lanes" per CTA (own TMEM slots, own smem stages, own epilogue
-//     warps) alternate on the single MMA-issuing thread, so one lane's epilogue overlaps
-//     the other lane's MMAs;
+//     it, then apply ReLU + residual (read from the shared-memory stage, not from L2),
+//     round to bf16 and store; the last layer also evaluates the detection head (HEAD);
+//   * two independent "lanes" per CTA, each with its own producer warp, MMA-issuing warp,
+//     four epilogue warps, TMEM slots and shared-memory stages: one lane's epilogue
+//     overlaps the other lane's MMAs, and two issuing warps keep the tensor queue fed;
 //   * work = the sequence of all (view, 128-px segment, residue, chain row) row-tiles, cut
 //     into 2 x gridDim equal contiguous ranges: balanced for any shape, at the cost of two
-//     halo steps per range/chain boundary.
-// The activation layout act[b][C/8][y][x][8] makes a TMA box land in shared memory as the
-// UMMA "K-major, no swizzle" operand: core matrix = 8 pixels x 16 B, contiguous, so a
-// horizontal tap is a 16-byte-granular shift of the descriptor start address.
+//     halo steps per range/chain boundary;
+//   * consecutive layers are chained by programmatic dependent launch: the prologue and the
+//     weight load of layer l+1 overlap the tail of layer l.
+// The activation layout act[b][C/8][y][x][8] makes a row segment of one chunk plane land in
+// shared memory as the UMMA "K-major, no swizzle" operand: core matrix = 8 pixels x 16 B,
+// contiguous, so a horizontal tap is a 16-byte-granular shift of the descriptor start address.
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 
