@@ -217,7 +217,8 @@ def test_cfg4_dense_bf16(impl):
 
 # ------------------------------------------------------------------ bf16: tensor-core kernel vs CUDA-core kernel
 @pytest.mark.parametrize("C,H,W,dil", [(48, 70, 300, (1, 2, 4, 8)), (64, 40, 129, (8, 1)),
-                                       (16, 64, 64, (1, 2, 4, 8)), (32, 19, 517, (4, 2))])
+                                       (16, 64, 64, (1, 2, 4, 8)), (32, 19, 517, (4, 2)),
+                                       (16, 9, 9, (8, 4, 1)), (32, 3, 140, (2, 8)), (48, 1, 1, (1, 8))])
 def test_tcgen05_matches_direct_bf16(C, H, W, dil):
     """Same rounding points (bf16 inputs and weights, fp32 accumulate, one RNE store), only the
     summation order differs: the stored bf16 maps may differ by an ulp here and there."""
