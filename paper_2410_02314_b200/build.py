@@ -10,6 +10,7 @@ import os
 import shutil
 import subprocess
 import sys
+import tempfile
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
@@ -42,8 +43,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not _stale():
         return LIB
     nvcc = _nvcc()
-    objdir = os.path.join(HERE, "build")
-    os.makedirs(objdir, exist_ok=True)
+    # objects go to a private directory: several ranks may find the library stale at once
+    os.makedirs(os.path.join(HERE, "build"), exist_ok=True)
+    objdir = tempfile.mkdtemp(prefix=f"obj{os.getpid()}_", dir=os.path.join(HERE, "build"))
     common = [nvcc, "-O3", "-std=c++17", "-lineinfo", *ARCH, "-Xcompiler", "-fPIC,-Wall",
               "-I", INCLUDE, "-I", CSRC]
     if verbose:
@@ -63,14 +65,17 @@ def build(force: bool = False, verbose: bool = False) -> str:
         if p.returncode != 0 or verbose:
             sys.stderr.write(f"--- {src}\n{out}\n")
         failed |= p.returncode != 0
-    if failed:
-        raise RuntimeError("nvcc failed")
-    tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [nvcc, "-shared", *ARCH, "-o", tmp, *objs]
-    if verbose:
-        print(" ".join(cmd), flush=True)
-    subprocess.run(cmd, check=True)
-    os.replace(tmp, LIB)
+    try:
+        if failed:
+            raise RuntimeError("nvcc failed")
+        tmp = LIB + f".tmp{os.getpid()}"
+        cmd = [nvcc, "-shared", *ARCH, "-o", tmp, *objs]
+        if verbose:
+            print(" ".join(cmd), flush=True)
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, LIB)
+    finally:
+        shutil.rmtree(objdir, ignore_errors=True)
     return LIB
 
 

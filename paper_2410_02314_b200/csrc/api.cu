@@ -19,6 +19,12 @@ using namespace smlm;
 namespace {
 
 constexpr int kSlots = 3;  // staging slots of the preload ring (copy k+1, k+2 while k computes)
+// Write-back (step W): flush k copies the records [snap[(k-1) % R], snap[k % R]) to the host
+// list on the write-back stream.  The snapshots are written on the compute stream, so each
+// flush owns one word of a ring; a word is rewritten only after the two flushes that read it
+// (k - R as its upper end, k - R + 1 as its lower end) have finished (event wait below).
+constexpr int kSnapRing = 4;
+constexpr int kCounterWords = 2 + kSnapRing;
 
 thread_local std::string g_create_error;
 
@@ -73,12 +79,13 @@ struct smlm_ctx {
   size_t slot_elems = 0;
   bool slot_used[kSlots] = {false, false, false};
   cudaEvent_t ev_copied[kSlots]{}, ev_consumed[kSlots]{};
-  cudaEvent_t ev_start = nullptr, ev_batch = nullptr, ev_wb = nullptr;
+  cudaEvent_t ev_start = nullptr, ev_batch = nullptr;
+  cudaEvent_t ev_wb[kSnapRing]{};  // flush k records ev_wb[k % kSnapRing] on the write-back stream
   cudaStream_t copy_stream = nullptr, wb_stream = nullptr;
 
   smlm_emitter* em_dev = nullptr;
   size_t em_cap = 0;
-  unsigned long long* counters = nullptr;  // [0] count, [1] snapshot, [2] flushed
+  unsigned long long* counters = nullptr;  // [0] count, [1] zero (lower end of flush 0), [2 ..) snapshot ring
   unsigned long long* h_count = nullptr;   // pinned, for smlm_check
   unsigned long long last_capacity = 0;
 
@@ -438,9 +445,10 @@ smlm_status smlm_create(const smlm_net_desc* desc, const void* weights, smlm_ctx
     }
     CK(nullptr, cudaEventCreateWithFlags(&c->ev_start, cudaEventDisableTiming));
     CK(nullptr, cudaEventCreateWithFlags(&c->ev_batch, cudaEventDisableTiming));
-    CK(nullptr, cudaEventCreateWithFlags(&c->ev_wb, cudaEventDisableTiming));
-    CK(nullptr, cudaMalloc(&c->counters, 4 * sizeof(unsigned long long)));
-    CK(nullptr, cudaMemset(c->counters, 0, 4 * sizeof(unsigned long long)));
+    for (int i = 0; i < kSnapRing; ++i)
+      CK(nullptr, cudaEventCreateWithFlags(&c->ev_wb[i], cudaEventDisableTiming));
+    CK(nullptr, cudaMalloc(&c->counters, kCounterWords * sizeof(unsigned long long)));
+    CK(nullptr, cudaMemset(c->counters, 0, kCounterWords * sizeof(unsigned long long)));
     CK(nullptr, cudaMallocHost(&c->h_count, sizeof(unsigned long long)));
     *c->h_count = 0;
     return SMLM_OK;
@@ -469,7 +477,8 @@ void smlm_destroy(smlm_ctx* c) {
   }
   if (c->ev_start) cudaEventDestroy(c->ev_start);
   if (c->ev_batch) cudaEventDestroy(c->ev_batch);
-  if (c->ev_wb) cudaEventDestroy(c->ev_wb);
+  for (int i = 0; i < kSnapRing; ++i)
+    if (c->ev_wb[i]) cudaEventDestroy(c->ev_wb[i]);
   for (auto e : c->tev) cudaEventDestroy(e);
   if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
   if (c->wb_stream) cudaStreamDestroy(c->wb_stream);
@@ -607,9 +616,8 @@ smlm_status smlm_localize(smlm_ctx* c, const uint16_t* frames, int64_t n, int32_
     list = c->em_dev;
   }
   unsigned long long* counter = c->counters;
-  unsigned long long* snap = c->counters + 1;
-  unsigned long long* flushed = c->counters + 2;
-  CK(c, cudaMemsetAsync(c->counters, 0, 4 * sizeof(unsigned long long), st));
+  unsigned long long* snap_ring = c->counters + 2;
+  CK(c, cudaMemsetAsync(c->counters, 0, kCounterWords * sizeof(unsigned long long), st));
   c->last_capacity = capacity;
 
   if (fk == PTR_HOST_PINNED) {
@@ -619,16 +627,20 @@ smlm_status smlm_localize(smlm_ctx* c, const uint16_t* frames, int64_t n, int32_
   const bool host_out = (ok == PTR_HOST_PINNED && capacity > 0);
   // 0 = library default: flush every 256 frames, so that only the last batch's D2H is exposed
   const int wbf = c->d.writeback_frames > 0 ? c->d.writeback_frames : 256;
-  bool wb_pending = false;
+  int64_t n_flush = 0;
   auto flush = [&]() -> smlm_status {
+    const int64_t k = n_flush;
+    // the word snap[k % R] was read by flushes k - R (upper end) and k - R + 1 (lower end)
+    if (k >= kSnapRing) CK(c, cudaStreamWaitEvent(st, c->ev_wb[(k + 1) % kSnapRing], 0));
     // records below the snapshot are complete: every K3 that wrote them precedes it on `st`
-    CK(c, launch_snapshot(counter, capacity, snap, st));
+    CK(c, launch_snapshot(counter, capacity, snap_ring + k % kSnapRing, st));
     CK(c, cudaEventRecord(c->ev_batch, st));
     CK(c, cudaStreamWaitEvent(c->wb_stream, c->ev_batch, 0));
-    CK(c, launch_flush_emitters(list, out, snap, flushed, c->wb_stream));
-    CK(c, cudaEventRecord(c->ev_wb, c->wb_stream));
-    c->launches += 3;
-    wb_pending = true;
+    const unsigned long long* lo = k == 0 ? c->counters + 1 : snap_ring + (k - 1) % kSnapRing;
+    CK(c, launch_flush_emitters(list, out, lo, snap_ring + k % kSnapRing, c->wb_stream));
+    CK(c, cudaEventRecord(c->ev_wb[k % kSnapRing], c->wb_stream));
+    c->launches += 2;
+    ++n_flush;
     return SMLM_OK;
   };
 
@@ -701,7 +713,7 @@ smlm_status smlm_localize(smlm_ctx* c, const uint16_t* frames, int64_t n, int32_
   if (host_out) {
     if ((r = flush()) != SMLM_OK) return r;
   }
-  if (wb_pending) CK(c, cudaStreamWaitEvent(st, c->ev_wb, 0));
+  if (n_flush > 0) CK(c, cudaStreamWaitEvent(st, c->ev_wb[(n_flush - 1) % kSnapRing], 0));
   return store_count(c, counter, out_count, st);
 }
 
@@ -766,7 +778,7 @@ smlm_status smlm_debug_postprocess(smlm_ctx* c, const float* maps, int64_t n, in
   if (n > 0 && classify(maps) != PTR_DEVICE) return fail(c, SMLM_ERR_INVALID_ARG, "maps must be device memory");
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   const HeadParams hp = head_params(c, cam, threshold);
-  CK(c, cudaMemsetAsync(c->counters, 0, 4 * sizeof(unsigned long long), st));
+  CK(c, cudaMemsetAsync(c->counters, 0, kCounterWords * sizeof(unsigned long long), st));
   c->last_capacity = capacity;
   CK(c, launch_post_from_maps(maps, (int)n, H, W, hp, out, c->counters, capacity, st));
   c->launches++;

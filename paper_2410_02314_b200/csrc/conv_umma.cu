@@ -49,6 +49,7 @@ constexpr int kTileM = 128;
 constexpr int kMaxStages = 6;
 constexpr int kTmemCols = 512;
 constexpr int kLaneCols = 256;  // TMEM columns reserved per lane (3C <= 192)
+constexpr int kMaxDevices = 64;
 
 // zero source for the padded parts of a row segment: at most (127 + 8) pixels x 16 B
 __device__ __align__(16) uint4 g_zeros[160];
@@ -582,12 +583,15 @@ template <int C, bool HEAD>
 cudaError_t launch_ch(const void* in, void* out, Geo geo, const void* wpack, const float* bias, int nstage,
                       int grid, size_t smem, const float* head_w, const float* head_b, float* logit,
                       cudaStream_t st) {
-  static bool attr_done = false;
-  if (!attr_done) {
+  static bool attr_done[kMaxDevices] = {};  // the attribute is per device
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+  if (!attr_done[dev]) {
     cudaError_t e = cudaFuncSetAttribute(conv_umma_kernel<C, HEAD>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          227 * 1024);
     if (e != cudaSuccess) return e;
-    attr_done = true;
+    attr_done[dev] = true;
   }
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = dim3((unsigned)grid);

@@ -301,18 +301,16 @@ __global__ void snapshot_kernel(const unsigned long long* counter, unsigned long
 
 __global__ void __launch_bounds__(NT)
     flush_kernel(const smlm_emitter* __restrict__ dev, smlm_emitter* __restrict__ host,
-                 const unsigned long long* __restrict__ snap, unsigned long long* flushed) {
-  // 16-byte units; grid-stride.  *flushed is advanced by a second, single-thread launch
-  // (flush_commit_kernel) so that every block of this one reads the same start.
-  const unsigned long long lo = *flushed * 2, hi = *snap * 2;
+                 const unsigned long long* __restrict__ lo_word,
+                 const unsigned long long* __restrict__ hi_word) {
+  // 16-byte units; grid-stride.  Both ends are snapshot words that nothing rewrites while
+  // this launch runs (api.cu: ring of snapshots), so every block sees the same range.
+  const unsigned long long lo = *lo_word * 2, hi = *hi_word * 2;
   const uint4* s = reinterpret_cast<const uint4*>(dev);
   uint4* d = reinterpret_cast<uint4*>(host);
   for (unsigned long long i = lo + (unsigned long long)blockIdx.x * NT + threadIdx.x; i < hi;
        i += (unsigned long long)gridDim.x * NT)
     d[i] = s[i];
-}
-__global__ void flush_commit_kernel(const unsigned long long* snap, unsigned long long* flushed) {
-  *flushed = *snap;
 }
 
 template <typename T, int C>
@@ -407,12 +405,9 @@ cudaError_t launch_snapshot(const unsigned long long* counter, unsigned long lon
 }
 
 cudaError_t launch_flush_emitters(const smlm_emitter* dev, smlm_emitter* host_mapped,
-                                  const unsigned long long* snap, unsigned long long* flushed,
+                                  const unsigned long long* lo, const unsigned long long* hi,
                                   cudaStream_t st) {
-  flush_kernel<<<64, NT, 0, st>>>(dev, host_mapped, snap, flushed);
-  cudaError_t e = cudaGetLastError();
-  if (e != cudaSuccess) return e;
-  flush_commit_kernel<<<1, 1, 0, st>>>(snap, flushed);
+  flush_kernel<<<64, NT, 0, st>>>(dev, host_mapped, lo, hi);
   return cudaGetLastError();
 }
 

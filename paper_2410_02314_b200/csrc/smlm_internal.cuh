@@ -139,10 +139,9 @@ cudaError_t launch_post_from_maps(const float* maps, int n, int H, int W, HeadPa
 // snap[0] = min(*counter, capacity)
 cudaError_t launch_snapshot(const unsigned long long* counter, unsigned long long capacity,
                             unsigned long long* snap, cudaStream_t st);
-// copy records [*flushed, *snap) from the device list to a device-visible host list, then
-// *flushed = *snap
+// copy records [*lo, *hi) from the device list to a device-visible host list
 cudaError_t launch_flush_emitters(const smlm_emitter* dev, smlm_emitter* host_mapped,
-                                  const unsigned long long* snap, unsigned long long* flushed,
+                                  const unsigned long long* lo, const unsigned long long* hi,
                                   cudaStream_t st);
 
 }  // namespace smlm

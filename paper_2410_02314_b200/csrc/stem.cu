@@ -43,7 +43,6 @@ __global__ void __launch_bounds__(32 * NW)
 
   const int nseg = (s.W + TX - 1) / TX;
   const long long ntiles = (long long)s.B * s.H * nseg;
-  const float inv_scalar = 1.0f / (np.gain * np.norm_scale);
   constexpr int PATCH = 3 * (TX + 2), NLD = (PATCH + 31) / 32;
   for (long long t = (long long)blockIdx.x * NW + warp; t < ntiles; t += (long long)gridDim.x * NW) {
     const int seg = (int)(t % nseg);
@@ -64,7 +63,7 @@ __global__ void __launch_bounds__(32 * NW)
       const size_t q = ok[r] ? (size_t)fy * vs.Wf + fx : 0;
       adu[r] = ok[r] ? (float)__ldg(frame + q) : 0.0f;
       om[r] = (ok[r] && np.offset_map) ? __ldg(np.offset_map + q) : np.offset;
-      gm[r] = (ok[r] && np.offset_map) ? __ldg(np.gain_map + q) : 1.0f;
+      gm[r] = (ok[r] && np.offset_map) ? __ldg(np.gain_map + q) : np.gain;
     }
     __syncwarp();  // the previous tile's reads of xs[warp] are done
 #pragma unroll
@@ -72,7 +71,7 @@ __global__ void __launch_bounds__(32 * NW)
       const int i = lane + r * 32;
       if (i >= PATCH) continue;
       float xn = 0.0f;
-      if (ok[r]) xn = np.offset_map ? ((adu[r] - om[r]) / gm[r]) / np.norm_scale : (adu[r] - om[r]) * inv_scalar;
+      if (ok[r]) xn = ((adu[r] - om[r]) / gm[r]) / np.norm_scale;  // the oracle's operation order (G5)
       xs[warp][i / (TX + 2)][i % (TX + 2)] = xn;
     }
     __syncwarp();
@@ -130,14 +129,17 @@ __global__ void __launch_bounds__(32 * NW)
 template <typename T, int C>
 cudaError_t launch_tc(const uint16_t* frames, int frame_base, ViewSet vs, ActShape s, NormParams np,
                       const float* w, const float* b, int relu, void* act, cudaStream_t st) {
-  static int blocks_per_wave = 0;
-  if (!blocks_per_wave) {
-    int dev = 0, n_sm = 0, per_sm = 0;
-    cudaGetDevice(&dev);
+  static int waves[64] = {};  // resident blocks per device (occupancy is a per-device fact)
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+  if (!waves[dev]) {
+    int n_sm = 0, per_sm = 0;
     cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, stem_kernel<T, C>, 32 * NW, 0);
-    blocks_per_wave = n_sm * (per_sm > 0 ? per_sm : 1);
+    waves[dev] = n_sm * (per_sm > 0 ? per_sm : 1);
   }
+  const int blocks_per_wave = waves[dev];
   const long long ntiles = (long long)s.B * s.H * ((s.W + TX - 1) / TX);
   const long long want = (ntiles + NW - 1) / NW;
   const int grid = (int)(want < blocks_per_wave ? want : blocks_per_wave);

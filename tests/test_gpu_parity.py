@@ -42,7 +42,7 @@ def test_cfg0_fp32_trunk_maps_and_emitters():
     em_o = O.postprocess(net, o, cam, cfg.threshold)
     em_g = G.gpu_localize(cfg.net, w, fs.frames, ck, cfg.threshold)
     st = G.parity_gate(cfg.net, o, em_o, em_g, cfg.threshold, 1e-4, fs.pixel_size_nm, 64, 64)
-    print("cfg0 gate", st)
+    G.record("cfg0_fp32", gate=st)
     assert st["oracle"] > 50 and st["contested_frac"] < 0.5      # the gate is not vacuous
     assert st["rel_N"] < 1e-3 and st["rel_bg"] < 1e-3
 
@@ -162,57 +162,101 @@ def test_cfg1_hc_weights_fp32_mode_index_gate():
     em_o = O.postprocess(net, o, cam, cfg.threshold)
     em_g = G.gpu_localize(spec32, w, fs.frames, ck, cfg.threshold)
     st = G.parity_gate(cfg.net, o, em_o, em_g, cfg.threshold, 1e-4, fs.pixel_size_nm, 256, 256)
-    print("cfg1 hc fp32 gate", st)
+    G.record("cfg1_hc_fp32_mode", gate=st)
     assert st["oracle"] > 800 and st["contested_frac"] < 0.25 and st["flipped"] <= 4
+
+
+def _bf16_maps_and_gate(name, cfg, fs, w, impl, H, W, max_contested, check_tol=True):
+    """bf16 production precision: (1) every activated head map within 2e-2 of the oracle;
+    (2) the index gate with the contested set built from 2 x the MEASURED p-map error of this
+    run (gpu_util.parity_gate), its size bounded and recorded - the gate must not be vacuous."""
+    ck = G.cam_kwargs(fs)
+    net, cam, o, _ = G.oracle_run(name, cfg.net, w, fs.frames, ck)
+    og = G.gpu_forward_maps(cfg.net, w, fs.frames, ck, conv_impl=impl)
+    err = G.head_errors(cfg.net, o, og)
+    if check_tol:
+        assert err.max() < 2e-2, err
+    dp = G.p_error(o, og)
+    em_o = O.postprocess(net, o, cam, cfg.threshold)
+    em_g = G.gpu_localize(cfg.net, w, fs.frames, ck, cfg.threshold, conv_impl=impl)
+    st = G.parity_gate(cfg.net, o, em_o, em_g, cfg.threshold, 2e-2, fs.pixel_size_nm, H, W,
+                       dp_measured=dp, check_tol=check_tol, o_gpu=og)
+    impl_name = {P.CONV_DIRECT: "direct", P.CONV_TCGEN05: "tcgen05"}[impl]
+    G.record(f"{name}_bf16_{impl_name}", gate=st, head_max_err=err, frames=len(fs.frames), H=H, W=W)
+    assert st["contested_frac_local"] <= max_contested, st
+    assert st["uncontested_local"] >= 100, st
+    return st
 
 
 @pytest.mark.parametrize("impl", BF16_IMPLS)
 def test_cfg1_lc_weights_bf16_maps_and_gate(impl):
     cfg = get_config(1)
-    fs = make_frames(cfg, 2)
-    w = make_weights(cfg, "lc")
-    ck = G.cam_kwargs(fs)
-    net, cam, o, _ = G.oracle_run("cfg1lc", cfg.net, w, fs.frames, ck)
-    og = G.gpu_forward_maps(cfg.net, w, fs.frames, ck, conv_impl=impl)
-    err = np.abs(G.activated(cfg.net, og) - G.activated(cfg.net, o)).reshape(2, 5, -1).max(axis=(0, 2))
-    print("cfg1 lc bf16 map errors per head", err)
-    assert err.max() < 2e-2
-    em_o = O.postprocess(net, o, cam, cfg.threshold)
-    em_g = G.gpu_localize(cfg.net, w, fs.frames, ck, cfg.threshold, conv_impl=impl)
-    st = G.parity_gate(cfg.net, o, em_o, em_g, cfg.threshold, 2e-2, fs.pixel_size_nm, 256, 256)
-    print("cfg1 lc bf16 gate", st)
+    _bf16_maps_and_gate("cfg1lc", cfg, make_frames(cfg, 2), make_weights(cfg, "lc"), impl, 256, 256, 0.6)
+
+
+@pytest.mark.parametrize("impl", BF16_IMPLS)
+def test_cfg1_hc_weights_bf16_index_gate(impl):
+    """The high-contrast p-head (logit std 3, the survey's strong index test) through the bf16
+    kernels.  Its p-map error may exceed 2e-2 by construction (the logit error scales with the
+    contrast), so the map tolerance is not asserted here; the index gate is, with
+    the contested set from the measured error: no decision may differ outside it."""
+    cfg = get_config(1)
+    st = _bf16_maps_and_gate("cfg1hc", cfg, make_frames(cfg, 2), make_weights(cfg, "hc"), impl, 256, 256,
+                             0.6, check_tol=False)
+    assert st["oracle"] > 800
 
 
 @pytest.mark.parametrize("impl", BF16_IMPLS)
 def test_cfg2_crop_bf16_six_heads(impl):
     cfg = get_config(2)
-    fs = make_frames(cfg, 2, height=136, width=200)
-    w = make_weights(cfg, "lc")
-    ck = G.cam_kwargs(fs)
-    net, cam, o, _ = G.oracle_run("cfg2crop", cfg.net, w, fs.frames, ck)
-    og = G.gpu_forward_maps(cfg.net, w, fs.frames, ck, conv_impl=impl)
-    err = np.abs(G.activated(cfg.net, og) - G.activated(cfg.net, o)).reshape(2, 6, -1).max(axis=(0, 2))
-    print("cfg2 crop bf16 map errors per head", err)
-    assert err.max() < 2e-2
-    em_o = O.postprocess(net, o, cam, cfg.threshold)
-    em_g = G.gpu_localize(cfg.net, w, fs.frames, ck, cfg.threshold, conv_impl=impl)
-    st = G.parity_gate(cfg.net, o, em_o, em_g, cfg.threshold, 2e-2, fs.pixel_size_nm, 136, 200)
-    print("cfg2 crop gate", st)
+    _bf16_maps_and_gate("cfg2crop", cfg, make_frames(cfg, 2, height=136, width=200), make_weights(cfg, "lc"),
+                        impl, 136, 200, 0.6)
 
 
 @pytest.mark.parametrize("impl", BF16_IMPLS)
 def test_cfg4_dense_bf16(impl):
     cfg = get_config(4)
-    fs = make_frames(cfg, 1)
-    w = make_weights(cfg, "lc")
+    _bf16_maps_and_gate("cfg4", cfg, make_frames(cfg, 1), make_weights(cfg, "lc"), impl, 256, 256, 0.6)
+
+
+# ------------------------------------------------------------------ maps in the launch shape bench.py times
+def _launch_shape_maps(name, cfg, fs, w, n, sample, tol=2e-2):
+    """n frames cycling the distinct frames of fs through smlm_debug_forward_maps with the
+    default micro-batch (cfg 1: 64 + 64 + tail views per launch): K2's work split - lane
+    ranges of ~110 rows that start and end mid-chain - is the one of the timed run.  Sampled
+    frames are compared element by element with the oracle, and every frame with the first
+    occurrence of the same distinct frame bit by bit (position in the launch must not matter)."""
+    k = len(fs.frames)
     ck = G.cam_kwargs(fs)
-    net, cam, o, _ = G.oracle_run("cfg4", cfg.net, w, fs.frames, ck)
-    og = G.gpu_forward_maps(cfg.net, w, fs.frames, ck, conv_impl=impl)
-    assert np.max(np.abs(G.activated(cfg.net, og) - G.activated(cfg.net, o))) < 2e-2
-    em_o = O.postprocess(net, o, cam, cfg.threshold)
-    em_g = G.gpu_localize(cfg.net, w, fs.frames, ck, cfg.threshold, conv_impl=impl)
-    st = G.parity_gate(cfg.net, o, em_o, em_g, cfg.threshold, 2e-2, fs.pixel_size_nm, 256, 256)
-    print("cfg4 gate", st)
+    frames = np.ascontiguousarray(np.concatenate([fs.frames] * ((n + k - 1) // k))[:n])
+    net, cam, o, _ = G.oracle_run(name, cfg.net, w, fs.frames, ck)
+    og = G.gpu_forward_maps(cfg.net, w, frames, ck, conv_impl=P.CONV_TCGEN05)
+    for f in range(k, n):
+        assert np.array_equal(og[f], og[f % k]), f"frame {f} differs from frame {f % k}"
+    errs = {}
+    for f in sample:
+        e = G.head_errors(cfg.net, o[f % k:f % k + 1], og[f:f + 1])
+        assert e.max() < tol, (f, e)
+        errs[str(f)] = e
+    G.record(f"{name}_launch_shape_maps", frames=n, distinct=k, head_max_err=errs)
+
+
+def test_cfg1_maps_in_timed_launch_shape_130_frames():
+    cfg = get_config(1)
+    _launch_shape_maps("cfg1lc", cfg, make_frames(cfg, 2), make_weights(cfg, "lc"), 130, (0, 63, 64, 129))
+
+
+def test_cfg2_maps_full_frame_in_multi_view_launch():
+    cfg = get_config(2)
+    _launch_shape_maps("cfg2full", cfg, make_frames(cfg, 1), make_weights(cfg, "lc"), 12, (0, 11))
+
+
+def test_cfg3_tile_window_maps_in_multi_view_launch():
+    """cfg 3 launches sets of 606 x 606 windows (512 + 2 x 47); the same window shape through
+    the map export, 16 views per call, against the oracle on the same window."""
+    cfg = get_config(3)
+    fs = make_frames(cfg, 1, height=606, width=606)
+    _launch_shape_maps("cfg3win", cfg, fs, make_weights(cfg, "lc"), 16, (0, 15))
 
 
 # ------------------------------------------------------------------ bf16: tensor-core kernel vs CUDA-core kernel
@@ -282,6 +326,23 @@ def test_pinned_ring_and_writeback_batches_equal_device_path():
     a = ref[ref["frame"] < 8]
     b = ref[(ref["frame"] >= 8) & (ref["frame"] < 16)]
     assert np.array_equal(a["pix"], b["pix"]) and np.array_equal(a["frame"] + 8, b["frame"])
+
+
+def test_writeback_every_frame_stress_equals_device_path():
+    """A flush after every frame (writeback_frames = 1, micro_batch = 1): 600 flushes per call
+    whose snapshots are written on the compute stream while earlier flushes may still run on
+    the write-back stream.  The host list must equal the device-path list bit by bit."""
+    cfg = get_config(0)
+    fs = make_frames(cfg, 8)
+    frames = np.ascontiguousarray(np.concatenate([fs.frames] * 75)[:600])
+    w = make_weights(cfg)
+    ck = G.cam_kwargs(fs)
+    ref = G.gpu_localize(cfg.net, w, frames, ck, cfg.threshold, micro_batch=8)
+    assert len(ref) > 10000
+    for rep in range(20):
+        em = G.gpu_localize(cfg.net, w, frames, ck, cfg.threshold, host_frames=True, host_out=True,
+                            writeback_frames=1, micro_batch=1)
+        assert np.array_equal(em, ref), rep
 
 
 def test_edge_cases_empty_overflow_pageable_threshold():
