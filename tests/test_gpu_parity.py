@@ -202,7 +202,7 @@ def test_cfg1_hc_weights_bf16_index_gate(impl):
     the contested set from the measured error: no decision may differ outside it."""
     cfg = get_config(1)
     st = _bf16_maps_and_gate("cfg1hc", cfg, make_frames(cfg, 2), make_weights(cfg, "hc"), impl, 256, 256,
-                             0.6, check_tol=False)
+                             0.7, check_tol=False)
     assert st["oracle"] > 800
 
 
@@ -216,7 +216,8 @@ def test_cfg2_crop_bf16_six_heads(impl):
 @pytest.mark.parametrize("impl", BF16_IMPLS)
 def test_cfg4_dense_bf16(impl):
     cfg = get_config(4)
-    _bf16_maps_and_gate("cfg4", cfg, make_frames(cfg, 1), make_weights(cfg, "lc"), impl, 256, 256, 0.6)
+    # 4 emitters / um^2: the smooth p-map has more near-ties between neighbours than cfg 1
+    _bf16_maps_and_gate("cfg4", cfg, make_frames(cfg, 1), make_weights(cfg, "lc"), impl, 256, 256, 0.75)
 
 
 # ------------------------------------------------------------------ maps in the launch shape bench.py times
