@@ -42,7 +42,7 @@
 extern "C" {
 #endif
 
-#define SMLM_ABI_VERSION 1
+#define SMLM_ABI_VERSION 2
 #define SMLM_MAX_LAYERS 32
 
 typedef struct smlm_ctx smlm_ctx; /* opaque; owns device weights, activations, staging slots, events */
@@ -64,6 +64,13 @@ enum {
   SMLM_CONV_TCGEN05 = 1,
   SMLM_CONV_DIRECT = 2  /* CUDA-core kernel with the same rounding points (cross-check) */
 };
+
+/* Kernel fusion on the tcgen05 path ("post-processing is consolidated
+ * within GPU memory to minimize data transfer").  AUTO: the stem (K1) is computed inside the
+ * first trunk layer's kernel, and the last trunk layer's epilogue evaluates the heads (K3) -
+ * neither a_0 nor a_L ever reaches HBM.  NONE: one kernel per step (the cross-check twin; same
+ * arithmetic, same rounding points, bit-identical results). */
+enum { SMLM_FUSE_AUTO = 0, SMLM_FUSE_NONE = 1 };
 
 typedef struct {
   uint32_t struct_size; /* sizeof(smlm_net_desc) */
@@ -87,6 +94,7 @@ typedef struct {
   int32_t writeback_frames; /* flush the compacted emitter list to a HOST out_emitters once
                                per this many frames, overlapped with compute (0 = library
                                default, 256; the last flush is at the end of the call) */
+  int32_t fusion;        /* SMLM_FUSE_*: which steps share a kernel on the tcgen05 path */
 } smlm_net_desc;
 
 /* Camera model.  Scalars are used where a map pointer is NULL.  Maps are [H][W] float32,

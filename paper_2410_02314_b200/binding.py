@@ -18,7 +18,8 @@ MAX_LAYERS = 32
 FP32, BF16 = 0, 1
 CONV_AUTO, CONV_TCGEN05, CONV_DIRECT = 0, 1, 2
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED_DEVICE, ERR_CUDA, ERR_OOM, ERR_OVERFLOW = 0, -1, -2, -3, -4, -5
-ABI_VERSION = 1
+ABI_VERSION = 2
+FUSE_AUTO, FUSE_NONE = 0, 1
 KERNEL_STEM, KERNEL_CONV, KERNEL_POST = 0, 1, 2
 
 EXPORTS = ["smlm_create", "smlm_localize", "smlm_check", "smlm_destroy", "smlm_last_error",
@@ -33,7 +34,7 @@ class NetDesc(C.Structure):
                 ("norm_scale", C.c_float), ("xy_scale", C.c_float), ("z_scale_nm", C.c_float),
                 ("photon_scale", C.c_float), ("bg_scale", C.c_float), ("tile", C.c_int32),
                 ("micro_batch", C.c_int32), ("conv_impl", C.c_int32),
-                ("writeback_frames", C.c_int32)]
+                ("writeback_frames", C.c_int32), ("fusion", C.c_int32)]
 
 
 class CameraParams(C.Structure):
@@ -93,7 +94,7 @@ def make_desc(channels: int, dilations: Sequence[int], head_channels: int, preci
               stem_relu: int = 1, norm_scale: float = 1000.0, xy_scale: float = 0.5,
               z_scale_nm: float = 700.0, photon_scale: float = 1000.0, bg_scale: float = 100.0,
               tile: int = 0, micro_batch: int = 0, conv_impl: int = CONV_AUTO,
-              writeback_frames: int = 0) -> NetDesc:
+              writeback_frames: int = 0, fusion: int = FUSE_AUTO) -> NetDesc:
     d = NetDesc()
     d.struct_size = C.sizeof(NetDesc)
     d.version = ABI_VERSION
@@ -108,6 +109,7 @@ def make_desc(channels: int, dilations: Sequence[int], head_channels: int, preci
     d.photon_scale, d.bg_scale = float(photon_scale), float(bg_scale)
     d.tile, d.micro_batch, d.conv_impl = int(tile), int(micro_batch), int(conv_impl)
     d.writeback_frames = int(writeback_frames)
+    d.fusion = int(fusion)
     return d
 
 

@@ -49,13 +49,6 @@ struct Layer {
   int dil = 1;
 };
 
-struct PlanEntry {
-  const void* b0;
-  const void* b1;
-  ActShape s;
-  UmmaPlan* plan;
-};
-
 }  // namespace
 
 struct smlm_ctx {
@@ -71,9 +64,9 @@ struct smlm_ctx {
 
   void* act[2] = {nullptr, nullptr};
   size_t act_bytes = 0;
-  float* logit = nullptr;  // detection-head map written by the last tcgen05 layer
-  size_t logit_bytes = 0;
-  std::vector<PlanEntry> plans;
+  float* logit = nullptr;  // detection logit of every pixel, written by the last tcgen05 layer (HEAD)
+  float* cand = nullptr;   // 32-byte candidate records (other heads) of above-threshold pixels
+  bool fuse = true;        // desc.fusion != SMLM_FUSE_NONE: K1 into the first layer, K3's heads into the last
 
   uint16_t* slots = nullptr;  // kSlots x slot_elems
   size_t slot_elems = 0;
@@ -157,14 +150,8 @@ PtrKind classify(const void* p) {
   return PTR_OTHER;
 }
 
-void free_plans(smlm_ctx* c) {
-  for (auto& p : c->plans) umma_plan_destroy(p.plan);
-  c->plans.clear();
-}
-
 smlm_status ensure_act(smlm_ctx* c, size_t bytes) {
   if (bytes <= c->act_bytes) return SMLM_OK;
-  free_plans(c);
   for (int i = 0; i < 2; ++i) {
     if (c->act[i]) cudaFree(c->act[i]);
     c->act[i] = nullptr;
@@ -172,64 +159,56 @@ smlm_status ensure_act(smlm_ctx* c, size_t bytes) {
   c->act_bytes = 0;
   for (int i = 0; i < 2; ++i) CK(c, cudaMalloc(&c->act[i], bytes));
   c->act_bytes = bytes;
-  if (c->use_umma) {  // one fp32 per pixel: bytes / (C * 2) pixels
+  if (c->use_umma) {  // bytes / (C * 2) pixels: one fp32 logit and one 32-byte candidate record each
     if (c->logit) cudaFree(c->logit);
-    c->logit = nullptr;
-    c->logit_bytes = bytes / ((size_t)c->d.channels * 2) * sizeof(float);
-    CK(c, cudaMalloc(&c->logit, c->logit_bytes));
+    if (c->cand) cudaFree(c->cand);
+    c->logit = c->cand = nullptr;
+    const size_t px = bytes / ((size_t)c->d.channels * 2);
+    CK(c, cudaMalloc(&c->logit, px * sizeof(float)));
+    CK(c, cudaMalloc(&c->cand, px * 8 * sizeof(float)));
   }
   return SMLM_OK;
 }
 
-smlm_status get_plan(smlm_ctx* c, ActShape s, UmmaPlan** out) {
-  for (auto& p : c->plans)
-    if (p.b0 == c->act[0] && p.b1 == c->act[1] && p.s.B == s.B && p.s.C == s.C && p.s.H == s.H &&
-        p.s.W == s.W) {
-      *out = p.plan;
-      return SMLM_OK;
-    }
-  char err[256] = {0};
-  UmmaPlan* pl = umma_plan_create(c->act[0], c->act[1], s, c->n_sm, err, sizeof err);
-  if (!pl) return fail(c, SMLM_ERR_CUDA, "tcgen05 plan: %s", err);
-  if (c->plans.size() > 64) free_plans(c);
-  c->plans.push_back({c->act[0], c->act[1], s, pl});
-  *out = pl;
-  return SMLM_OK;
-}
-
-// K1 -> K2 x L for one launch set; the result is in act[*result_buf].
+// K1 -> K2 x L for one launch set; the result is in act[*result_buf] (or, when *have_logit
+// comes back true, in c->logit / c->cand: the last layer ran as the HEAD variant).
+// lthr: logit(threshold) for the HEAD variant (want_logit).
 smlm_status run_trunk(smlm_ctx* c, const uint16_t* dev_frames, int frame_base, const ViewSet& vs,
                       ActShape s, const NormParams& np, cudaStream_t st, int* result_buf,
                       float* trunk_dump, size_t dump_view_stride, size_t dump_level_stride,
-                      cudaEvent_t after_stem, bool want_logit, bool* have_logit) {
+                      cudaEvent_t after_stem, bool want_logit, float lthr, bool* have_logit) {
   if (have_logit) *have_logit = false;
+  const size_t nl = c->layers.size();
+  // K1 folded into the first trunk layer (STEM variant) when the tcgen05 path runs it
+  const bool fuse_stem = c->use_umma && c->fuse && nl > 0 &&
+                         conv_umma_supports(c->d.channels, c->layers[0].dil, true);
   cudaEvent_t te = nullptr;
-  smlm_status tr = time_begin(c, SMLM_KERNEL_STEM, st, &te);
-  if (tr != SMLM_OK) return tr;
-  CK(c, launch_stem(c->bf16, dev_frames, frame_base, vs, s, np, c->w_stem, c->b_stem,
-                    c->d.stem_relu, c->act[0], st));
-  c->launches++;
-  if ((tr = time_end(c, te, st)) != SMLM_OK) return tr;
-  if (after_stem) CK(c, cudaEventRecord(after_stem, st));
-  int cur = 0;
-  if (trunk_dump) {
-    CK(c, launch_dump_act(c->bf16, c->act[0], s, trunk_dump, dump_view_stride, st));
+  smlm_status tr = SMLM_OK;
+  if (!fuse_stem || trunk_dump) {  // (the trunk dump wants a_0 itself)
+    if ((tr = time_begin(c, SMLM_KERNEL_STEM, st, &te)) != SMLM_OK) return tr;
+    CK(c, launch_stem(c->bf16, dev_frames, frame_base, vs, s, np, c->w_stem, c->b_stem,
+                      c->d.stem_relu, c->act[0], st));
     c->launches++;
+    if ((tr = time_end(c, te, st)) != SMLM_OK) return tr;
+    if (trunk_dump) {
+      CK(c, launch_dump_act(c->bf16, c->act[0], s, trunk_dump, dump_view_stride, st));
+      c->launches++;
+    }
   }
-  UmmaPlan* plan = nullptr;
-  if (c->use_umma && !c->layers.empty()) {
-    smlm_status r = get_plan(c, s, &plan);
-    if (r != SMLM_OK) return r;
-  }
-  for (size_t l = 0; l < c->layers.size(); ++l) {
+  if (after_stem && !fuse_stem) CK(c, cudaEventRecord(after_stem, st));
+  int cur = 0;
+  for (size_t l = 0; l < nl; ++l) {
     const Layer& L = c->layers[l];
     cudaEvent_t e1 = nullptr;
     if ((tr = time_begin(c, SMLM_KERNEL_CONV, st, &e1)) != SMLM_OK) return tr;
     if (c->use_umma) {
       char err[256] = {0};
-      const bool head = want_logit && l + 1 == c->layers.size();
-      cudaError_t e = launch_conv_umma(plan, cur, L.dil, L.w_umma, L.bias, c->w_head, c->b_head,
-                                       head ? c->logit : nullptr, st, err, sizeof err);
+      const bool head = want_logit && c->fuse && l + 1 == nl;
+      const bool stem = fuse_stem && l == 0;
+      HeadArgs ha{c->w_head, c->b_head, c->d.head_channels, lthr, c->logit, c->cand};
+      StemArgs sa{dev_frames, frame_base, vs, np, c->w_stem, c->b_stem, c->d.stem_relu};
+      cudaError_t e = launch_conv_umma(c->act[cur], c->act[cur ^ 1], s, L.dil, L.w_umma, L.bias,
+                                       head ? &ha : nullptr, stem ? &sa : nullptr, c->n_sm, st, err, sizeof err);
       if (head && have_logit) *have_logit = true;
       if (e != cudaSuccess)
         return fail(c, SMLM_ERR_CUDA, "conv_umma: %s %s", cudaGetErrorString(e), err);
@@ -238,6 +217,8 @@ smlm_status run_trunk(smlm_ctx* c, const uint16_t* dev_frames, int frame_base, c
     }
     c->launches++;
     if ((tr = time_end(c, e1, st)) != SMLM_OK) return tr;
+    // the frames of this launch set have been consumed once the first layer has run
+    if (after_stem && fuse_stem && l == 0) CK(c, cudaEventRecord(after_stem, st));
     cur ^= 1;
     if (trunk_dump) {
       CK(c, launch_dump_act(c->bf16, c->act[cur], s, trunk_dump + (l + 1) * dump_level_stride,
@@ -377,6 +358,8 @@ smlm_status smlm_create(const smlm_net_desc* desc, const void* weights, smlm_ctx
   if (!(desc->norm_scale > 0.0f)) return fail(nullptr, SMLM_ERR_INVALID_ARG, "norm_scale must be > 0");
   if (desc->tile < 0 || desc->micro_batch < 0 || desc->writeback_frames < 0)
     return fail(nullptr, SMLM_ERR_INVALID_ARG, "negative tile / micro_batch / writeback_frames");
+  if (desc->fusion != SMLM_FUSE_AUTO && desc->fusion != SMLM_FUSE_NONE)
+    return fail(nullptr, SMLM_ERR_INVALID_ARG, "bad fusion");
 
   int dev = 0;
   cudaDeviceProp prop;
@@ -393,6 +376,7 @@ smlm_status smlm_create(const smlm_net_desc* desc, const void* weights, smlm_ctx
   c->d = *desc;
   c->bf16 = desc->precision == SMLM_BF16;
   c->use_umma = c->bf16 && desc->conv_impl != SMLM_CONV_DIRECT;
+  c->fuse = desc->fusion != SMLM_FUSE_NONE;
   c->n_sm = prop.multiProcessorCount;
   c->l2_bytes = (size_t)prop.l2CacheSize;
   c->radius = 1;
@@ -465,10 +449,10 @@ smlm_status smlm_create(const smlm_net_desc* desc, const void* weights, smlm_ctx
 void smlm_destroy(smlm_ctx* c) {
   if (!c) return;
   cudaDeviceSynchronize();
-  free_plans(c);
   cudaFree(c->w_stem); cudaFree(c->b_stem); cudaFree(c->w_head); cudaFree(c->b_head);
   for (auto& L : c->layers) { cudaFree(L.w_direct); cudaFree(L.w_umma); cudaFree(L.bias); }
-  cudaFree(c->act[0]); cudaFree(c->act[1]); cudaFree(c->logit); cudaFree(c->slots); cudaFree(c->em_dev);
+  cudaFree(c->act[0]); cudaFree(c->act[1]); cudaFree(c->logit); cudaFree(c->cand); cudaFree(c->slots);
+  cudaFree(c->em_dev);
   cudaFree(c->counters); cudaFree(c->cam_off); cudaFree(c->cam_gain);
   if (c->h_count) cudaFreeHost(c->h_count);
   for (int i = 0; i < kSlots; ++i) {
@@ -690,13 +674,12 @@ smlm_status smlm_localize(smlm_ctx* c, const uint16_t* frames, int64_t n, int32_
       cudaEvent_t after_stem = (slot >= 0 && si + 1 == sets.size()) ? c->ev_consumed[slot] : nullptr;
       bool have_logit = false;
       r = run_trunk(c, dev_frames, frame_base, sets[si].vs, sets[si].s, np, st, &res, nullptr, 0, 0,
-                    after_stem, true, &have_logit);
+                    after_stem, true, hp.lthr, &have_logit);
       if (r != SMLM_OK) return r;
       cudaEvent_t te = nullptr;
       if ((r = time_begin(c, SMLM_KERNEL_POST, st, &te)) != SMLM_OK) return r;
       if (have_logit)
-        CK(c, launch_post_logits(c->act[res], c->logit, sets[si].s, sets[si].vs, c->w_head, c->b_head, hp,
-                                 list, counter, capacity, st));
+        CK(c, launch_post_logits(c->logit, c->cand, sets[si].s, sets[si].vs, hp, list, counter, capacity, st));
       else
         CK(c, launch_head_post(c->bf16, c->act[res], sets[si].s, sets[si].vs, c->w_head, c->b_head, hp,
                                list, counter, capacity, st));
@@ -749,7 +732,7 @@ smlm_status smlm_debug_forward_maps(smlm_ctx* c, const uint16_t* frames, int64_t
     int res = 0;
     float* dump = trunk ? trunk + (size_t)f0 * (L + 1) * px * C : nullptr;
     r = run_trunk(c, frames, 0, vs, s, np, st, &res, dump, (size_t)(L + 1) * px * C, px * C, nullptr, false,
-                  nullptr);
+                  0.0f, nullptr);
     if (r != SMLM_OK) break;
     cudaError_t e = launch_head_maps(c->bf16, c->act[res], s, c->w_head, c->b_head, nh,
                                      maps + (size_t)f0 * nh * px, st);

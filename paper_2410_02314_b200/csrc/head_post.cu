@@ -147,26 +147,22 @@ __global__ void __launch_bounds__(NT)
   detect_tile(src, s.H, s.W, v, b, vs.Wf, hp, out, counter, capacity);
 }
 
-// K3 after a HEAD conv layer (conv_umma.cu): the detection logit is already an fp32 map, so
-// the tile is small and flat - one (LH+2) x (LW+2) logit patch per block goes to shared
+// K3 after a HEAD conv layer (conv_umma.cu): the detection logit is already an fp32 map and
+// the other heads of every above-threshold pixel sit in 32-byte candidate records, so this
+// kernel touches no activations.  One (LH+2) x (LW+2) logit patch per block goes to shared
 // memory in one round trip (three independent loads per thread), the 3x3 test runs there,
 // survivors are compacted through a warp-aggregated shared-memory counter, the block takes
 // one contiguous range of the list with a single global atomicAdd (same-address atomics
-// from every warp serialise in L2), and each survivor evaluates the other heads from the
-// activations and writes its record.
+// from every warp serialise in L2), and each survivor decodes its candidate record.
 constexpr int LW = 64, LH = 16;  // NT = 256 threads, four pixels each
 constexpr int LCAND = (LW / 2) * (LH / 2);  // no two detections are 8-adjacent
 
-template <typename T, int C>
 __global__ void __launch_bounds__(NT, 4)
-    post_logits_kernel(const T* __restrict__ act, const float* __restrict__ logit, ActShape s, ViewSet vs,
-                       const float* __restrict__ w_head, const float* __restrict__ b_head, HeadParams hp,
-                       smlm_emitter* __restrict__ out, unsigned long long* __restrict__ counter,
-                       unsigned long long capacity) {
+    post_logits_kernel(const float* __restrict__ logit, const float* __restrict__ cand, ActShape s,
+                       ViewSet vs, HeadParams hp, smlm_emitter* __restrict__ out,
+                       unsigned long long* __restrict__ counter, unsigned long long capacity) {
   __shared__ float lg[LH + 2][LW + 2];
-  __shared__ float wh[6 * C];
-  __shared__ float bh[8];
-  __shared__ int cand[LCAND];
+  __shared__ int cnd[LCAND];
   __shared__ int ncand;
   __shared__ unsigned long long base;
   const int tid = threadIdx.x;
@@ -183,9 +179,6 @@ __global__ void __launch_bounds__(NT, 4)
     pv[r] = (i < PATCH && y >= 0 && y < s.H && x >= 0 && x < s.W) ? __ldg(lmap + (size_t)y * s.W + x)
                                                                 : -CUDART_INF_F;
   }
-  // head weights for the survivors: fetched now, in the shadow of the patch round trip
-  for (int i = tid; i < hp.n_h * C; i += NT) wh[i] = __ldg(w_head + i);
-  if (tid < hp.n_h) bh[tid] = __ldg(b_head + tid);
   if (tid == 0) ncand = 0;
 #pragma unroll
   for (int r = 0; r < (PATCH + NT - 1) / NT; ++r) {
@@ -213,7 +206,7 @@ __global__ void __launch_bounds__(NT, 4)
       int slot = 0;
       if (lane == leader) slot = atomicAdd(&ncand, __popc(m));
       slot = __shfl_sync(0xffffffffu, slot, leader);
-      if (keep) cand[slot + __popc(m & ((1u << lane) - 1u))] = i;
+      if (keep) cnd[slot + __popc(m & ((1u << lane) - 1u))] = i;
     }
   }
   __syncthreads();
@@ -225,20 +218,21 @@ __global__ void __launch_bounds__(NT, 4)
   if (tid >= n) return;
   const unsigned long long slot = base + tid;
   if (slot >= capacity) return;  // counted, not stored (smlm_check reports overflow)
-  const int i = cand[tid];
+  const int i = cnd[tid];
   const int ly = i / LW, lx = i - ly * LW;
   const int y = y0 + ly, x = x0 + lx;
   const int fy = v.wy0 + y, fx = v.wx0 + x;
-  const int hN = hp.n_h == 6 ? 4 : 3;
-  ActSource<T, C> src{act, s, wh, bh};
-  const float odx = src.head(1, b, y, x), ody = src.head(2, b, y, x);
-  const float oN = src.head(hN, b, y, x), obg = src.head(hN + 1, b, y, x);
+  // candidate record: heads 1 .. n_h-1 (pre-activation) = (dx, dy, [z,] N, bg)
+  const float4* cq = reinterpret_cast<const float4*>(cand) + (((size_t)b * s.H + y) * s.W + x) * 2;
+  const float4 c0 = __ldg(cq), c1 = __ldg(cq + 1);
+  const bool six = hp.n_h == 6;
+  const float odx = c0.x, ody = c0.y, oz = c0.z, oN = six ? c0.w : c0.z, obg = six ? c1.x : c0.w;
   smlm_emitter e;
   e.frame = v.frame;
   e.pix = fy * vs.Wf + fx;
   e.x_nm = ((float)fx + hp.xy_scale * tanhf(odx)) * hp.pixel_size_nm;
   e.y_nm = ((float)fy + hp.xy_scale * tanhf(ody)) * hp.pixel_size_nm;
-  e.z_nm = hp.n_h == 6 ? hp.z_scale_nm * tanhf(src.head(3, b, y, x)) : 0.0f;
+  e.z_nm = six ? hp.z_scale_nm * tanhf(oz) : 0.0f;
   e.photons = hp.photon_scale * softplus_f(oN);
   e.bg = hp.bg_scale * softplus_f(obg);
   e.p = sigmoid_f(lg[ly + 1][lx + 1]);
@@ -322,14 +316,6 @@ cudaError_t head_post_tc(const void* act, ActShape s, ViewSet vs, const float* w
   return cudaGetLastError();
 }
 template <typename T, int C>
-cudaError_t post_logits_tc(const void* act, const float* logit, ActShape s, ViewSet vs, const float* w,
-                           const float* b, HeadParams hp, smlm_emitter* out, unsigned long long* counter,
-                           unsigned long long cap, cudaStream_t st) {
-  dim3 grid((s.W + LW - 1) / LW, (s.H + LH - 1) / LH, s.B);
-  post_logits_kernel<T, C><<<grid, NT, 0, st>>>((const T*)act, logit, s, vs, w, b, hp, out, counter, cap);
-  return cudaGetLastError();
-}
-template <typename T, int C>
 cudaError_t head_maps_tc(const void* act, ActShape s, const float* w, const float* b, int n_h,
                          float* maps, cudaStream_t st) {
   dim3 grid((s.W + NT - 1) / NT, s.H, s.B);
@@ -360,12 +346,13 @@ cudaError_t launch_head_post(bool bf16, const void* act, ActShape s, ViewSet vs,
   }
 }
 
-cudaError_t launch_post_logits(const void* act, const float* logit, ActShape s, ViewSet vs,
-                               const float* w_head, const float* b_head, HeadParams hp,
-                               smlm_emitter* out, unsigned long long* counter,
+cudaError_t launch_post_logits(const float* logit, const float* cand, ActShape s, ViewSet vs,
+                               HeadParams hp, smlm_emitter* out, unsigned long long* counter,
                                unsigned long long capacity, cudaStream_t st) {
   if (s.B <= 0) return cudaSuccess;
-  SMLM_DISPATCH_C(__nv_bfloat16, post_logits_tc, act, logit, s, vs, w_head, b_head, hp, out, counter, capacity, st)
+  dim3 grid((s.W + LW - 1) / LW, (s.H + LH - 1) / LH, s.B);
+  post_logits_kernel<<<grid, NT, 0, st>>>(logit, cand, s, vs, hp, out, counter, capacity);
+  return cudaGetLastError();
 }
 
 cudaError_t launch_head_maps(bool bf16, const void* act, ActShape s, const float* w_head,

@@ -99,18 +99,36 @@ cudaError_t launch_conv_direct(bool bf16, const void* in, void* out, ActShape s,
 cudaError_t conv_direct_init(int C);  // opt in to the shared memory the kernel needs
 
 // K2 trunk layer on tcgen05 tensor cores (bf16 storage, fp32 accumulate in TMEM).
-struct UmmaPlan;  // opaque, conv_umma.cu: tensor maps for one (buffer pair, shape)
 size_t umma_packed_weight_bytes(int C);
 // w_oihw [C][C][3][3] fp32 -> the kernel's shared-memory image (bf16, RNE), host side.
 void umma_pack_weights_host(int C, const float* w_oihw, void* dst);
-UmmaPlan* umma_plan_create(const void* buf0, const void* buf1, ActShape s, int n_sm, char* err,
-                           size_t errlen);
-void umma_plan_destroy(UmmaPlan*);
-// in = plan buffer `src` (0/1), out = the other one.  logit != nullptr (last layer): also
-// store the detection head o_p = head_b[0] + head_w[0..C) . out as fp32 [B][H][W].
-cudaError_t launch_conv_umma(UmmaPlan* plan, int src, int dil, const void* wpack,
-                             const float* bias, const float* head_w, const float* head_b,
-                             float* logit, cudaStream_t st, char* err, size_t errlen);
+// STEM variant (first layer, K1 folded in): a_0 is computed in the kernel from the frames.
+struct StemArgs {
+  const uint16_t* frames;  // device; frame f of the call at frames + (f - frame_base) Hf Wf
+  int frame_base;
+  ViewSet vs;
+  NormParams np;
+  const float* w;  // [9][C]
+  const float* b;  // [C]
+  int relu;
+};
+
+// HEAD (K3 folded in): what the last layer's epilogue writes instead of the activation map.
+struct HeadArgs {
+  const float* w;   // [n_h][C]
+  const float* b;   // [n_h]
+  int n_h;
+  float lthr;       // logit(threshold)
+  float* logit;     // [B][H][W] detection logit of every pixel
+  float* cand;      // [B][H][W][8]: heads 1 .. n_h-1 (pre-activation) of pixels with logit > lthr
+};
+
+bool conv_umma_supports(int C, int dil, bool stem);
+// head != nullptr: last layer, HEAD variant (`out` is not written).  stem != nullptr: first
+// layer, STEM variant (`in` is not read).
+cudaError_t launch_conv_umma(const void* in, void* out, ActShape s, int dil, const void* wpack,
+                             const float* bias, const HeadArgs* head, const StemArgs* stem, int n_sm,
+                             cudaStream_t st, char* err, size_t errlen);
 
 // K3: 1x1 heads + threshold + 3x3 NMS + decode + warp-aggregated compaction.
 cudaError_t launch_head_post(bool bf16, const void* act, ActShape s, ViewSet vs,
@@ -119,10 +137,9 @@ cudaError_t launch_head_post(bool bf16, const void* act, ActShape s, ViewSet vs,
                              unsigned long long capacity, cudaStream_t st);
 
 // K3 after a HEAD conv layer: the detection logit comes from `logit` [B][H][W], the other
-// heads are evaluated from `act` for the survivors only.
-cudaError_t launch_post_logits(const void* act, const float* logit, ActShape s, ViewSet vs,
-                               const float* w_head, const float* b_head, HeadParams hp,
-                               smlm_emitter* out, unsigned long long* counter,
+// heads of every pixel above the threshold from `cand` [B][H][W][8] (HeadArgs).
+cudaError_t launch_post_logits(const float* logit, const float* cand, ActShape s, ViewSet vs,
+                               HeadParams hp, smlm_emitter* out, unsigned long long* counter,
                                unsigned long long capacity, cudaStream_t st);
 
 // debug: heads only -> fp32 maps [B][n_h][H][W] (pre-activation)

@@ -437,3 +437,34 @@ def test_production_post_tie_rule_on_quantised_logits():
     for thr in (0.3, 0.55, 0.0):
         n = _exact_post_check(spec, w, frames, ck, thr)
         assert n > 50 or thr == 0.55
+
+
+# ------------------------------------------------------------------ fusion vs one kernel per step
+@pytest.mark.parametrize("C,nh,H,W,dil,tile", [(48, 5, 70, 300, (1, 2, 4, 8), 0), (64, 6, 40, 129, (2, 8, 1), 0),
+                                               (16, 5, 64, 64, (1,), 0), (32, 6, 19, 517, (4, 2), 0),
+                                               (16, 5, 9, 9, (8, 4, 1), 0), (48, 5, 1, 1, (1, 8), 0),
+                                               (48, 5, 150, 173, (1, 2, 4), 64)])
+def test_fused_stem_and_heads_equal_unfused_bit_exact(C, nh, H, W, dil, tile):
+    """SMLM_FUSE_AUTO (K1 inside the first layer's kernel, K3's heads inside the last layer's
+    epilogue) against SMLM_FUSE_NONE (stem_kernel, plain layers, heads from the stored map):
+    same arithmetic and rounding points, so trunk levels and emitter records are identical
+    bit by bit - with per-pixel camera maps, ragged sizes, H < d, 1x1 frames and tiles."""
+    spec = NetSpec(C, dil, nh, "bf16")
+    w = _rand_blob(spec, 300 + C + H, scale=(2.0 / (9 * C)) ** 0.5 * 0.6)
+    off = C * 10 + len(dil) * (C * C * 9 + C)
+    w[off + nh * C] = 0.2                                     # p-head bias: a usable detection rate
+    rng = np.random.default_rng(H * 1000 + W)
+    frames = rng.integers(80, 3000, size=(3, H, W)).astype(np.uint16)
+    offm = rng.normal(100, 2, size=(H, W)).astype(np.float32)
+    gm = np.clip(rng.normal(2.0, 0.1, size=(H, W)), 0.5, None).astype(np.float32)
+    ck = dict(pixel_size_nm=100.0, offset=0.0, gain=1.0, offset_map=offm, gain_map=gm)
+    kw = dict(conv_impl=P.CONV_TCGEN05)
+    if not tile:
+        ma, ta = G.gpu_forward_maps(spec, w, frames, ck, dump_trunk=True, fusion=P.FUSE_NONE, **kw)
+        mb, tb = G.gpu_forward_maps(spec, w, frames, ck, dump_trunk=True, fusion=P.FUSE_AUTO, **kw)
+        assert np.array_equal(ta, tb) and np.array_equal(ma, mb)
+    for thr in (0.5, 0.0):
+        a = G.gpu_localize(spec, w, frames, ck, thr, fusion=P.FUSE_NONE, tile=tile, **kw)
+        b = G.gpu_localize(spec, w, frames, ck, thr, fusion=P.FUSE_AUTO, tile=tile, **kw)
+        assert len(a) == len(b) and (len(a) > 0 or H * W < 100)
+        assert a.tobytes() == b.tobytes(), thr
