@@ -143,7 +143,7 @@ def main():
     ap.add_argument("--frames", type=int, default=0, help="override the number of frames per step")
     ap.add_argument("--conv-impl", default="auto", choices=["auto", "tcgen05", "direct"])
     ap.add_argument("--micro-batch", type=int, default=0)
-    ap.add_argument("--fusion", default="auto", choices=["auto", "none"])
+    ap.add_argument("--fusion", default="auto", choices=["auto", "none", "all"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     cfg = get_config(args.config)
@@ -172,7 +172,7 @@ def main():
     conv_impl = {"auto": P.CONV_AUTO, "tcgen05": P.CONV_TCGEN05, "direct": P.CONV_DIRECT}[args.conv_impl]
     desc = P.desc_from_spec(cfg.net, tile=cfg.tile, micro_batch=args.micro_batch, conv_impl=conv_impl,
                             writeback_frames=cfg.writeback_batch,
-                            fusion={"auto": P.FUSE_AUTO, "none": P.FUSE_NONE}[args.fusion])
+                            fusion={"auto": P.FUSE_AUTO, "none": P.FUSE_NONE, "all": P.FUSE_ALL}[args.fusion])
     loc = P.Localizer(desc, weights)
     cap = int(n_frames * max(4 * cfg.frames.emitters_per_frame, 1024))
     cap = min(cap, n_frames * ((H + 1) // 2) * ((W + 1) // 2))

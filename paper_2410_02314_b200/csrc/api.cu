@@ -46,6 +46,7 @@ struct Layer {
   float* w_direct = nullptr;  // [9][C][C] (tap, ci, co)
   void* w_umma = nullptr;     // packed bf16 image for conv_umma
   float* bias = nullptr;
+  LayerConst lc{};            // the bias again, as a kernel parameter of conv_umma
   int dil = 1;
 };
 
@@ -60,13 +61,16 @@ struct smlm_ctx {
   size_t l2_bytes = 0;
 
   float *w_stem = nullptr, *b_stem = nullptr, *w_head = nullptr, *b_head = nullptr;
+  StemArgs stem_args{};  // host templates of conv_umma's parameter blocks (weights filled at create)
+  HeadArgs head_args{};
   std::vector<Layer> layers;
 
   void* act[2] = {nullptr, nullptr};
   size_t act_bytes = 0;
   float* logit = nullptr;  // detection logit of every pixel, written by the last tcgen05 layer (HEAD)
   float* cand = nullptr;   // 32-byte candidate records (other heads) of above-threshold pixels
-  bool fuse = true;        // desc.fusion != SMLM_FUSE_NONE: K1 into the first layer, K3's heads into the last
+  bool fuse = true;        // desc.fusion != SMLM_FUSE_NONE: K3's heads in the last layer's epilogue
+  bool fuse_stem = false;  // desc.fusion == SMLM_FUSE_ALL: K1 inside the first layer's kernel
 
   uint16_t* slots = nullptr;  // kSlots x slot_elems
   size_t slot_elems = 0;
@@ -180,7 +184,7 @@ smlm_status run_trunk(smlm_ctx* c, const uint16_t* dev_frames, int frame_base, c
   if (have_logit) *have_logit = false;
   const size_t nl = c->layers.size();
   // K1 folded into the first trunk layer (STEM variant) when the tcgen05 path runs it
-  const bool fuse_stem = c->use_umma && c->fuse && nl > 0 &&
+  const bool fuse_stem = c->use_umma && c->fuse_stem && nl > 0 &&
                          conv_umma_supports(c->d.channels, c->layers[0].dil, true);
   cudaEvent_t te = nullptr;
   smlm_status tr = SMLM_OK;
@@ -205,10 +209,21 @@ smlm_status run_trunk(smlm_ctx* c, const uint16_t* dev_frames, int frame_base, c
       char err[256] = {0};
       const bool head = want_logit && c->fuse && l + 1 == nl;
       const bool stem = fuse_stem && l == 0;
-      HeadArgs ha{c->w_head, c->b_head, c->d.head_channels, lthr, c->logit, c->cand};
-      StemArgs sa{dev_frames, frame_base, vs, np, c->w_stem, c->b_stem, c->d.stem_relu};
-      cudaError_t e = launch_conv_umma(c->act[cur], c->act[cur ^ 1], s, L.dil, L.w_umma, L.bias,
-                                       head ? &ha : nullptr, stem ? &sa : nullptr, c->n_sm, st, err, sizeof err);
+      if (head) {
+        c->head_args.lthr = lthr;
+        c->head_args.logit = c->logit;
+        c->head_args.cand = c->cand;
+      }
+      if (stem) {
+        c->stem_args.frames = dev_frames;
+        c->stem_args.frame_base = frame_base;
+        c->stem_args.vs = vs;
+        c->stem_args.np = np;
+        c->stem_args.relu = c->d.stem_relu;
+      }
+      cudaError_t e = launch_conv_umma(c->act[cur], c->act[cur ^ 1], s, L.dil, L.w_umma, L.lc,
+                                       head ? &c->head_args : nullptr, stem ? &c->stem_args : nullptr,
+                                       c->n_sm, st, err, sizeof err);
       if (head && have_logit) *have_logit = true;
       if (e != cudaSuccess)
         return fail(c, SMLM_ERR_CUDA, "conv_umma: %s %s", cudaGetErrorString(e), err);
@@ -358,7 +373,7 @@ smlm_status smlm_create(const smlm_net_desc* desc, const void* weights, smlm_ctx
   if (!(desc->norm_scale > 0.0f)) return fail(nullptr, SMLM_ERR_INVALID_ARG, "norm_scale must be > 0");
   if (desc->tile < 0 || desc->micro_batch < 0 || desc->writeback_frames < 0)
     return fail(nullptr, SMLM_ERR_INVALID_ARG, "negative tile / micro_batch / writeback_frames");
-  if (desc->fusion != SMLM_FUSE_AUTO && desc->fusion != SMLM_FUSE_NONE)
+  if (desc->fusion < SMLM_FUSE_AUTO || desc->fusion > SMLM_FUSE_ALL)
     return fail(nullptr, SMLM_ERR_INVALID_ARG, "bad fusion");
 
   int dev = 0;
@@ -377,6 +392,7 @@ smlm_status smlm_create(const smlm_net_desc* desc, const void* weights, smlm_ctx
   c->bf16 = desc->precision == SMLM_BF16;
   c->use_umma = c->bf16 && desc->conv_impl != SMLM_CONV_DIRECT;
   c->fuse = desc->fusion != SMLM_FUSE_NONE;
+  c->fuse_stem = desc->fusion == SMLM_FUSE_ALL;
   c->n_sm = prop.multiProcessorCount;
   c->l2_bytes = (size_t)prop.l2CacheSize;
   c->radius = 1;
@@ -394,6 +410,9 @@ smlm_status smlm_create(const smlm_net_desc* desc, const void* weights, smlm_ctx
     for (int co = 0; co < C; ++co)
       for (int t = 0; t < 9; ++t) tmp[t * C + co] = w[co * 9 + t];
     if ((st = upload(tmp, &c->w_stem)) != SMLM_OK) return st;
+    for (int t = 0; t < 9; ++t)
+      for (int co = 0; co < C; ++co) c->stem_args.w[t][co] = tmp[t * C + co];
+    for (int co = 0; co < C; ++co) c->stem_args.b[co] = w[9 * C + co];
     if ((st = upload(std::vector<float>(w + 9 * C, w + 10 * C), &c->b_stem)) != SMLM_OK) return st;
     w += 10 * C;
     c->layers.resize(L);
@@ -411,6 +430,7 @@ smlm_status smlm_create(const smlm_net_desc* desc, const void* weights, smlm_ctx
       if ((st = upload(wd, &Ly.w_direct)) != SMLM_OK) return st;
       if ((st = upload(std::vector<float>(w + (size_t)9 * C * C, w + (size_t)9 * C * C + C), &Ly.bias)) != SMLM_OK)
         return st;
+      for (int co = 0; co < C; ++co) Ly.lc.bias[co] = w[(size_t)9 * C * C + co];
       if (c->use_umma) {
         umma_pack_weights_host(C, w, pack.data());
         CK(nullptr, cudaMalloc(&Ly.w_umma, pack.size()));
@@ -419,6 +439,11 @@ smlm_status smlm_create(const smlm_net_desc* desc, const void* weights, smlm_ctx
       w += (size_t)9 * C * C + C;
     }
     if ((st = upload(std::vector<float>(w, w + nh * C), &c->w_head)) != SMLM_OK) return st;
+    for (int h = 0; h < nh; ++h) {
+      for (int ci = 0; ci < C; ++ci) c->head_args.w[ci][h] = w[h * C + ci];
+      c->head_args.b[h] = w[nh * C + h];
+    }
+    c->head_args.n_h = nh;
     if ((st = upload(std::vector<float>(w + nh * C, w + nh * C + nh), &c->b_head)) != SMLM_OK) return st;
     CK(nullptr, conv_direct_init(C));
     CK(nullptr, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));

@@ -46,6 +46,7 @@
 
 #include <cstdio>
 #include <cstring>
+#include <type_traits>
 #include <vector>
 
 #include "smlm_internal.cuh"
@@ -53,13 +54,20 @@
 namespace smlm {
 namespace {
 
-constexpr int kThreads = 384;  // warps 0 / 2: TMA lane 0 / 1 (2 also owns TMEM alloc), 1 / 3: MMA lane 0 / 1, 4-7 / 8-11: epilogue
+// warps 0-7 / 8-15: epilogue of lane 0 / 1; 16 / 18: producer of lane 0 / 1 (18 also owns the TMEM
+// allocation), 17 / 19: MMA issuer of lane 0 / 1.  Eight epilogue warps per lane: warp pair
+// (q, q + 4) shares TMEM lane quadrant q (32 pixels of the row tile) and splits the channels
+// in halves.  The epilogue's instruction stream is latency-bound (about 4.5 cycles per
+// instruction with so few warps per scheduler: profiles/), and its length per step, not the
+// MMA time, set the pace of a lane; half the channels per thread halve it.
+constexpr int kThreads = 640;
+constexpr int kEpiWarps = 8;  // per lane
 constexpr int kTileM = 128;
 constexpr int kMaxStages = 6;
 constexpr int kTmemCols = 512;
 constexpr int kLaneCols = 256;  // TMEM columns reserved per lane (3C <= 192)
 constexpr int kMaxDevices = 64;
-constexpr int kLaneBars = 2 * kMaxStages + 2 + 2 * 3;  // mbarriers per lane (SmemLayout)
+constexpr int kLaneBars = 2 * kMaxStages + 2;  // mbarriers per lane (SmemLayout)
 constexpr int kMaxDilation = 8;
 
 // zero source for the padded parts of a row segment: at most (127 + 8) pixels x 16 B
@@ -109,6 +117,11 @@ __device__ __forceinline__ void bulk_load(uint32_t dst, const void* src, uint32_
       "l"(reinterpret_cast<uint64_t>(src)), "r"(bytes), "r"(bar)
       : "memory");
 }
+__device__ __forceinline__ void cp_async4(uint32_t dst, const void* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(reinterpret_cast<uint64_t>(src)) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_commit(uint32_t bar) {
@@ -141,6 +154,17 @@ __device__ __forceinline__ void tc_st16(uint32_t taddr, const uint32_t (&r)[16])
       "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]),
       "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
       : "memory");
+}
+__device__ __forceinline__ void tc_ld8(uint32_t taddr, uint32_t (&r)[8]) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7])
+               : "r"(taddr)
+               : "memory");
+}
+__device__ __forceinline__ void tc_st8(uint32_t taddr, const uint32_t (&r)[8]) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(taddr),
+               "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7])
+               : "memory");
 }
 __device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tc_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
@@ -246,33 +270,51 @@ __device__ __forceinline__ unsigned long long ffma2(unsigned long long a, unsign
   asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
   return d;
 }
-// One pixel of a_0, all C channels, rounded to bf16 and written to the stage in operand
-// layout (chunk k of the pixel at dst + k * plane).  Two channels per fma.rn.f32x2 (two
-// independent IEEE fp32 FMAs).  valid == false (pixel outside the window): zeros.
+// Chunk k (8 channels) of a_0 for the four pixels lane, lane + 32, lane + 64, lane + 96 of a
+// 128-pixel segment, rounded to bf16 and written to the stage in operand layout.  One warp
+// per chunk: every weight fetched from shared memory (a broadcast read costs a full
+// wavefront per 4 bytes) serves four pixels, and the shared-memory pipe - which the tensor
+// core's operand fetch needs - sees a quarter of the traffic of a pixel-per-thread mapping.
+// Two channels per fma.rn.f32x2 (two independent IEEE fp32 FMAs); per channel the chain is
+// bias, then the nine taps in (ky, kx) order - the same as stem.cu, so the bits agree.
 template <int C>
-__device__ __forceinline__ void stem_pixel(const float (&xv)[9], const float* ws, const float* bs,
-                                           int relu, bool valid, uint8_t* dst, uint32_t plane) {
-  unsigned long long xx[9];
-#pragma unroll
-  for (int t = 0; t < 9; ++t) xx[t] = pack2f(xv[t], xv[t]);
-#pragma unroll 2
-  for (int k = 0; k < C / 8; ++k) {
+__device__ __forceinline__ void stem_chunk4(const float* const (&rows)[3], int d, int lane, int k,
+                                            const float* ws, const float* bs, int relu, int x0, int W,
+                                            uint8_t* stage, uint32_t plane) {
+  unsigned long long acc[4][4];
+  {
     const ulonglong2 b01 = *reinterpret_cast<const ulonglong2*>(bs + k * 8);
     const ulonglong2 b23 = *reinterpret_cast<const ulonglong2*>(bs + k * 8 + 4);
-    unsigned long long acc[4] = {b01.x, b01.y, b23.x, b23.y};
 #pragma unroll
-    for (int t = 0; t < 9; ++t) {
-      const ulonglong2 w01 = *reinterpret_cast<const ulonglong2*>(ws + t * C + k * 8);
-      const ulonglong2 w23 = *reinterpret_cast<const ulonglong2*>(ws + t * C + k * 8 + 4);
-      acc[0] = ffma2(xx[t], w01.x, acc[0]);
-      acc[1] = ffma2(xx[t], w01.y, acc[1]);
-      acc[2] = ffma2(xx[t], w23.x, acc[2]);
-      acc[3] = ffma2(xx[t], w23.y, acc[3]);
+    for (int p = 0; p < 4; ++p) {
+      acc[p][0] = b01.x;
+      acc[p][1] = b01.y;
+      acc[p][2] = b23.x;
+      acc[p][3] = b23.y;
     }
+  }
+#pragma unroll
+  for (int t = 0; t < 9; ++t) {
+    const ulonglong2 w01 = *reinterpret_cast<const ulonglong2*>(ws + t * C + k * 8);
+    const ulonglong2 w23 = *reinterpret_cast<const ulonglong2*>(ws + t * C + k * 8 + 4);
+    const float* prow = rows[t / 3] + d + lane + t % 3;
+#pragma unroll
+    for (int p = 0; p < 4; ++p) {
+      const float x = prow[32 * p];
+      const unsigned long long xx = pack2f(x, x);
+      acc[p][0] = ffma2(xx, w01.x, acc[p][0]);
+      acc[p][1] = ffma2(xx, w01.y, acc[p][1]);
+      acc[p][2] = ffma2(xx, w23.x, acc[p][2]);
+      acc[p][3] = ffma2(xx, w23.y, acc[p][3]);
+    }
+  }
+#pragma unroll
+  for (int p = 0; p < 4; ++p) {
     uint32_t ow[4];
+    const bool valid = x0 + lane + 32 * p < W;
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-      float v0 = __uint_as_float((uint32_t)acc[i]), v1 = __uint_as_float((uint32_t)(acc[i] >> 32));
+      float v0 = __uint_as_float((uint32_t)acc[p][i]), v1 = __uint_as_float((uint32_t)(acc[p][i] >> 32));
       if (relu) {
         v0 = fmaxf(v0, 0.0f);
         v1 = fmaxf(v1, 0.0f);
@@ -280,39 +322,41 @@ __device__ __forceinline__ void stem_pixel(const float (&xv)[9], const float* ws
       __nv_bfloat162 h = __floats2bfloat162_rn(v0, v1);
       ow[i] = valid ? *reinterpret_cast<uint32_t*>(&h) : 0u;
     }
-    *reinterpret_cast<uint4*>(dst + (size_t)k * plane) = make_uint4(ow[0], ow[1], ow[2], ow[3]);
+    *reinterpret_cast<uint4*>(stage + (size_t)k * plane + (size_t)(d + lane + 32 * p) * 16u) =
+        make_uint4(ow[0], ow[1], ow[2], ow[3]);
   }
 }
 
-constexpr int kPatchSlots = 3;  // STEM: ring of normalised input patches per lane
+constexpr int kRingRows = 8;  // STEM: ring of normalised input rows per lane
 
 struct SmemLayout {
   uint32_t w_off, w_bytes;
   uint32_t stage_off, stage_bytes;  // per (lane, stage)
-  uint32_t bias_off;  // float: layer bias [C], detection-head row [C], other head rows [C][8], head bias [8]
-  uint32_t stem_off;  // float: stem weights [9][C], stem bias [C]
-  uint32_t patch_off, patch_bytes, patch_row;  // STEM: per (lane, slot): float xhat[3][patch_row], int x0
+  uint32_t xch_off;   // HEAD: float [2 lanes][128 px][8] partial head sums of the upper channel half
+  uint32_t stem_off;  // STEM: float stem weights [9][C], stem bias [C]
+  uint32_t patch_off, patch_bytes, patch_row;  // STEM: per lane: float xhat[kRingRows][patch_row]
+  uint32_t raw_off;   // STEM: uint32 raw[2 lanes][2 sets][5 fields][256 threads] (cp.async landing slots)
   uint32_t bar_off;
   uint32_t tmem_off;
   uint32_t total;
   int nstage;
 };
 
-__host__ __device__ inline SmemLayout smem_layout(int C, int d, int nstage, bool stem) {
+__host__ __device__ inline SmemLayout smem_layout(int C, int d, int nstage, bool stem, bool head) {
   SmemLayout L;
   L.w_off = 0;
   L.w_bytes = 30u * C * C;  // 3 kx * C/8 chunks * 5C rows * 16 B
   L.stage_bytes = (((uint32_t)(C / 8) * (kTileM + 2 * d) * 16u) + 127u) & ~127u;
   L.stage_off = (L.w_off + L.w_bytes + 127u) & ~127u;
   L.nstage = nstage;
-  L.bias_off = L.stage_off + 2u * nstage * L.stage_bytes;
-  L.stem_off = L.bias_off + (uint32_t)(10 * C + 8) * 4u;
-  L.patch_off = L.stem_off + (uint32_t)(10 * C) * 4u;
+  L.xch_off = L.stage_off + 2u * nstage * L.stage_bytes;
+  L.stem_off = L.xch_off + (head ? 2u * kTileM * 8u * 4u : 0u);
+  L.patch_off = L.stem_off + (stem ? (uint32_t)(10 * C) * 4u : 0u);
   L.patch_row = (uint32_t)(kTileM + 2 * d + 2 + 3) & ~3u;  // the segment plus the stem's own 1-px halo
-  L.patch_bytes = stem ? (3u * L.patch_row + 4u) * 4u : 0u;
-  L.bar_off = L.patch_off + 2u * kPatchSlots * L.patch_bytes;
-  // barriers: wbar, per lane: full[kMaxStages], empty[kMaxStages], acc_full, acc_free,
-  // patch_full[kPatchSlots], patch_empty[kPatchSlots]
+  L.patch_bytes = stem ? (uint32_t)kRingRows * L.patch_row * 4u : 0u;
+  L.raw_off = L.patch_off + 2u * L.patch_bytes;
+  L.bar_off = L.raw_off + (stem ? 2u * 2u * 5u * 256u * 4u : 0u);
+  // barriers: wbar, per lane: full[kMaxStages], empty[kMaxStages], acc_full, acc_free
   L.tmem_off = L.bar_off + 8u * (1 + 2 * kLaneBars);
   L.total = L.tmem_off + 16u;
   return L;
@@ -326,14 +370,19 @@ __host__ __device__ inline SmemLayout smem_layout(int C, int d, int nstage, bool
 template <int C, bool HEAD, bool STEM>
 __global__ void __launch_bounds__(kThreads, 1)
     conv_umma_kernel(const __nv_bfloat16* __restrict__ in, __nv_bfloat16* __restrict__ out, Geo geo,
-                     const uint8_t* __restrict__ wpack, const float* __restrict__ bias, int nstage,
-                     const HeadArgs ha, const StemArgs sa) {
+                     const uint8_t* __restrict__ wpack, int nstage, const __grid_constant__ LayerConst lc,
+                     const __grid_constant__ HeadArgs ha, const __grid_constant__ StemArgs sa) {
   extern __shared__ uint8_t smem_raw[];
-  const SmemLayout L = smem_layout(C, geo.d, nstage, STEM);
+  const SmemLayout L = smem_layout(C, geo.d, nstage, STEM, HEAD);
   const uint32_t sraw = smem_u32(smem_raw);
   const uint32_t sbase = (sraw + 1023u) & ~1023u;  // the launch reserves 1 KB of slack for this
   uint8_t* smem = smem_raw + (sbase - sraw);
+  // Role of a warp.  The schedulers favour the highest warp id among eligible warps, so the
+  // four single-thread roles (which feed the tensor pipe and must never queue behind the
+  // epilogue's long instruction streams) take the top ids: role 0 / 2 = producer of lane 0 / 1,
+  // 1 / 3 = MMA issuer of lane 0 / 1; warps 0 .. 15 are the epilogue (quadrant = warp % 4).
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int role = warp - 2 * kEpiWarps;  // < 0: epilogue
   const int d = geo.d;
 
   const uint32_t wbar = sbase + L.bar_off;
@@ -342,13 +391,11 @@ __global__ void __launch_bounds__(kThreads, 1)
   auto empty_bar = [&](int ln, int s) { return lane_bar(ln, kMaxStages + s); };
   auto acc_full_bar = [&](int ln) { return lane_bar(ln, 2 * kMaxStages); };
   auto acc_free_bar = [&](int ln) { return lane_bar(ln, 2 * kMaxStages + 1); };
-  auto patch_full_bar = [&](int ln, int s) { return lane_bar(ln, 2 * kMaxStages + 2 + s); };
-  auto patch_empty_bar = [&](int ln, int s) { return lane_bar(ln, 2 * kMaxStages + 2 + kPatchSlots + s); };
-  auto patch_ptr = [&](int ln, int s) {
-    return reinterpret_cast<float*>(smem + L.patch_off + (uint32_t)(ln * kPatchSlots + s) * L.patch_bytes);
-  };
   auto stage_addr = [&](int ln, int s) { return sbase + L.stage_off + (uint32_t)(ln * nstage + s) * L.stage_bytes; };
-  float* bias_s = reinterpret_cast<float*>(smem + L.bias_off);
+  auto ring_row = [&](int ln, int r) {
+    return reinterpret_cast<float*>(smem + L.patch_off + (uint32_t)ln * L.patch_bytes) +
+           (size_t)(r & (kRingRows - 1)) * L.patch_row;
+  };
   volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + L.tmem_off);
 
   // ---- one-time setup
@@ -356,42 +403,26 @@ __global__ void __launch_bounds__(kThreads, 1)
     mbar_init(wbar, 1);
     for (int ln = 0; ln < 2; ++ln) {
       for (int s = 0; s < kMaxStages; ++s) {
-        // full: the TMA transaction count, or (STEM) the four epilogue warps
-        mbar_init(full_bar(ln, s), STEM ? 4 : 1);
-        mbar_init(empty_bar(ln, s), 5);  // MMA commit + one arrival per epilogue warp
+        // full: the TMA transaction count, or (STEM) the epilogue warps
+        mbar_init(full_bar(ln, s), STEM ? kEpiWarps : 1);
+        mbar_init(empty_bar(ln, s), 1 + kEpiWarps);  // MMA commit + one arrival per epilogue warp
       }
       mbar_init(acc_full_bar(ln), 1);
-      mbar_init(acc_free_bar(ln), 4);  // one arrival per epilogue warp
-      for (int s = 0; s < kPatchSlots; ++s) {
-        mbar_init(patch_full_bar(ln, s), 1);   // the producer warp
-        mbar_init(patch_empty_bar(ln, s), 4);  // one arrival per epilogue warp
-      }
+      mbar_init(acc_free_bar(ln), kEpiWarps);  // one arrival per epilogue warp
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
-  if (warp == 2) {
+  if (role == 2) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(sbase + L.tmem_off),
                  "n"(kTmemCols)
                  : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
-  for (int i = threadIdx.x; i < C; i += kThreads) bias_s[i] = bias[i];
-  float* head_s = bias_s + C;        // detection head row [C]
-  float* headq_s = bias_s + 2 * C;   // [C][8]: rows 1 .. n_h-1 of channel c, zero padded
-  float* headb_s = bias_s + 10 * C;  // [8]: head biases 0 .. n_h-1, zero padded
-  if (HEAD) {
-    for (int i = threadIdx.x; i < C; i += kThreads) head_s[i] = ha.w[i];
-    for (int i = threadIdx.x; i < 8 * C; i += kThreads) {
-      const int c = i >> 3, h = 1 + (i & 7);
-      headq_s[i] = h < ha.n_h ? ha.w[h * C + c] : 0.0f;
-    }
-    if (threadIdx.x < 8) headb_s[threadIdx.x] = (int)threadIdx.x < ha.n_h ? ha.b[threadIdx.x] : 0.0f;
-  }
   float* stem_w_s = reinterpret_cast<float*>(smem + L.stem_off);  // [9][C]
   float* stem_b_s = stem_w_s + 9 * C;
   if (STEM) {
-    for (int i = threadIdx.x; i < 9 * C; i += kThreads) stem_w_s[i] = sa.w[i];
+    for (int i = threadIdx.x; i < 9 * C; i += kThreads) stem_w_s[i] = sa.w[i / C][i % C];
     for (int i = threadIdx.x; i < C; i += kThreads) stem_b_s[i] = sa.b[i];
   }
   tc_fence_before();
@@ -410,10 +441,10 @@ __global__ void __launch_bounds__(kThreads, 1)
   // addresses in uniform registers (inside an `if (lane == 0)` region it falls back to a
   // per-instruction R2UR broadcast loop, ~19 instructions per MMA: the issue thread, not
   // the tensor pipe, was then the limiter - profiles/conv_umma_r1_full.md).
-  if (warp == 0 || warp == 2) {
+  if (role == 0 || role == 2) {
     // =========================== TMA producers: warp 0 -> lane 0, warp 2 -> lane 1 ========
-    const int ln = warp >> 1;
-    if (warp == 0 && elect_one()) {
+    const int ln = role >> 1;
+    if (role == 0 && elect_one()) {
       // the layer's weights: one bulk copy stream into shared memory, resident for the launch
       mbar_expect_tx(wbar, L.w_bytes);
       for (uint32_t off = 0; off < L.w_bytes; off += 16384u) {
@@ -426,102 +457,7 @@ __global__ void __launch_bounds__(kThreads, 1)
     // still reading `out`) before the first activation access.
     asm volatile("griddepcontrol.wait;" ::: "memory");
     if (STEM) {
-      // STEM producer.  Per valid step: (1) the normalised input patch xhat[3][130 + 2d] (rows
-      // row-1, row, row+1; columns x0-d-1 .. x0+128+d) goes to a ring in shared memory, from
-      // which the epilogue threads take the inputs of their pixel (and of the 2d halo pixels
-      // of the segment, which they share out by channel).  When a step continues the previous
-      // one with d = 1, two of its three rows are the previous patch's rows 1 and 2 (copied
-      // inside shared memory) and only the new row is loaded.  The global loads of step s+1
-      // are in flight while step s is processed (two register sets, loop unrolled by two),
-      // and the warp runs as far ahead as the rings allow: it is off the critical path.
-      const int pcols = kTileM + 2 * d + 2;      // patch columns in use
-      constexpr int NJ = (kTileM + 2 * kMaxDilation + 2 + 31) / 32;  // column passes per row
-      ValidSteps steps;
-      steps.init(geo, 2 * blockIdx.x + ln, nlanes);
-      uint32_t ps = 0, pempty_par = 1;
-      struct Raw {
-        uint16_t adu[3][NJ];
-        float om[3][NJ], gm[3][NJ];
-      };
-      // (uniform branches on `reuse`: predicated-off instructions would still cost issue slots)
-      auto issue = [&](const Step& sp, bool reuse, Raw& rw) {
-        const View v = view_of(sa.vs, sp.b, geo.H, geo.W);
-        const uint16_t* frame = sa.frames + (size_t)(v.frame - sa.frame_base) * sa.vs.Hf * sa.vs.Wf;
-        const int fx0 = v.wx0 + sp.x0 - d - 1 + lane;
-        auto load_row = [&](int py, uint16_t (&adu)[NJ], float (&om)[NJ], float (&gm)[NJ]) {
-          const int fy = v.wy0 + sp.row - 1 + py;
-          const bool row_ok = fy >= 0 && fy < sa.vs.Hf;
-          const size_t rowq = (size_t)(row_ok ? fy : 0) * sa.vs.Wf;
-#pragma unroll
-          for (int j = 0; j < NJ; ++j) {
-            const int fx = fx0 + 32 * j;
-            const bool ok = row_ok && lane + 32 * j < pcols && fx >= 0 && fx < sa.vs.Wf;
-            const size_t q = rowq + (ok ? fx : 0);
-            adu[j] = ok ? __ldg(frame + q) : (uint16_t)0;  // (0 - 0) / 1 normalises to exactly 0
-            om[j] = ok ? (sa.np.offset_map ? __ldg(sa.np.offset_map + q) : sa.np.offset) : 0.0f;
-            gm[j] = ok ? (sa.np.offset_map ? __ldg(sa.np.gain_map + q) : sa.np.gain) : 1.0f;
-          }
-        };
-        if (!reuse) {
-          load_row(0, rw.adu[0], rw.om[0], rw.gm[0]);
-          load_row(1, rw.adu[1], rw.om[1], rw.gm[1]);
-        }
-        load_row(2, rw.adu[2], rw.om[2], rw.gm[2]);
-      };
-      auto process = [&](const Step& sp, bool reuse, const Raw& rw) {
-        float* patch = patch_ptr(ln, ps);
-        const float* prev = patch_ptr(ln, ps == 0 ? kPatchSlots - 1 : ps - 1);
-        mbar_wait(patch_empty_bar(ln, ps), pempty_par);
-        auto norm_row = [&](int py, const uint16_t (&adu)[NJ], const float (&om)[NJ], const float (&gm)[NJ]) {
-#pragma unroll
-          for (int j = 0; j < NJ; ++j) {
-            const int pxx = lane + 32 * j;
-            if (pxx < pcols)
-              patch[py * L.patch_row + pxx] = (((float)adu[j] - om[j]) / gm[j]) / sa.np.norm_scale;
-          }
-        };
-        if (reuse) {
-#pragma unroll
-          for (int j = 0; j < NJ; ++j) {
-            const int pxx = lane + 32 * j;
-            if (pxx < pcols) {
-              patch[pxx] = prev[L.patch_row + pxx];
-              patch[L.patch_row + pxx] = prev[2 * L.patch_row + pxx];
-            }
-          }
-        } else {
-          norm_row(0, rw.adu[0], rw.om[0], rw.gm[0]);
-          norm_row(1, rw.adu[1], rw.om[1], rw.gm[1]);
-        }
-        norm_row(2, rw.adu[2], rw.om[2], rw.gm[2]);
-        if (lane == 0) reinterpret_cast<int*>(patch)[3 * L.patch_row] = sp.x0;
-        __syncwarp();
-        if (lane == 0) mbar_arrive(patch_full_bar(ln, ps));
-        if (++ps == (uint32_t)kPatchSlots) {
-          ps = 0;
-          pempty_par ^= 1u;
-        }
-      };
-      // a step continues the previous one (same view and segment, next row) iff d == 1
-      auto continues = [&](const Step& a, const Step& b) {
-        return d == 1 && b.b == a.b && b.x0 == a.x0 && b.row == a.row + 1;
-      };
-      Raw rA, rB;
-      Step sA{0, 0, 0}, sB{0, 0, 0};
-      bool reA = false, reB = false;
-      bool haveA = steps.next(geo, sA), haveB = false;
-      if (haveA) issue(sA, false, rA);
-      while (haveA) {
-        haveB = steps.next(geo, sB);
-        reB = haveB && continues(sA, sB);
-        if (haveB) issue(sB, reB, rB);
-        process(sA, reA, rA);
-        if (!haveB) break;
-        haveA = steps.next(geo, sA);
-        reA = haveA && continues(sB, sA);
-        if (haveA) issue(sA, reA, rA);
-        process(sB, reB, rB);
-      }
+      // (the lane's epilogue warps produce the input themselves, see below)
     } else {
       // One input row segment = C/8 contiguous runs of (128 + 2d) pixels x 16 B in the
       // chunk-planar layout: one 1-D bulk copy each (a tensor-map box with a 16-byte inner
@@ -577,12 +513,12 @@ __global__ void __launch_bounds__(kThreads, 1)
         }
       }
     }
-  } else if (warp == 1 || warp == 3) {
+  } else if (role == 1 || role == 3) {
     // =========================== MMA issuers: warp 1 -> lane 0, warp 3 -> lane 1 ==========
     // One issuing warp per lane: the tensor pipe's instruction queue is short, so while one
     // warp is busy with barriers and bookkeeping between two steps the other one's MMAs keep
     // the pipe fed (the lanes are independent: own TMEM columns, own stages).
-    const int ln = warp >> 1;
+    const int ln = role >> 1;
     asm volatile("griddepcontrol.wait;" ::: "memory");
     mbar_wait(wbar, 0);
     constexpr uint32_t idesc = umma_idesc(kTileM, 3 * C);
@@ -633,21 +569,32 @@ __global__ void __launch_bounds__(kThreads, 1)
         m = m == 2 ? 0u : m + 1u;
       }
     }
-  } else if (warp >= 4) {
+  } else {
     // =========================== epilogue ===========================
-    const int ln = (warp - 4) >> 2;
-    const int qd = warp & 3;  // TMEM lane quadrant this warp may access
+    const int e = warp;
+    const int ln = e >> 3;       // lane of the CTA
+    const int qd = warp & 3;     // TMEM lane quadrant this warp may access
+    const int half = (e >> 2) & 1;
+    constexpr int CH = C / 2;    // channels per thread
+    constexpr int KH = C / 16;   // 8-channel chunks per thread
+    const int k0 = half * KH;    // first chunk
     asm volatile("griddepcontrol.wait;" ::: "memory");
     const int px = qd * 32 + lane;
-    const uint32_t tlane = tmem_base + ((uint32_t)(qd * 32) << 16) + (uint32_t)ln * kLaneCols;
+    const uint32_t tlane = tmem_base + ((uint32_t)(qd * 32) << 16) + (uint32_t)ln * kLaneCols + (uint32_t)(half * CH);
+    // the CH accumulator columns of this thread: groups of 16 (and one of 8 when CH % 16 == 8)
+    auto ld_cols = [&](uint32_t slot, uint32_t (&acc)[CH]) {
+#pragma unroll
+      for (int g = 0; g + 16 <= CH; g += 16)
+        tc_ld16(tlane + slot * C + g, *reinterpret_cast<uint32_t(*)[16]>(&acc[g]));
+      if (CH % 16) tc_ld8(tlane + slot * C + (CH - 8), *reinterpret_cast<uint32_t(*)[8]>(&acc[CH - 8]));
+    };
+    // a finished slot is re-armed with zeros (registers only); the bias is added below
     auto init_slot = [&](uint32_t slot) {
+      const uint32_t z16[16] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
+      const uint32_t z8[8] = {0u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
 #pragma unroll
-      for (int g16 = 0; g16 < C / 16; ++g16) {
-        uint32_t v[16];
-#pragma unroll
-        for (int i = 0; i < 16; ++i) v[i] = __float_as_uint(bias_s[g16 * 16 + i]);
-        tc_st16(tlane + slot * C + g16 * 16, v);
-      }
+      for (int g = 0; g + 16 <= CH; g += 16) tc_st16(tlane + slot * C + g, z16);
+      if (CH % 16) tc_st8(tlane + slot * C + (CH - 8), z8);
     };
     init_slot(0);
     init_slot(1);
@@ -674,41 +621,134 @@ __global__ void __launch_bounds__(kThreads, 1)
     //     it after use; no extra registers, no fence (3 % faster at C = 48).
     constexpr bool kEarly = C >= 64;
 
-    // STEM: this thread computes pixel x0 + px of a_0 for the segment of the valid step that is
-    // two steps ahead of the one being retired (the MMAs of the step in between are running
-    // meanwhile).  Its nine inputs come from the producer warp's patch ring.
-    uint32_t sst = 0, sempty_par = 1, sps = 0, spfull_par = 0;
-    long long stems_left = 0;
-    auto stem_advance = [&]() {
-      if (stems_left <= 0) return;
-      --stems_left;
-      const float* patch = patch_ptr(ln, sps);
-      mbar_wait(patch_full_bar(ln, sps), spfull_par);
-      float xv[9];
+    // STEM (K1 folded in): the lane's 256 epilogue threads build the layer's input themselves.
+    // For the valid step that is two steps ahead of the one being retired (the MMAs of the
+    // step in between are running meanwhile) they need the normalised rows row-1, row, row+1,
+    // columns x0-d-1 .. x0+128+d.  Rows live in a ring in shared memory; when a step continues
+    // the previous one with d = 1 only its last row is new.  One thread per aligned 32-bit
+    // word of a raw uint16 row (two pixels; plus the two offset / gain values of a per-pixel
+    // camera): the words are fetched with cp.async one call ahead into the thread's own
+    // shared-memory slots - asynchronous copies stay in flight across the fences and barrier
+    // arrivals of a step, which ordinary loads do not - and normalised into the ring now.  A
+    // 256-thread named barrier makes the rows visible; then warp = channel chunk, thread =
+    // four pixels compute a_0 into the stage (stem_chunk4), plus the 2d halo pixels shared out
+    // by channel.  (A word may straddle the end of a row, so up to two bytes beyond the last
+    // pixel of the frame buffer are read; they are never used.)
+    struct StemPend {
+      Step sp;
+      int base;    // ring slot of the step's first row
+      bool reuse;  // rows 0 and 1 are the previous step's rows 1 and 2
+    };
+    const int ew = e & 7;            // epilogue warp within the lane: the stem's channel chunk
+    const int et = ew * 32 + lane;   // thread within the lane's epilogue
+    const int pcols = kTileM + 2 * d + 2;
+    const int aw = pcols / 2 + 1;    // words that cover a row of pcols pixels at any alignment
+    const int lane_bar = 9 + ln;
+    // this thread's word: row 2 (the new row) for et < aw, row 0 for aw <= et < 2 aw, row 1 next
+    const int my_py = et < aw ? 2 : (et < 2 * aw ? 0 : (et < 3 * aw ? 1 : -1));
+    const int my_w = et < aw ? et : (et < 2 * aw ? et - aw : et - 2 * aw);
+    uint32_t* raw_base = reinterpret_cast<uint32_t*>(smem + L.raw_off) + (size_t)ln * 2 * 5 * 256 + et;
+    ValidSteps ssteps;
+    StemPend pend{{0, 0, 0}, 0, false};
+    bool have_pend = false;
+    int sset = 0;
+    uint32_t sst = 0, sempty_par = 1;
+    // pixel column (in the patch) of the first pixel of this thread's word, and its frame position
+    auto word_geom = [&](const StemPend& pd, int& col0, long long& q0, bool& row_ok, const uint16_t*& frame) {
+      const View v = view_of(sa.vs, pd.sp.b, geo.H, geo.W);
+      frame = sa.frames + (size_t)(v.frame - sa.frame_base) * sa.vs.Hf * sa.vs.Wf;
+      const int fy = v.wy0 + pd.sp.row - 1 + my_py, fx0 = v.wx0 + pd.sp.x0 - d - 1;
+      row_ok = fy >= 0 && fy < sa.vs.Hf;
+      const long long qrow = (long long)fy * sa.vs.Wf + fx0;  // pixel index of patch column 0
+      // alignment of patch column 0 inside its 32-bit word: 0 or 1 pixels
+      const int sh = (int)((reinterpret_cast<uintptr_t>(frame + qrow) >> 1) & 1);
+      col0 = 2 * my_w - sh;
+      q0 = qrow + col0;
+    };
+    auto stem_issue = [&](const StemPend& pd, int set) {
+      if (my_py < 0 || (pd.reuse && my_py != 2)) return;
+      int col0;
+      long long q0;
+      bool row_ok;
+      const uint16_t* frame;
+      word_geom(pd, col0, q0, row_ok, frame);
+      uint32_t* slot = raw_base + (size_t)set * 5 * 256;
+      const View v = view_of(sa.vs, pd.sp.b, geo.H, geo.W);
+      const int fxa = v.wx0 + pd.sp.x0 - d - 1 + col0;  // frame x of the word's first pixel
+      const bool in0 = row_ok && col0 >= 0 && col0 < pcols && fxa >= 0 && fxa < sa.vs.Wf;
+      const bool in1 = row_ok && col0 + 1 >= 0 && col0 + 1 < pcols && fxa + 1 >= 0 && fxa + 1 < sa.vs.Wf;
+      if (in0 || in1) cp_async4(smem_u32(slot), frame + q0);
+      if (sa.np.offset_map) {
+        if (in0) {
+          cp_async4(smem_u32(slot + 256), sa.np.offset_map + q0);
+          cp_async4(smem_u32(slot + 3 * 256), sa.np.gain_map + q0);
+        }
+        if (in1) {
+          cp_async4(smem_u32(slot + 2 * 256), sa.np.offset_map + q0 + 1);
+          cp_async4(smem_u32(slot + 4 * 256), sa.np.gain_map + q0 + 1);
+        }
+      }
+    };
+    auto stem_store = [&](const StemPend& pd, int set) {
+      if (my_py < 0 || (pd.reuse && my_py != 2)) return;
+      int col0;
+      long long q0;
+      bool row_ok;
+      const uint16_t* frame;
+      word_geom(pd, col0, q0, row_ok, frame);
+      const View v = view_of(sa.vs, pd.sp.b, geo.H, geo.W);
+      const int fxa = v.wx0 + pd.sp.x0 - d - 1 + col0;
+      const uint32_t* slot = raw_base + (size_t)set * 5 * 256;
+      const uint32_t wv = slot[0];
+      float* rowp = ring_row(ln, pd.base + my_py);
 #pragma unroll
-      for (int t = 0; t < 9; ++t) xv[t] = patch[(t / 3) * L.patch_row + d + px + t % 3];
-      const int x0 = reinterpret_cast<const int*>(patch)[3 * L.patch_row];
+      for (int i = 0; i < 2; ++i) {
+        const int col = col0 + i;
+        if (col < 0 || col >= pcols) continue;
+        const bool in = row_ok && fxa + i >= 0 && fxa + i < sa.vs.Wf;
+        float xh = 0.0f;
+        if (in) {
+          const float adu = (float)(i ? (wv >> 16) : (wv & 0xffffu));
+          const float om = sa.np.offset_map ? __uint_as_float(slot[(1 + i) * 256]) : sa.np.offset;
+          const float gm = sa.np.offset_map ? __uint_as_float(slot[(3 + i) * 256]) : sa.np.gain;
+          xh = ((adu - om) / gm) / sa.np.norm_scale;
+        }
+        rowp[col] = xh;
+      }
+    };
+    auto stem_advance = [&]() {
+      if (!have_pend) return;
+      cp_async_wait_all();  // this thread's words of the pending step (issued one call ago)
+      stem_store(pend, sset);
+      StemPend nx;
+      const bool have_next = ssteps.next(geo, nx.sp);
+      if (have_next) {
+        nx.reuse = d == 1 && nx.sp.b == pend.sp.b && nx.sp.x0 == pend.sp.x0 && nx.sp.row == pend.sp.row + 1;
+        nx.base = pend.base + (nx.reuse ? 1 : 3);
+        stem_issue(nx, sset ^ 1);  // in flight until the next call
+      }
+      cp_async_commit();
+      asm volatile("bar.sync %0, 256;" ::"r"(lane_bar) : "memory");
+      const float* const rows[3] = {ring_row(ln, pend.base), ring_row(ln, pend.base + 1),
+                                    ring_row(ln, pend.base + 2)};
+      const int x0 = pend.sp.x0;
       mbar_wait(empty_bar(ln, sst), sempty_par);
       uint8_t* stage = smem + (stage_addr(ln, sst) - sbase);
-      const uint32_t splane = (uint32_t)(kTileM + 2 * d) * 16u;
+      if (ew < C / 8) stem_chunk4<C>(rows, d, lane, ew, stem_w_s, stem_b_s, sa.relu, x0, geo.W, stage, plane);
       // the 2d halo pixels of the segment (positions [0, d) and [d + 128, 128 + 2d)): one
       // (pixel, channel) output per thread and pass, the same fmaf chain
-      for (int o = px; o < 2 * d * C; o += kTileM) {
+      for (int o = et; o < 2 * d * C; o += 32 * kEpiWarps) {
         const int h = o / C, c = o - h * C;
         const int pos = h < d ? h : kTileM + h;  // position in the (128 + 2d)-pixel segment
         const int x = x0 - d + pos;              // window coordinate
         float a = stem_b_s[c];
 #pragma unroll
-        for (int t = 0; t < 9; ++t)
-          a = fmaf(patch[(t / 3) * L.patch_row + pos + t % 3], stem_w_s[t * C + c], a);
+        for (int t = 0; t < 9; ++t) a = fmaf(rows[t / 3][pos + t % 3], stem_w_s[t * C + c], a);
         if (sa.relu) a = fmaxf(a, 0.0f);
         const __nv_bfloat16 hb = __float2bfloat16_rn(a);
         const uint16_t bits = (x >= 0 && x < geo.W) ? *reinterpret_cast<const uint16_t*>(&hb) : (uint16_t)0;
-        *reinterpret_cast<uint16_t*>(stage + (size_t)(c >> 3) * splane + (size_t)pos * 16u + (c & 7) * 2) = bits;
+        *reinterpret_cast<uint16_t*>(stage + (size_t)(c >> 3) * plane + (size_t)pos * 16u + (c & 7) * 2) = bits;
       }
-      __syncwarp();
-      if (lane == 0) mbar_arrive(patch_empty_bar(ln, sps));
-      stem_pixel<C>(xv, stem_w_s, stem_b_s, sa.relu, x0 + px < geo.W, stage + (size_t)(d + px) * 16u, splane);
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
       __syncwarp();
       if (lane == 0) mbar_arrive(full_bar(ln, sst));
@@ -716,33 +756,38 @@ __global__ void __launch_bounds__(kThreads, 1)
         sst = 0;
         sempty_par ^= 1u;
       }
-      if (++sps == (uint32_t)kPatchSlots) {
-        sps = 0;
-        spfull_par ^= 1u;
-      }
+      pend = nx;
+      have_pend = have_next;
+      sset ^= 1;
     };
     if (STEM) {
-      ValidSteps cnt;  // number of valid steps of this lane
-      cnt.init(geo, 2 * blockIdx.x + ln, nlanes);
-      Step tmp;
-      while (cnt.next(geo, tmp)) ++stems_left;
+      ssteps.init(geo, 2 * blockIdx.x + ln, nlanes);
+      have_pend = ssteps.next(geo, pend.sp);
+      if (have_pend) stem_issue(pend, sset);
+      cp_async_commit();
       stem_advance();
       stem_advance();
     }
+
+    // HEAD: every head is the sum of two fmaf chains, one per channel half (head_post.cu
+    // evaluates the same two chains), so the warp pair exchanges partial sums: half 1 hands
+    // its six partials to half 0 through shared memory (one 64-thread named barrier).
+    float* xch = reinterpret_cast<float*>(smem + L.xch_off) + (size_t)(ln * kTileM + px) * 8;
+    const int pair_bar = 1 + ln * 4 + qd;
 
     LaneRuns runs;
     runs.init(geo, 2 * blockIdx.x + ln, nlanes);
     Run run;
     uint32_t slot = 2, acc_par = 0, st = 0, prev_st = 0;
     bool prev_valid = false;
-    uint4 res[C / 8];
+    uint4 res[KH];
 #pragma unroll
-    for (int k = 0; k < C / 8; ++k) res[k] = make_uint4(0u, 0u, 0u, 0u);
+    for (int k = 0; k < KH; ++k) res[k] = make_uint4(0u, 0u, 0u, 0u);
     while (runs.next(geo, run)) {
       const int x = run.x0 + px;
       int row = run.r + (run.i0 - 1) * d;  // input row of the step; the output row is row - d
       uint4* orow = reinterpret_cast<uint4*>(out) +
-                    ((size_t)run.b * (C / 8) * geo.H * geo.W + (long long)(row - d) * geo.W + x);
+                    (((size_t)run.b * (C / 8) + k0) * geo.H * geo.W + (long long)(row - d) * geo.W + x);
       for (int j = 0; j < run.n + 2; ++j, row += d, orow += (size_t)d * geo.W) {
         const bool in_valid = row >= 0 && row < geo.H;
         const bool out_valid = j >= 2 && row - d < geo.H;
@@ -750,11 +795,9 @@ __global__ void __launch_bounds__(kThreads, 1)
         mbar_wait(acc_full_bar(ln), acc_par);
         acc_par ^= 1u;
         tc_fence_after();
-        uint32_t acc[C];
+        uint32_t acc[CH];
         if (out_valid) {
-#pragma unroll
-          for (int g16 = 0; g16 < C / 16; ++g16)
-            tc_ld16(tlane + slot * C + g16 * 16, *reinterpret_cast<uint32_t(*)[16]>(&acc[g16 * 16]));
+          ld_cols(slot, acc);
           tc_wait_ld();
         }
         init_slot(slot);
@@ -766,64 +809,71 @@ __global__ void __launch_bounds__(kThreads, 1)
         // lane's MMA warp, whose tcgen05.commit on acc_full this thread has observed in turn)
         const uint4* rprev = reinterpret_cast<const uint4*>(smem + (stage_addr(ln, prev_st) - sbase) +
                                                             (uint32_t)(d + px) * 16u);
-        if (store) {
-          float lg = HEAD ? headb_s[0] : 0.0f;
-          uint32_t orw[HEAD ? C / 2 : 1];  // HEAD: the rounded output row stays in registers
+        // ReLU(acc + bias) + residual, one RNE rounding, store; HEAD: this half's partial sums
+        // of the six heads on the rounded values.  Specialised on the channel half so that
+        // bias and head weights are compile-time-indexed kernel parameters.
+        float hp[6] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};
+        auto post = [&](auto HALF) {
+          constexpr int kHalf = decltype(HALF)::value;
+          if (HEAD && kHalf == 0) {
 #pragma unroll
-          for (int k = 0; k < C / 8; ++k) {
-            const uint4 rk = kEarly ? res[k] : rprev[(size_t)k * (plane / 16u)];
+            for (int h = 0; h < 6; ++h) hp[h] = ha.b[h];
+          }
+#pragma unroll
+          for (int kk = 0; kk < KH; ++kk) {
+            constexpr int kc0 = kHalf * KH;
+            const uint4 rk = kEarly ? res[kk] : rprev[(size_t)(kc0 + kk) * (plane / 16u)];
             const uint32_t rw[4] = {rk.x, rk.y, rk.z, rk.w};
             uint32_t ow[4];
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
+              const int c0 = (kc0 + kk) * 8 + 2 * i;
               float r0 = __uint_as_float(rw[i] << 16), r1 = __uint_as_float(rw[i] & 0xffff0000u);
-              float v0 = r0 + fmaxf(__uint_as_float(acc[k * 8 + 2 * i]), 0.0f);
-              float v1 = r1 + fmaxf(__uint_as_float(acc[k * 8 + 2 * i + 1]), 0.0f);
-              __nv_bfloat162 h = __floats2bfloat162_rn(v0, v1);
-              ow[i] = *reinterpret_cast<uint32_t*>(&h);
+              float v0 = r0 + fmaxf(__uint_as_float(acc[kk * 8 + 2 * i]) + lc.bias[c0], 0.0f);
+              float v1 = r1 + fmaxf(__uint_as_float(acc[kk * 8 + 2 * i + 1]) + lc.bias[c0 + 1], 0.0f);
+              __nv_bfloat162 hb = __floats2bfloat162_rn(v0, v1);
+              ow[i] = *reinterpret_cast<uint32_t*>(&hb);
               if (HEAD) {
-                lg = fmaf(__uint_as_float(ow[i] << 16), head_s[k * 8 + 2 * i], lg);
-                lg = fmaf(__uint_as_float(ow[i] & 0xffff0000u), head_s[k * 8 + 2 * i + 1], lg);
-                orw[k * 4 + i] = ow[i];
+                const float a0 = __uint_as_float(ow[i] << 16), a1 = __uint_as_float(ow[i] & 0xffff0000u);
+#pragma unroll
+                for (int h = 0; h < 6; ++h) hp[h] = fmaf(a0, ha.w[c0][h], hp[h]);
+#pragma unroll
+                for (int h = 0; h < 6; ++h) hp[h] = fmaf(a1, ha.w[c0 + 1][h], hp[h]);
               }
             }
-            if (!HEAD) orow[(size_t)k * plane_px] = make_uint4(ow[0], ow[1], ow[2], ow[3]);
+            if (!HEAD) orow[(size_t)kk * plane_px] = make_uint4(ow[0], ow[1], ow[2], ow[3]);
           }
-          if (HEAD) {
+        };
+        if (store) {
+          if (half == 0) post(std::integral_constant<int, 0>{});
+          else post(std::integral_constant<int, 1>{});
+        }
+        if (HEAD && out_valid) {
+          if (half == 1) {
+            *reinterpret_cast<float4*>(xch) = make_float4(hp[0], hp[1], hp[2], hp[3]);
+            *reinterpret_cast<float2*>(xch + 4) = make_float2(hp[4], hp[5]);
+          }
+          asm volatile("bar.sync %0, 64;" ::"r"(pair_bar) : "memory");
+          if (half == 0 && store) {
+            const float4 o03 = *reinterpret_cast<const float4*>(xch);
+            const float2 o45 = *reinterpret_cast<const float2*>(xch + 4);
+            const float lg = hp[0] + o03.x;
             const size_t q = ((size_t)run.b * geo.H + (row - d)) * geo.W + x;
             ha.logit[q] = lg;
-            if (lg > ha.lthr) {
-              // candidate: the other heads, each the same fmaf chain over the channels as
-              // head_post.cu, two heads per fma.rn.f32x2 (independent IEEE fp32 FMAs)
-              unsigned long long a12 = pack2f(headb_s[1], headb_s[2]), a34 = pack2f(headb_s[3], headb_s[4]),
-                                 a5 = pack2f(headb_s[5], 0.0f);
-              const bool six = ha.n_h == 6;
-#pragma unroll
-              for (int c2 = 0; c2 < C / 2; ++c2) {
-#pragma unroll
-                for (int half = 0; half < 2; ++half) {
-                  const float av = __uint_as_float(half ? (orw[c2] & 0xffff0000u) : (orw[c2] << 16));
-                  const unsigned long long aa = pack2f(av, av);
-                  const float* wq = headq_s + (2 * c2 + half) * 8;
-                  const ulonglong2 w14 = *reinterpret_cast<const ulonglong2*>(wq);
-                  a12 = ffma2(aa, w14.x, a12);
-                  a34 = ffma2(aa, w14.y, a34);
-                  if (six) a5 = ffma2(aa, *reinterpret_cast<const unsigned long long*>(wq + 4), a5);
-                }
-              }
+            if (lg > ha.lthr) {  // candidate record: heads 1 .. 5 (pre-activation; zero beyond n_h)
               float4* cq = reinterpret_cast<float4*>(ha.cand) + q * 2;
-              cq[0] = make_float4(__uint_as_float((uint32_t)a12), __uint_as_float((uint32_t)(a12 >> 32)),
-                                  __uint_as_float((uint32_t)a34), __uint_as_float((uint32_t)(a34 >> 32)));
-              cq[1] = make_float4(__uint_as_float((uint32_t)a5), 0.0f, 0.0f, 0.0f);
+              cq[0] = make_float4(hp[1] + o03.y, hp[2] + o03.z, hp[3] + o03.w, hp[4] + o45.x);
+              cq[1] = make_float4(hp[5] + o45.y, 0.0f, 0.0f, 0.0f);
             }
           }
+          asm volatile("bar.sync %0, 64;" ::"r"(pair_bar) : "memory");  // xch may be rewritten
         }
         if (kEarly) {
           if (in_valid) {
             const uint4* rp = reinterpret_cast<const uint4*>(smem + (stage_addr(ln, st) - sbase) +
                                                              (uint32_t)(d + px) * 16u);
 #pragma unroll
-            for (int k = 0; k < C / 8; ++k) res[k] = rp[(size_t)k * (plane / 16u)];
+            for (int kk = 0; kk < KH; ++kk) res[kk] = rp[(size_t)(k0 + kk) * (plane / 16u)];
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             __syncwarp();
             if (lane == 0) mbar_arrive(empty_bar(ln, st));
@@ -846,7 +896,7 @@ __global__ void __launch_bounds__(kThreads, 1)
   // ---- teardown
   tc_fence_before();
   __syncthreads();
-  if (warp == 2) {
+  if (role == 2) {
     tc_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(kTmemCols) : "memory");
   }
@@ -862,7 +912,7 @@ uint16_t bf16_bits(float f) {
 }
 
 template <int C, bool HEAD, bool STEM>
-cudaError_t launch_chs(const void* in, void* out, Geo geo, const void* wpack, const float* bias, int nstage,
+cudaError_t launch_chs(const void* in, void* out, Geo geo, const void* wpack, const LayerConst& lc, int nstage,
                        int grid, size_t smem, const HeadArgs& ha, const StemArgs& sa, cudaStream_t st) {
   static bool attr_done[kMaxDevices] = {};  // the attribute is per device
   int dev = 0;
@@ -885,25 +935,25 @@ cudaError_t launch_chs(const void* in, void* out, Geo geo, const void* wpack, co
   cfg.attrs = attr;
   cfg.numAttrs = 1;
   return cudaLaunchKernelEx(&cfg, conv_umma_kernel<C, HEAD, STEM>, (const __nv_bfloat16*)in,
-                            (__nv_bfloat16*)out, geo, (const uint8_t*)wpack, bias, nstage, ha, sa);
+                            (__nv_bfloat16*)out, geo, (const uint8_t*)wpack, nstage, lc, ha, sa);
 }
 template <int C>
-cudaError_t launch_c(const void* in, void* out, Geo geo, const void* wpack, const float* bias, int nstage,
+cudaError_t launch_c(const void* in, void* out, Geo geo, const void* wpack, const LayerConst& lc, int nstage,
                      int grid, size_t smem, const HeadArgs* ha, const StemArgs* sa, cudaStream_t st) {
-  const HeadArgs h0{};
-  const StemArgs s0{};
-  if (ha && sa) return launch_chs<C, true, true>(in, out, geo, wpack, bias, nstage, grid, smem, *ha, *sa, st);
-  if (ha) return launch_chs<C, true, false>(in, out, geo, wpack, bias, nstage, grid, smem, *ha, s0, st);
-  if (sa) return launch_chs<C, false, true>(in, out, geo, wpack, bias, nstage, grid, smem, h0, *sa, st);
-  return launch_chs<C, false, false>(in, out, geo, wpack, bias, nstage, grid, smem, h0, s0, st);
+  static const HeadArgs h0{};
+  static const StemArgs s0{};
+  if (ha && sa) return launch_chs<C, true, true>(in, out, geo, wpack, lc, nstage, grid, smem, *ha, *sa, st);
+  if (ha) return launch_chs<C, true, false>(in, out, geo, wpack, lc, nstage, grid, smem, *ha, s0, st);
+  if (sa) return launch_chs<C, false, true>(in, out, geo, wpack, lc, nstage, grid, smem, h0, *sa, st);
+  return launch_chs<C, false, false>(in, out, geo, wpack, lc, nstage, grid, smem, h0, s0, st);
 }
 
 // stages: as many as fit next to the resident weights (<= kMaxStages; >= 2 for any overlap of
 // load and MMA; the STEM variant computes two steps ahead and needs >= 3)
-int pick_stages(int C, int dil, bool stem) {
+int pick_stages(int C, int dil, bool stem, bool head) {
   int nstage = kMaxStages;
   const int min_stage = stem ? 3 : 2;
-  while (nstage >= min_stage && smem_layout(C, dil, nstage, stem).total + 1024 > 227u * 1024u) --nstage;
+  while (nstage >= min_stage && smem_layout(C, dil, nstage, stem, head).total + 1024 > 227u * 1024u) --nstage;
   return nstage >= min_stage ? nstage : 0;
 }
 
@@ -929,11 +979,11 @@ void umma_pack_weights_host(int C, const float* w /*[C][C][3][3]*/, void* dst) {
 }
 
 bool conv_umma_supports(int C, int dil, bool stem) {
-  return C >= 16 && C <= 64 && C % 16 == 0 && dil >= 1 && dil <= kMaxDilation && pick_stages(C, dil, stem) > 0;
+  return C >= 16 && C <= 64 && C % 16 == 0 && dil >= 1 && dil <= kMaxDilation && pick_stages(C, dil, stem, true) > 0;
 }
 
 cudaError_t launch_conv_umma(const void* in, void* out, ActShape s, int dil, const void* wpack,
-                             const float* bias, const HeadArgs* head, const StemArgs* stem, int n_sm,
+                             const LayerConst& lc, const HeadArgs* head, const StemArgs* stem, int n_sm,
                              cudaStream_t st, char* err, size_t errlen) {
   if (dil < 1 || dil > kMaxDilation || s.C % 16 || s.C < 16 || s.C > 64) {
     snprintf(err, errlen, "unsupported channels / dilation");
@@ -948,21 +998,21 @@ cudaError_t launch_conv_umma(const void* in, void* out, ActShape s, int dil, con
   geo.nseg = (s.W + kTileM - 1) / kTileM;
   geo.Lmax = (s.H + dil - 1) / dil;
   geo.total = (long long)s.B * geo.nseg * dil * geo.Lmax;
-  const int nstage = pick_stages(s.C, dil, stem != nullptr);
+  const int nstage = pick_stages(s.C, dil, stem != nullptr, head != nullptr);
   if (nstage == 0) {
     snprintf(err, errlen, "shared memory budget exceeded");
     return cudaErrorInvalidValue;
   }
-  const SmemLayout L = smem_layout(s.C, dil, nstage, stem != nullptr);
+  const SmemLayout L = smem_layout(s.C, dil, nstage, stem != nullptr, head != nullptr);
   // at least ~12 row-tiles per lane, at most one CTA per SM
   long long want = (geo.total + 23) / 24;
   int grid = (int)(want < 1 ? 1 : (want > n_sm ? n_sm : want));
   const size_t smem = L.total + 1024;
   switch (s.C) {
-    case 16: return launch_c<16>(in, out, geo, wpack, bias, nstage, grid, smem, head, stem, st);
-    case 32: return launch_c<32>(in, out, geo, wpack, bias, nstage, grid, smem, head, stem, st);
-    case 48: return launch_c<48>(in, out, geo, wpack, bias, nstage, grid, smem, head, stem, st);
-    case 64: return launch_c<64>(in, out, geo, wpack, bias, nstage, grid, smem, head, stem, st);
+    case 16: return launch_c<16>(in, out, geo, wpack, lc, nstage, grid, smem, head, stem, st);
+    case 32: return launch_c<32>(in, out, geo, wpack, lc, nstage, grid, smem, head, stem, st);
+    case 48: return launch_c<48>(in, out, geo, wpack, lc, nstage, grid, smem, head, stem, st);
+    case 64: return launch_c<64>(in, out, geo, wpack, lc, nstage, grid, smem, head, stem, st);
   }
   return cudaErrorInvalidValue;
 }

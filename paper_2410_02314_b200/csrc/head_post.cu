@@ -22,8 +22,10 @@ constexpr int MAX_CAND = (TW / 2) * (TH / 2);  // no two detections are 8-adjace
 __device__ inline float sigmoid_f(float v) { return 1.0f / (1.0f + expf(-v)); }
 __device__ inline float softplus_f(float v) { return fmaxf(v, 0.0f) + log1pf(expf(-fabsf(v))); }
 
-// One head of one pixel from the activations: fixed summation order (chunk, channel), so
-// every kernel in this file produces bit-identical values for the same pixel.
+// One head of one pixel from the activations.  Fixed summation order, shared with the HEAD
+// epilogue of conv_umma.cu (whose two warps per pixel each own one channel half): two fmaf
+// chains, channels [0, C/2) starting from the bias and [C/2, C) starting from zero, added at
+// the end - so every kernel produces bit-identical values for the same pixel.
 template <typename T, int C>
 struct ActSource {
   const T* act;
@@ -31,16 +33,19 @@ struct ActSource {
   const float* wh;  // shared memory [n_h][C]
   const float* bh;  // shared memory [n_h]
   __device__ inline float head(int h, int b, int y, int x) const {
-    float acc = bh[h];
+    float acc0 = bh[h], acc1 = 0.0f;
     const float* w = wh + h * C;
 #pragma unroll
     for (int k = 0; k < C / 8; ++k) {
       float v[8];
       Chunk<T>::load(act, s.chunk_index(b, k, y, x), v);
 #pragma unroll
-      for (int c = 0; c < 8; ++c) acc = fmaf(v[c], w[k * 8 + c], acc);
+      for (int c = 0; c < 8; ++c) {
+        if (k < C / 16) acc0 = fmaf(v[c], w[k * 8 + c], acc0);
+        else acc1 = fmaf(v[c], w[k * 8 + c], acc1);
+      }
     }
-    return acc;
+    return acc0 + acc1;
   }
 };
 

@@ -103,31 +103,38 @@ size_t umma_packed_weight_bytes(int C);
 // w_oihw [C][C][3][3] fp32 -> the kernel's shared-memory image (bf16, RNE), host side.
 void umma_pack_weights_host(int C, const float* w_oihw, void* dst);
 // STEM variant (first layer, K1 folded in): a_0 is computed in the kernel from the frames.
+// The per-layer constants travel as kernel parameters: parameters live in constant memory,
+// so a weight with a compile-time index is a free operand of the FMA that uses it (no
+// shared-memory or register traffic - the shared-memory pipe belongs to the tensor core's
+// operand fetch, profiles/).
+struct LayerConst {
+  float bias[64];
+};
 struct StemArgs {
   const uint16_t* frames;  // device; frame f of the call at frames + (f - frame_base) Hf Wf
   int frame_base;
   ViewSet vs;
   NormParams np;
-  const float* w;  // [9][C]
-  const float* b;  // [C]
   int relu;
+  float w[9][64];  // [tap ky*3+kx][channel]
+  float b[64];
 };
 
 // HEAD (K3 folded in): what the last layer's epilogue writes instead of the activation map.
 struct HeadArgs {
-  const float* w;   // [n_h][C]
-  const float* b;   // [n_h]
   int n_h;
   float lthr;       // logit(threshold)
   float* logit;     // [B][H][W] detection logit of every pixel
   float* cand;      // [B][H][W][8]: heads 1 .. n_h-1 (pre-activation) of pixels with logit > lthr
+  float w[64][8];   // [channel][head], zero beyond n_h
+  float b[8];
 };
 
 bool conv_umma_supports(int C, int dil, bool stem);
 // head != nullptr: last layer, HEAD variant (`out` is not written).  stem != nullptr: first
 // layer, STEM variant (`in` is not read).
 cudaError_t launch_conv_umma(const void* in, void* out, ActShape s, int dil, const void* wpack,
-                             const float* bias, const HeadArgs* head, const StemArgs* stem, int n_sm,
+                             const LayerConst& lc, const HeadArgs* head, const StemArgs* stem, int n_sm,
                              cudaStream_t st, char* err, size_t errlen);
 
 // K3: 1x1 heads + threshold + 3x3 NMS + decode + warp-aggregated compaction.

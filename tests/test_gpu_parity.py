@@ -445,8 +445,9 @@ def test_production_post_tie_rule_on_quantised_logits():
                                                (16, 5, 9, 9, (8, 4, 1), 0), (48, 5, 1, 1, (1, 8), 0),
                                                (48, 5, 150, 173, (1, 2, 4), 64)])
 def test_fused_stem_and_heads_equal_unfused_bit_exact(C, nh, H, W, dil, tile):
-    """SMLM_FUSE_AUTO (K1 inside the first layer's kernel, K3's heads inside the last layer's
-    epilogue) against SMLM_FUSE_NONE (stem_kernel, plain layers, heads from the stored map):
+    """SMLM_FUSE_ALL (K1 inside the first layer's kernel, K3's heads inside the last layer's
+    epilogue) and SMLM_FUSE_AUTO (heads only) against SMLM_FUSE_NONE (stem_kernel, plain layers,
+    heads from the stored map):
     same arithmetic and rounding points, so trunk levels and emitter records are identical
     bit by bit - with per-pixel camera maps, ragged sizes, H < d, 1x1 frames and tiles."""
     spec = NetSpec(C, dil, nh, "bf16")
@@ -461,10 +462,11 @@ def test_fused_stem_and_heads_equal_unfused_bit_exact(C, nh, H, W, dil, tile):
     kw = dict(conv_impl=P.CONV_TCGEN05)
     if not tile:
         ma, ta = G.gpu_forward_maps(spec, w, frames, ck, dump_trunk=True, fusion=P.FUSE_NONE, **kw)
-        mb, tb = G.gpu_forward_maps(spec, w, frames, ck, dump_trunk=True, fusion=P.FUSE_AUTO, **kw)
+        mb, tb = G.gpu_forward_maps(spec, w, frames, ck, dump_trunk=True, fusion=P.FUSE_ALL, **kw)
         assert np.array_equal(ta, tb) and np.array_equal(ma, mb)
     for thr in (0.5, 0.0):
         a = G.gpu_localize(spec, w, frames, ck, thr, fusion=P.FUSE_NONE, tile=tile, **kw)
-        b = G.gpu_localize(spec, w, frames, ck, thr, fusion=P.FUSE_AUTO, tile=tile, **kw)
-        assert len(a) == len(b) and (len(a) > 0 or H * W < 100)
-        assert a.tobytes() == b.tobytes(), thr
+        assert len(a) > 0 or H * W < 100
+        for fusion in (P.FUSE_AUTO, P.FUSE_ALL):
+            b = G.gpu_localize(spec, w, frames, ck, thr, fusion=fusion, tile=tile, **kw)
+            assert len(a) == len(b) and a.tobytes() == b.tobytes(), (thr, fusion)
