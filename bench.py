@@ -133,7 +133,51 @@ def run_reference(args, cfg):
     return 0
 
 
-def main():
+def _rank_entry(rank, world, port, argv):
+    """One rank of a self-spawned run: the same environment torchrun would set."""
+    os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), LOCAL_WORLD_SIZE=str(world),
+                      MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    rc = main(argv)
+    if rc:
+        raise SystemExit(rc)
+
+
+def spawn_ranks(args, argv):
+    """python bench.py --gpus N without torchrun: start N ranks, one per GPU (multi-GPU =
+    independent replicas: the only communication is the barrier and the reduction of
+    two scalars)."""
+    import socket
+    import torch
+    import torch.multiprocessing as mp
+    if not args.selftest_spawn and torch.cuda.device_count() < args.gpus:
+        raise SystemExit(f"bench.py --gpus {args.gpus}: only {torch.cuda.device_count()} CUDA device(s) visible")
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    mp.spawn(_rank_entry, args=(args.gpus, port, argv), nprocs=args.gpus, join=True)
+    return 0
+
+
+def selftest_spawn(args, cfg):
+    """Host logic of the N > 1 path on CPU (gloo): sharding + whole-job throughput."""
+    import torch.distributed as dist
+    from paper_2410_02314_b200.replicas import job_throughput, shard_frames
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    if world > 1:
+        dist.init_process_group("gloo")
+    n = args.frames or cfg.frames.n_frames
+    lo, hi = shard_frames(n, rank, world) if args.scaling == "strong" else (0, n)
+    ms = 10.0 + rank                                   # synthetic device time: the slowest rank decides
+    value, ms_max = job_throughput(hi - lo, ms, dist if world > 1 else None, "cpu")
+    if rank == 0:
+        print(json.dumps({"selftest": True, "n_gpus": world, "scaling": args.scaling, "value": value,
+                          "ms_max": ms_max, "frames_rank0": hi - lo}), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
@@ -145,11 +189,22 @@ def main():
     ap.add_argument("--micro-batch", type=int, default=0)
     ap.add_argument("--fusion", default="auto", choices=["auto", "none", "all"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    args = ap.parse_args()
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = every rank localises the config's full stack (replicas); "
+                         "strong = the stack is sharded by frame range (shard_frames)")
+    ap.add_argument("--disk", default="", help="also time smlm_localize_ring from a frame file written to this directory")
+    ap.add_argument("--selftest-spawn", action="store_true",
+                    help="CPU only: exercise the --gpus N spawn path, the frame sharding and the max-over-ranks "
+                         "reduction over gloo with synthetic per-rank timings")
+    args = ap.parse_args(argv)
     cfg = get_config(args.config)
     if args.impl == "reference":
         return run_reference(args, cfg)
     args.warmup = max(args.warmup, 3)
+    if "WORLD_SIZE" not in os.environ and args.gpus > 1:
+        return spawn_ranks(args, sys.argv[1:] if argv is None else list(argv))
+    if args.selftest_spawn:
+        return selftest_spawn(args, cfg)
 
     import torch
     import paper_2410_02314_b200 as P
@@ -162,10 +217,15 @@ def main():
     torch.cuda.set_device(local)
     dist = None
     if world > 1:
+        os.environ.setdefault("NCCL_DEBUG", "INFO")     # the communicator line (nranks) goes to stderr
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
 
     n_frames = args.frames or cfg.frames.n_frames
+    if world > 1 and args.scaling == "strong":          # frame-range sharding, no exchange step
+        from paper_2410_02314_b200.replicas import shard_frames
+        lo, hi = shard_frames(n_frames, rank, world)
+        n_frames = hi - lo
     fs, frames = workload(cfg, n_frames)
     weights = make_weights(cfg)
     H, W = frames.shape[1:]
@@ -223,6 +283,29 @@ def main():
     # launching stream (the events serialise a little, so `value` is not taken from this pass)
     ms_rf, _, _, kt = timed(frames_dev, out_dev, args.steps, kernel_timing=True)
     conv_ms, conv_n = kt[P.KERNEL_CONV]
+    disk = None
+    if args.disk:
+        # the paper's storage -> GPU experiment: reader threads fill the pinned ring
+        # from a raw frame file while earlier chunks are localised (smlm_localize_ring)
+        os.makedirs(args.disk, exist_ok=True)
+        path = os.path.join(args.disk, f"bench_frames_rank{rank}.u16")
+        frames.tofile(path)
+        chunk, slots, threads = 256, 4, 4
+        with P.Ring(path, n_frames, H, W, chunk, n_slots=slots, n_threads=threads) as ring:
+            loc.localize_ring(ring, cam, cfg.threshold, out_host, cap, stream=stream)    # warm-up (page cache)
+            torch.cuda.synchronize()
+            barrier()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(args.steps):
+                loc.localize_ring(ring, cam, cfg.threshold, out_host, cap, stream=stream)
+            e1.record(stream)
+            barrier()
+            ms_disk = e0.elapsed_time(e1)
+        os.remove(path)
+        disk = {"value": n_frames * args.steps / (ms_disk * 1e-3), "unit": UNIT, "ms_per_step": ms_disk / args.steps,
+                "file_bytes": int(frames.nbytes), "chunk_frames": chunk, "ring_slots": slots, "reader_threads": threads,
+                "note": "file re-read from the OS page cache after the warm-up pass"}
     sampler.stop_flag.set()
     sampler.join(timeout=2)
 
@@ -290,7 +373,7 @@ def main():
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None,
+        "scaling": args.scaling, "vs_baseline": None,
         "dtype": "bf16" if cfg.net.precision == "bf16" else "f32", "data": "synthetic",
         "config": {"workload": cfg.name, "frames_per_step": n_frames, "H": H, "W": W, "channels": C,
                    "layers": L, "head_channels": cfg.net.head_channels, "tile": cfg.tile,
@@ -307,6 +390,7 @@ def main():
         "roofline": roofline,
         "io_kernels": io_kernels,
         "cpu_baseline": cpu,
+        "from_disk": disk,
         "tensor_frac_whole_step": (cfg.net.flop_per_px() * H * W * n_frames * args.steps / (ms_max * 1e-3) / 1e12)
                                   / float(peaks["bf16_tflops"]),
     }

@@ -155,6 +155,41 @@ smlm_status smlm_localize(smlm_ctx* ctx, const uint16_t* frames_u16, int64_t n_f
  * found more emitters than the capacity, SMLM_ERR_CUDA if an asynchronous error is pending. */
 smlm_status smlm_check(smlm_ctx* ctx);
 
+/*
+ * The preload ring fed from storage ("multiple processes handle data loading and network
+ * inference simultaneously"; "images are loaded in advance into specified memory
+ * locations"; the NVMe -> GPU experiment of P:196-198).
+ *   smlm_ring_open: `path` is a raw little-endian uint16 file holding [n_frames][H][W] at
+ *     `byte_offset`.  `n_threads` reader threads (pread) fill a ring of `n_slots` >= 2 chunks of
+ *     `chunk_frames` frames in PINNED host memory, in file order, as slots become free.
+ *     flags: SMLM_RING_PAGEABLE allocates the ring with malloc (host-logic tests on a machine
+ *     without a GPU; smlm_localize_ring refuses such a ring).
+ *     Errors: INVALID_ARG (bad sizes, file missing or too short), CUDA (pinned allocation), OOM.
+ *   smlm_localize_ring: smlm_localize over the whole file.  Chunk k is localized from ring slot
+ *     k % n_slots (H2D on the ctx's copy stream) while the readers fill the following slots;
+ *     a slot is handed back to the readers when its last H2D copy has finished.  `frame` of
+ *     the records is the index in the file; one emitter list, same arguments and error
+ *     behaviour as smlm_localize.  Enqueues GPU work asynchronously but BLOCKS the calling
+ *     host thread while it waits for the disk.  The ring is rewound first, so it can be used
+ *     for several passes.
+ *   smlm_ring_acquire / smlm_ring_release: the consumer side by hand (tests, custom loops):
+ *     acquire blocks until the next chunk is in memory (*n_frames = 0 at the end of the file),
+ *     release(first_frame) lets the readers refill its slot.
+ *   smlm_ring_close: stops the readers, frees the ring.  NULL is allowed.
+ */
+typedef struct smlm_ring smlm_ring;
+enum { SMLM_RING_PAGEABLE = 1 };
+smlm_status smlm_ring_open(const char* path, int64_t byte_offset, int64_t n_frames, int32_t H, int32_t W,
+                           int32_t chunk_frames, int32_t n_slots, int32_t n_threads, int32_t flags,
+                           smlm_ring** out_ring);
+smlm_status smlm_localize_ring(smlm_ctx* ctx, smlm_ring* ring, const smlm_camera_params* camera,
+                               float threshold, smlm_emitter* out_emitters, int64_t* out_count,
+                               void* cuda_stream);
+smlm_status smlm_ring_acquire(smlm_ring* ring, const uint16_t** frames, int64_t* n_frames,
+                              int64_t* first_frame);
+smlm_status smlm_ring_release(smlm_ring* ring, int64_t first_frame);
+void smlm_ring_close(smlm_ring* ring);
+
 /* Synchronise, free everything the ctx owns.  NULL is allowed. */
 void smlm_destroy(smlm_ctx* ctx);
 

@@ -24,7 +24,10 @@ KERNEL_STEM, KERNEL_CONV, KERNEL_POST = 0, 1, 2
 
 EXPORTS = ["smlm_create", "smlm_localize", "smlm_check", "smlm_destroy", "smlm_last_error",
            "smlm_launch_count", "smlm_kernel_timing", "smlm_kernel_time_ms",
-           "smlm_debug_forward_maps", "smlm_debug_postprocess"]
+           "smlm_debug_forward_maps", "smlm_debug_postprocess",
+           "smlm_ring_open", "smlm_localize_ring", "smlm_ring_acquire", "smlm_ring_release",
+           "smlm_ring_close"]
+RING_PAGEABLE = 1
 
 
 class NetDesc(C.Structure):
@@ -86,6 +89,16 @@ def lib():
         L.smlm_debug_postprocess.restype = C.c_int
         L.smlm_debug_postprocess.argtypes = [vp, vp, i64, i32, i32, C.POINTER(CameraParams), f32,
                                              vp, C.POINTER(i64), vp]
+        L.smlm_ring_open.restype = C.c_int
+        L.smlm_ring_open.argtypes = [C.c_char_p, i64, i64, i32, i32, i32, i32, i32, i32, C.POINTER(vp)]
+        L.smlm_localize_ring.restype = C.c_int
+        L.smlm_localize_ring.argtypes = [vp, vp, C.POINTER(CameraParams), f32, vp, C.POINTER(i64), vp]
+        L.smlm_ring_acquire.restype = C.c_int
+        L.smlm_ring_acquire.argtypes = [vp, C.POINTER(vp), C.POINTER(i64), C.POINTER(i64)]
+        L.smlm_ring_release.restype = C.c_int
+        L.smlm_ring_release.argtypes = [vp, i64]
+        L.smlm_ring_close.restype = None
+        L.smlm_ring_close.argtypes = [vp]
         _LIB = L
     return _LIB
 
@@ -189,6 +202,17 @@ class Localizer:
         self._check(st)
         return count
 
+    def localize_ring(self, ring: "Ring", cam: CameraParams, threshold: float, out_emitters,
+                      capacity: int, stream=None, count: Optional[C.c_int64] = None) -> C.c_int64:
+        """smlm_localize_ring: the whole frame file behind `ring`, chunk by chunk."""
+        if count is None:
+            count = C.c_int64()
+        count.value = int(capacity)
+        st = lib().smlm_localize_ring(self._h, ring._h, C.byref(cam), float(threshold),
+                                      _ptr(out_emitters), C.byref(count), _stream_handle(stream))
+        self._check(st)
+        return count
+
     def check(self) -> int:
         return lib().smlm_check(self._h)
 
@@ -237,6 +261,54 @@ class Localizer:
 
     def __exit__(self, *a):
         self.close()
+
+
+class Ring:
+    """smlm_ring_open / smlm_ring_close: reader threads + pinned host ring over a raw uint16
+    frame file [n_frames][H][W] (the paper's preloading)."""
+
+    def __init__(self, path: str, n_frames: int, H: int, W: int, chunk_frames: int, n_slots: int = 3,
+                 n_threads: int = 2, byte_offset: int = 0, pageable: bool = False):
+        self._h = C.c_void_p()
+        self.n_frames, self.H, self.W, self.chunk_frames = int(n_frames), int(H), int(W), int(chunk_frames)
+        st = lib().smlm_ring_open(os.fsencode(path), int(byte_offset), int(n_frames), int(H), int(W),
+                                  int(chunk_frames), int(n_slots), int(n_threads),
+                                  RING_PAGEABLE if pageable else 0, C.byref(self._h))
+        if st != OK:
+            raise SmlmError(st, f"smlm_ring_open({path!r})")
+
+    def acquire(self):
+        """-> (numpy view [n][H][W] of the next chunk, first_frame) or (None, None) at the end."""
+        p, n, first = C.c_void_p(), C.c_int64(), C.c_int64()
+        st = lib().smlm_ring_acquire(self._h, C.byref(p), C.byref(n), C.byref(first))
+        if st != OK:
+            raise SmlmError(st, "smlm_ring_acquire")
+        if n.value == 0:
+            return None, None
+        arr = np.ctypeslib.as_array(C.cast(p, C.POINTER(C.c_uint16)), shape=(n.value, self.H, self.W))
+        return arr, first.value
+
+    def release(self, first_frame: int):
+        st = lib().smlm_ring_release(self._h, int(first_frame))
+        if st != OK:
+            raise SmlmError(st, "smlm_ring_release")
+
+    def close(self):
+        if self._h:
+            lib().smlm_ring_close(self._h)
+            self._h = C.c_void_p()
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 def emitters_to_numpy(buf, count: int) -> np.ndarray:

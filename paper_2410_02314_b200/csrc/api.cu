@@ -12,6 +12,7 @@
 #include <string>
 #include <vector>
 
+#include "ring.cuh"
 #include "smlm_internal.cuh"
 
 using namespace smlm;
@@ -533,75 +534,110 @@ smlm_status smlm_check(smlm_ctx* c) {
   return SMLM_OK;
 }
 
-smlm_status smlm_localize(smlm_ctx* c, const uint16_t* frames, int64_t n, int32_t H, int32_t W,
-                          const smlm_camera_params* cam, float threshold, smlm_emitter* out,
-                          int64_t* out_count, void* cuda_stream) {
-  if (!c) return SMLM_ERR_INVALID_ARG;
+}  // extern "C"
+
+namespace {
+
+// One smlm_localize call, cut into begin / frames / end so that the frames may arrive in
+// pieces (smlm_localize_ring feeds one ring chunk at a time; frame indices stay global).
+struct Call {
+  smlm_ctx* c = nullptr;
+  cudaStream_t st = nullptr;
+  int H = 0, W = 0, C = 0;
+  int64_t n_total = 0;     // frames of the whole call
+  NormParams np{};
+  HeadParams hp{};
+  bool tiled = false;
+  int tile = 0, halo = 0, mb = 0, F = 1;
+  std::vector<Range> ycls, xcls;
+  smlm_emitter* out = nullptr;   // caller's list
+  smlm_emitter* list = nullptr;  // where K3 appends (== out, or the ctx's device list)
+  unsigned long long capacity = 0;
+  bool host_out = false;
+  int wbf = 256;
+  int64_t n_flush = 0, chunk = 0;
+};
+
+smlm_status call_flush(Call& k) {
+  smlm_ctx* c = k.c;
+  unsigned long long* counter = c->counters;
+  unsigned long long* snap_ring = c->counters + 2;
+  const int64_t i = k.n_flush;
+  // the word snap[i % R] was read by flushes i - R (upper end) and i - R + 1 (lower end)
+  if (i >= kSnapRing) CK(c, cudaStreamWaitEvent(k.st, c->ev_wb[(i + 1) % kSnapRing], 0));
+  // records below the snapshot are complete: every K3 that wrote them precedes it on `st`
+  CK(c, launch_snapshot(counter, k.capacity, snap_ring + i % kSnapRing, k.st));
+  CK(c, cudaEventRecord(c->ev_batch, k.st));
+  CK(c, cudaStreamWaitEvent(c->wb_stream, c->ev_batch, 0));
+  const unsigned long long* lo = i == 0 ? c->counters + 1 : snap_ring + (i - 1) % kSnapRing;
+  CK(c, launch_flush_emitters(k.list, k.out, lo, snap_ring + i % kSnapRing, c->wb_stream));
+  CK(c, cudaEventRecord(c->ev_wb[i % kSnapRing], c->wb_stream));
+  c->launches += 2;
+  ++k.n_flush;
+  return SMLM_OK;
+}
+
+smlm_status call_begin(Call& k, smlm_ctx* c, int64_t n, int32_t H, int32_t W, const smlm_camera_params* cam,
+                       float threshold, smlm_emitter* out, int64_t* out_count, bool host_frames,
+                       int64_t max_piece, cudaStream_t st) {
   if (!cam || !out_count) return fail(c, SMLM_ERR_INVALID_ARG, "NULL camera / out_count");
   if (n < 0 || H < 1 || W < 1 || (int64_t)H * W > (int64_t)1 << 30 || n > INT32_MAX)
     return fail(c, SMLM_ERR_INVALID_ARG, "bad n_frames / H / W");
   if (*out_count < 0) return fail(c, SMLM_ERR_INVALID_ARG, "negative capacity");
   if (!(threshold == threshold)) return fail(c, SMLM_ERR_INVALID_ARG, "threshold is NaN");
   if (!(cam->pixel_size_nm > 0.0f)) return fail(c, SMLM_ERR_INVALID_ARG, "pixel_size_nm must be > 0");
-  const unsigned long long capacity = (unsigned long long)*out_count;
-  if (capacity > 0 && !out) return fail(c, SMLM_ERR_INVALID_ARG, "NULL out_emitters with capacity > 0");
-  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-
-  PtrKind fk = PTR_DEVICE;
-  if (n > 0) {
-    if (!frames) return fail(c, SMLM_ERR_INVALID_ARG, "NULL frames");
-    fk = classify(frames);
-    if (fk == PTR_OTHER)
-      return fail(c, SMLM_ERR_INVALID_ARG,
-                  "frames_u16 must be pinned host memory (the preload ring) or device memory");
-  }
+  k.c = c;
+  k.st = st;
+  k.H = H;
+  k.W = W;
+  k.C = c->d.channels;
+  k.n_total = n;
+  k.capacity = (unsigned long long)*out_count;
+  k.out = out;
+  if (k.capacity > 0 && !out) return fail(c, SMLM_ERR_INVALID_ARG, "NULL out_emitters with capacity > 0");
   PtrKind ok = PTR_DEVICE;
-  if (capacity > 0) {
+  if (k.capacity > 0) {
     ok = classify(out);
     if (ok == PTR_OTHER)
       return fail(c, SMLM_ERR_INVALID_ARG, "out_emitters must be device or pinned host memory");
   }
-
-  NormParams np;
-  smlm_status r = setup_camera(c, cam, H, W, st, &np);
+  smlm_status r = setup_camera(c, cam, H, W, st, &k.np);
   if (r != SMLM_OK) return r;
-  const HeadParams hp = head_params(c, cam, threshold);
-  const int C = c->d.channels;
+  k.hp = head_params(c, cam, threshold);
 
   // ---- geometry: launch sets (all views of a set share one window size)
-  const int tile = c->d.tile;
-  const bool tiled = tile > 0 && (tile < H || tile < W);
-  const int halo = c->radius + 1;  // maps need `radius`; the 3x3 test reads one more pixel
-  std::vector<Range> ycls, xcls;
-  if (tiled) {
-    ycls = tile_classes(H, tile, halo);
-    xcls = tile_classes(W, tile, halo);
+  k.tile = c->d.tile;
+  k.tiled = k.tile > 0 && (k.tile < H || k.tile < W);
+  k.halo = c->radius + 1;  // maps need `radius`; the 3x3 test reads one more pixel
+  if (k.tiled) {
+    k.ycls = tile_classes(H, k.tile, k.halo);
+    k.xcls = tile_classes(W, k.tile, k.halo);
   } else {
-    ycls.push_back({0, 1, H});
-    xcls.push_back({0, 1, W});
+    k.ycls.push_back({0, 1, H});
+    k.xcls.push_back({0, 1, W});
   }
   int maxHw = 0, maxWw = 0;
-  for (auto& a : ycls) maxHw = std::max(maxHw, a.ext);
-  for (auto& a : xcls) maxWw = std::max(maxWw, a.ext);
-  const int mb = auto_micro_batch(c, maxHw, maxWw);   // views per launch
+  for (auto& a : k.ycls) maxHw = std::max(maxHw, a.ext);
+  for (auto& a : k.xcls) maxWw = std::max(maxWw, a.ext);
+  k.mb = auto_micro_batch(c, maxHw, maxWw);  // views per launch
   // frames per chunk: whole frames -> one view each; tiles -> as many frames as keep the
   // largest launch set (all tiles of one window class, times the frames) within mb views
   int tiles_per_frame = 0;
-  for (auto& a : ycls)
-    for (auto& b : xcls) tiles_per_frame = std::max(tiles_per_frame, a.n * b.n);
-  const int F = (int)std::max<int64_t>(1, std::min<int64_t>(tiled ? mb / std::max(tiles_per_frame, 1) : mb,
-                                                           std::max<int64_t>(n, 1)));
+  for (auto& a : k.ycls)
+    for (auto& b : k.xcls) tiles_per_frame = std::max(tiles_per_frame, a.n * b.n);
+  const int64_t piece = std::max<int64_t>(1, std::min<int64_t>(std::max<int64_t>(n, 1), max_piece));
+  k.F = (int)std::max<int64_t>(1, std::min<int64_t>(k.tiled ? k.mb / std::max(tiles_per_frame, 1) : k.mb, piece));
   size_t need = 0;
-  for (auto& a : ycls)
-    for (auto& b : xcls) {
-      int nv = tiled ? std::max(1, std::min(mb, F * a.n * b.n)) : F;
-      need = std::max(need, (size_t)nv * a.ext * b.ext * C * elt_size(c));
+  for (auto& a : k.ycls)
+    for (auto& b : k.xcls) {
+      int nv = k.tiled ? std::max(1, std::min(k.mb, k.F * a.n * b.n)) : k.F;
+      need = std::max(need, (size_t)nv * a.ext * b.ext * k.C * elt_size(c));
     }
   if ((r = ensure_act(c, need)) != SMLM_OK) return r;
 
   const size_t frame_elems = (size_t)H * W;
-  if (fk == PTR_HOST_PINNED && n > 0) {
-    size_t se = (size_t)std::min<int64_t>(F, n) * frame_elems;
+  if (host_frames && n > 0) {
+    size_t se = (size_t)k.F * frame_elems;
     if (se > c->slot_elems) {
       CK(c, cudaDeviceSynchronize());  // a previous call may still read the old slots
       if (c->slots) cudaFree(c->slots);
@@ -612,60 +648,52 @@ smlm_status smlm_localize(smlm_ctx* c, const uint16_t* frames, int64_t n, int32_
       for (int i = 0; i < kSlots; ++i) c->slot_used[i] = false;
     }
   }
-  smlm_emitter* list = out;
-  if (ok == PTR_HOST_PINNED && capacity > 0) {
-    if (capacity > c->em_cap) {
+  k.list = out;
+  if (ok == PTR_HOST_PINNED && k.capacity > 0) {
+    if (k.capacity > c->em_cap) {
       CK(c, cudaDeviceSynchronize());
       if (c->em_dev) cudaFree(c->em_dev);
       c->em_dev = nullptr;
       c->em_cap = 0;
-      CK(c, cudaMalloc(&c->em_dev, capacity * sizeof(smlm_emitter)));
-      c->em_cap = capacity;
+      CK(c, cudaMalloc(&c->em_dev, k.capacity * sizeof(smlm_emitter)));
+      c->em_cap = k.capacity;
     }
-    list = c->em_dev;
+    k.list = c->em_dev;
   }
-  unsigned long long* counter = c->counters;
-  unsigned long long* snap_ring = c->counters + 2;
   CK(c, cudaMemsetAsync(c->counters, 0, kCounterWords * sizeof(unsigned long long), st));
-  c->last_capacity = capacity;
-
-  if (fk == PTR_HOST_PINNED) {
+  c->last_capacity = k.capacity;
+  if (host_frames) {
     CK(c, cudaEventRecord(c->ev_start, st));
     CK(c, cudaStreamWaitEvent(c->copy_stream, c->ev_start, 0));
   }
-  const bool host_out = (ok == PTR_HOST_PINNED && capacity > 0);
+  k.host_out = (ok == PTR_HOST_PINNED && k.capacity > 0);
   // 0 = library default: flush every 256 frames, so that only the last batch's D2H is exposed
-  const int wbf = c->d.writeback_frames > 0 ? c->d.writeback_frames : 256;
-  int64_t n_flush = 0;
-  auto flush = [&]() -> smlm_status {
-    const int64_t k = n_flush;
-    // the word snap[k % R] was read by flushes k - R (upper end) and k - R + 1 (lower end)
-    if (k >= kSnapRing) CK(c, cudaStreamWaitEvent(st, c->ev_wb[(k + 1) % kSnapRing], 0));
-    // records below the snapshot are complete: every K3 that wrote them precedes it on `st`
-    CK(c, launch_snapshot(counter, capacity, snap_ring + k % kSnapRing, st));
-    CK(c, cudaEventRecord(c->ev_batch, st));
-    CK(c, cudaStreamWaitEvent(c->wb_stream, c->ev_batch, 0));
-    const unsigned long long* lo = k == 0 ? c->counters + 1 : snap_ring + (k - 1) % kSnapRing;
-    CK(c, launch_flush_emitters(list, out, lo, snap_ring + k % kSnapRing, c->wb_stream));
-    CK(c, cudaEventRecord(c->ev_wb[k % kSnapRing], c->wb_stream));
-    c->launches += 2;
-    ++n_flush;
-    return SMLM_OK;
-  };
+  k.wbf = c->d.writeback_frames > 0 ? c->d.writeback_frames : 256;
+  return SMLM_OK;
+}
 
-  int64_t chunk = 0;
-  for (int64_t f0 = 0; f0 < n; f0 += F, ++chunk) {
-    const int nf = (int)std::min<int64_t>(F, n - f0);
+// frames [f_first, f_first + n) of the call, stored at `frames` (pinned host or device).
+// *copied (may be NULL): an event of the copy stream to record once the last H2D copy of
+// this piece has been enqueued (the ring loader releases its slot when it fires).
+smlm_status call_frames(Call& k, const uint16_t* frames, int64_t f_first, int64_t n, bool host_frames) {
+  smlm_ctx* c = k.c;
+  cudaStream_t st = k.st;
+  const int H = k.H, W = k.W, C = k.C, F = k.F;
+  const size_t frame_elems = (size_t)H * W;
+  unsigned long long* counter = c->counters;
+  smlm_status r = SMLM_OK;
+  for (int64_t f0 = f_first; f0 < f_first + n; f0 += F, ++k.chunk) {
+    const int nf = (int)std::min<int64_t>(F, f_first + n - f0);
     const uint16_t* dev_frames = frames;
-    int frame_base = 0;
+    int frame_base = (int)f_first;
     int slot = -1;
-    if (fk == PTR_HOST_PINNED) {
+    if (host_frames) {
       // P1: the preload ring.  Copy chunk k into slot k % kSlots on the copy stream as soon
       // as the stem of chunk k - kSlots has consumed it; compute waits for the copy only.
-      slot = (int)(chunk % kSlots);
+      slot = (int)(k.chunk % kSlots);
       if (c->slot_used[slot]) CK(c, cudaStreamWaitEvent(c->copy_stream, c->ev_consumed[slot], 0));
       uint16_t* dst = c->slots + (size_t)slot * c->slot_elems;
-      CK(c, cudaMemcpyAsync(dst, frames + (size_t)f0 * frame_elems, (size_t)nf * frame_elems * 2,
+      CK(c, cudaMemcpyAsync(dst, frames + (size_t)(f0 - f_first) * frame_elems, (size_t)nf * frame_elems * 2,
                             cudaMemcpyHostToDevice, c->copy_stream));
       CK(c, cudaEventRecord(c->ev_copied[slot], c->copy_stream));
       CK(c, cudaStreamWaitEvent(st, c->ev_copied[slot], 0));
@@ -676,20 +704,20 @@ smlm_status smlm_localize(smlm_ctx* c, const uint16_t* frames, int64_t n, int32_
     // launch sets of this chunk
     struct Set { ViewSet vs; ActShape s; };
     std::vector<Set> sets;
-    if (!tiled) {
+    if (!k.tiled) {
       ViewSet vs{(int)f0, H, W, 0, 0, 0, 1, 0, 1};
       sets.push_back({vs, ActShape{nf, C, H, W}});
     } else {
-      for (auto& a : ycls)
-        for (auto& b : xcls) {
+      for (auto& a : k.ycls)
+        for (auto& b : k.xcls) {
           // all tiles of the class for the nf frames of the chunk in one set if that is at
           // most mb views, else sub-blocks of tiles (times the frames) of at most mb views
-          const int per_frame = std::max(1, mb / nf);
+          const int per_frame = std::max(1, k.mb / nf);
           int bx = std::min(b.n, per_frame), by = std::max(1, std::min(a.n, per_frame / bx));
           for (int ty = a.t0; ty < a.t0 + a.n; ty += by)
             for (int tx = b.t0; tx < b.t0 + b.n; tx += bx) {
               int ny = std::min(by, a.t0 + a.n - ty), nx = std::min(bx, b.t0 + b.n - tx);
-              ViewSet vs{(int)f0, H, W, tile, halo, ty, ny, tx, nx};
+              ViewSet vs{(int)f0, H, W, k.tile, k.halo, ty, ny, tx, nx};
               sets.push_back({vs, ActShape{nf * ny * nx, C, a.ext, b.ext}});
             }
         }
@@ -698,31 +726,96 @@ smlm_status smlm_localize(smlm_ctx* c, const uint16_t* frames, int64_t n, int32_
       int res = 0;
       cudaEvent_t after_stem = (slot >= 0 && si + 1 == sets.size()) ? c->ev_consumed[slot] : nullptr;
       bool have_logit = false;
-      r = run_trunk(c, dev_frames, frame_base, sets[si].vs, sets[si].s, np, st, &res, nullptr, 0, 0,
-                    after_stem, true, hp.lthr, &have_logit);
+      r = run_trunk(c, dev_frames, frame_base, sets[si].vs, sets[si].s, k.np, st, &res, nullptr, 0, 0,
+                    after_stem, true, k.hp.lthr, &have_logit);
       if (r != SMLM_OK) return r;
       cudaEvent_t te = nullptr;
       if ((r = time_begin(c, SMLM_KERNEL_POST, st, &te)) != SMLM_OK) return r;
       if (have_logit)
-        CK(c, launch_post_logits(c->logit, c->cand, sets[si].s, sets[si].vs, hp, list, counter, capacity, st));
+        CK(c, launch_post_logits(c->logit, c->cand, sets[si].s, sets[si].vs, k.hp, k.list, counter, k.capacity, st));
       else
-        CK(c, launch_head_post(c->bf16, c->act[res], sets[si].s, sets[si].vs, c->w_head, c->b_head, hp,
-                               list, counter, capacity, st));
+        CK(c, launch_head_post(c->bf16, c->act[res], sets[si].s, sets[si].vs, c->w_head, c->b_head, k.hp,
+                               k.list, counter, k.capacity, st));
       c->launches++;
       if ((r = time_end(c, te, st)) != SMLM_OK) return r;
     }
-    if (host_out && wbf > 0) {
+    if (k.host_out && k.wbf > 0) {
       int64_t done = f0 + nf;
-      if (done < n && done / wbf != f0 / wbf) {
-        if ((r = flush()) != SMLM_OK) return r;
+      if (done < k.n_total && done / k.wbf != f0 / k.wbf) {
+        if ((r = call_flush(k)) != SMLM_OK) return r;
       }
     }
   }
-  if (host_out) {
-    if ((r = flush()) != SMLM_OK) return r;
+  return SMLM_OK;
+}
+
+smlm_status call_end(Call& k, int64_t* out_count) {
+  smlm_ctx* c = k.c;
+  smlm_status r;
+  if (k.host_out) {
+    if ((r = call_flush(k)) != SMLM_OK) return r;
   }
-  if (n_flush > 0) CK(c, cudaStreamWaitEvent(st, c->ev_wb[(n_flush - 1) % kSnapRing], 0));
-  return store_count(c, counter, out_count, st);
+  if (k.n_flush > 0) CK(c, cudaStreamWaitEvent(k.st, c->ev_wb[(k.n_flush - 1) % kSnapRing], 0));
+  return store_count(c, c->counters, out_count, k.st);
+}
+
+}  // namespace
+
+extern "C" {
+
+smlm_status smlm_localize(smlm_ctx* c, const uint16_t* frames, int64_t n, int32_t H, int32_t W,
+                          const smlm_camera_params* cam, float threshold, smlm_emitter* out,
+                          int64_t* out_count, void* cuda_stream) {
+  if (!c) return SMLM_ERR_INVALID_ARG;
+  PtrKind fk = PTR_DEVICE;
+  if (n > 0) {
+    if (!frames) return fail(c, SMLM_ERR_INVALID_ARG, "NULL frames");
+    fk = classify(frames);
+    if (fk == PTR_OTHER)
+      return fail(c, SMLM_ERR_INVALID_ARG,
+                  "frames_u16 must be pinned host memory (the preload ring) or device memory");
+  }
+  Call k;
+  smlm_status r = call_begin(k, c, n, H, W, cam, threshold, out, out_count, fk == PTR_HOST_PINNED,
+                             INT64_MAX, static_cast<cudaStream_t>(cuda_stream));
+  if (r != SMLM_OK) return r;
+  if ((r = call_frames(k, frames, 0, n, fk == PTR_HOST_PINNED)) != SMLM_OK) return r;
+  return call_end(k, out_count);
+}
+
+namespace {
+struct RingRelease { smlm_ring* r; int64_t k; };
+void CUDART_CB ring_release_cb(void* p) {
+  RingRelease* rr = static_cast<RingRelease*>(p);
+  ring_release_chunk(rr->r, rr->k);
+  delete rr;
+}
+}  // namespace
+
+smlm_status smlm_localize_ring(smlm_ctx* c, smlm_ring* ring, const smlm_camera_params* cam, float threshold,
+                               smlm_emitter* out, int64_t* out_count, void* cuda_stream) {
+  if (!c) return SMLM_ERR_INVALID_ARG;
+  if (!ring) return fail(c, SMLM_ERR_INVALID_ARG, "NULL ring");
+  if (!ring->pinned) return fail(c, SMLM_ERR_INVALID_ARG, "the ring is pageable (SMLM_RING_PAGEABLE is for tests)");
+  ring_rewind(ring);
+  Call k;
+  smlm_status r = call_begin(k, c, ring->n_frames, ring->H, ring->W, cam, threshold, out, out_count, true,
+                             ring->chunk_frames, static_cast<cudaStream_t>(cuda_stream));
+  if (r != SMLM_OK) return r;
+  for (int64_t ck = 0; ck < ring->n_chunks; ++ck) {
+    const uint16_t* p = ring_wait_chunk(ring, ck);  // blocks on the disk only
+    if (!p) return fail(c, SMLM_ERR_INVALID_ARG, "frame file: %s", ring->error.c_str());
+    if ((r = call_frames(k, p, ck * ring->chunk_frames, ring->frames_of(ck), true)) != SMLM_OK) return r;
+    // the slot goes back to the readers when the copy stream has drained this chunk's copies
+    RingRelease* rr = new (std::nothrow) RingRelease{ring, ck};
+    if (!rr) return fail(c, SMLM_ERR_OOM, "host allocation failed");
+    cudaError_t e = cudaLaunchHostFunc(c->copy_stream, ring_release_cb, rr);
+    if (e != cudaSuccess) {
+      delete rr;
+      return fail(c, SMLM_ERR_CUDA, "cudaLaunchHostFunc: %s", cudaGetErrorString(e));
+    }
+  }
+  return call_end(k, out_count);
 }
 
 smlm_status smlm_debug_forward_maps(smlm_ctx* c, const uint16_t* frames, int64_t n, int32_t H,

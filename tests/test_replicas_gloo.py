@@ -50,3 +50,21 @@ def test_job_throughput_is_sum_over_max_world2():
 def test_job_throughput_single_process():
     v, ms = job_throughput(100, 50.0)
     assert ms == 50.0 and v == pytest.approx(2000.0)
+
+
+@pytest.mark.parametrize("scaling,frames0,value", [("weak", 1000, 2000 / 11e-3), ("strong", 500, 1000 / 11e-3)])
+def test_bench_spawns_its_own_ranks(scaling, frames0, value):
+    """`python bench.py --gpus 2` without torchrun: bench.py starts the ranks itself
+    (torch.multiprocessing.spawn), shards by frame range in the strong case and reports
+    whole-job units / slowest rank's time.  Exercised on CPU over gloo with synthetic timings."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--selftest-spawn",
+                          "--scaling", scaling], capture_output=True, text=True, timeout=300, env=env)
+    assert out.returncode == 0, out.stderr[-2000:]
+    line = json.loads([l for l in out.stdout.splitlines() if l.startswith("{")][-1])
+    assert line["n_gpus"] == 2 and line["scaling"] == scaling and line["frames_rank0"] == frames0
+    assert line["ms_max"] == pytest.approx(11.0) and line["value"] == pytest.approx(value)
