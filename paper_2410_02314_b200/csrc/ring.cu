@@ -18,20 +18,23 @@ namespace {
 
 void reader_main(smlm_ring* r) {
   for (;;) {
-    int64_t k;
+    int64_t k, g;
     {
       std::unique_lock<std::mutex> lk(r->mu);
       if (r->stop) return;
       k = r->next_chunk.load();
+      g = r->gen;
       if (k >= r->n_chunks) {
         // wait for a rewind or for the end
-        r->cv.wait(lk, [&] { return r->stop || r->next_chunk.load() < r->n_chunks; });
+        r->cv.wait(lk, [&] { return r->stop || r->gen != g || r->next_chunk.load() < r->n_chunks; });
         continue;
       }
       r->next_chunk.store(k + 1);
       const int s = (int)(k % r->n_slots);
-      r->cv.wait(lk, [&] { return r->stop || r->free_from[s] == k; });
+      r->cv.wait(lk, [&] { return r->stop || r->gen != g || r->free_from[s] == k; });
       if (r->stop) return;
+      if (r->gen != g) continue;  // rewound while waiting: this assignment is void
+      ++r->active_reads;
     }
     const int s = (int)(k % r->n_slots);
     uint8_t* dst = reinterpret_cast<uint8_t*>(r->buf + (size_t)s * r->slot_elems());
@@ -51,10 +54,11 @@ void reader_main(smlm_ring* r) {
     }
     {
       std::lock_guard<std::mutex> lk(r->mu);
+      --r->active_reads;
       if (!err.empty()) {
         r->error = err;
         r->stop = true;
-      } else {
+      } else if (r->gen == g) {
         r->loaded[s] = k;
       }
     }
@@ -67,6 +71,7 @@ void reader_main(smlm_ring* r) {
 const uint16_t* ring_wait_chunk(smlm_ring* r, int64_t k) {
   const int s = (int)(k % r->n_slots);
   std::unique_lock<std::mutex> lk(r->mu);
+  r->touched = true;
   r->cv.wait(lk, [&] { return r->stop || r->loaded[s] == k; });
   if (r->loaded[s] != k) return nullptr;
   return r->buf + (size_t)s * r->slot_elems();
@@ -84,15 +89,23 @@ void ring_release_chunk(smlm_ring* r, int64_t k) {
   r->cv.notify_all();
 }
 
+// Start over at chunk 0.  Nothing to do on a ring no chunk of which has been handed out; else
+// the readers' pending assignments are voided (generation bump) and the call waits for reads
+// in flight, so that no stale reader writes into a slot of the new pass.
 void ring_rewind(smlm_ring* r) {
   {
-    std::lock_guard<std::mutex> lk(r->mu);
+    std::unique_lock<std::mutex> lk(r->mu);
+    if (!r->touched) return;
+    ++r->gen;
+    r->cv.notify_all();
+    r->cv.wait(lk, [&] { return r->stop || r->active_reads == 0; });
     for (int s = 0; s < r->n_slots; ++s) {
       r->loaded[s] = -1;
       r->free_from[s] = s;
     }
     r->next_chunk.store(0);
     r->next_acquire = 0;
+    r->touched = false;
   }
   r->cv.notify_all();
 }

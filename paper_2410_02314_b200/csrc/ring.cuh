@@ -29,6 +29,9 @@ struct smlm_ring {
   std::vector<int64_t> loaded, free_from;
   std::atomic<int64_t> next_chunk{0};
   int64_t next_acquire = 0;
+  int64_t gen = 0;       // bumped by a rewind: readers drop the chunk they were assigned before it
+  int active_reads = 0;  // readers inside pread
+  bool touched = false;  // a chunk has been handed out since the last rewind
   bool stop = false;
   std::string error;
   std::vector<std::thread> readers;
