@@ -46,6 +46,44 @@ class NetSpec:
 
 
 @dataclass(frozen=True)
+class DlocSpec:
+    """The paper's own topology: DCD dense blocks of dilated
+    convolutions, a two-stage U-Net, DECODE-style heads with uncertainties.  The paper gives no
+    widths: every number here is a reading (D1-D9)."""
+    c0: int = 48                                  # base width (D1)
+    growth: int = 16                              # channels per DCD layer (D1)
+    n_blocks: int = 4                             # 1 coarse-grained + 3 multi-scale (P:59)
+    dilations: Tuple[int, ...] = (2, 4, 8, 16)    # P:144
+    in_frames: int = 1                            # 3: frames f-1, f, f+1 (P:53, D8)
+    precision: str = "fp32"
+    stem_relu: int = 1
+    norm_scale: float = 1000.0
+    xy_scale: float = 0.5
+    z_scale_nm: float = 700.0
+    photon_scale: float = 1000.0
+    bg_scale: float = 100.0
+    sigma_xy_px: float = 3.0                      # D7
+    sigma_z_nm: float = 700.0
+    sigma_photons: float = 1000.0
+    head_channels: int = 10
+
+    def layers(self):
+        """(name, c_out, c_in, k) of every convolution in blob order."""
+        C, G = self.c0, self.growth
+        out = [("stem", C, self.in_frames, 3)]
+        for b in range(self.n_blocks):
+            for i in range(len(self.dilations)):
+                out.append((f"b{b}l{i}", G, C + i * G, 3))
+            out.append((f"b{b}t", C, C + len(self.dilations) * G, 1))
+        out += [("enc1", 2 * C, C, 3), ("enc2", 4 * C, 2 * C, 3), ("dec1", 2 * C, 6 * C, 3), ("dec0", C, 3 * C, 3),
+                ("head", self.head_channels, C, 1)]
+        return out
+
+    def n_params(self) -> int:
+        return sum(co * ci * k * k + co for _, co, ci, k in self.layers())
+
+
+@dataclass(frozen=True)
 class FrameSpec:
     n_frames: int
     height: int

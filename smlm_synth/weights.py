@@ -116,3 +116,21 @@ def make_weights(cfg: Config, flavour: Optional[str] = None, seed: Optional[int]
         raise KeyError(f"no calibration entry {key!r}; run tests/golden/make_calibration.py")
     e = cal[key]
     return apply_recipe(net, blob, cfg.g_res, e["row_gain"], e["kappa"], e["b_p"])
+
+
+def dloc_he_normal_blob(spec, seed: int, head_gain: float = 1.0, p_bias: float = 0.0) -> np.ndarray:
+    """He-normal weights (std = sqrt(2 / fan_in)) and zero biases for a DlocSpec, in blob order
+    (smlm.h: DilatedLoc topology); the head rows are scaled by head_gain and the detection bias
+    set to p_bias (input choices, like kappa / b_p of the residual nets)."""
+    rng = np.random.default_rng([int(seed), 0xD10C])
+    parts = []
+    for name, co, ci, k in spec.layers():
+        w = rng.normal(0.0, np.sqrt(2.0 / (ci * k * k)), size=co * ci * k * k)
+        b = np.zeros(co)
+        if name == "head":
+            w *= head_gain
+            b[0] = p_bias
+        parts += [w, b]
+    blob = np.concatenate(parts).astype(np.float32)
+    assert blob.size == spec.n_params()
+    return blob
