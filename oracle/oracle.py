@@ -27,7 +27,8 @@ class OracleNet(C.Structure):
     _fields_ = [("channels", C.c_int32), ("n_layers", C.c_int32),
                 ("dilations", C.c_int32 * MAX_LAYERS), ("head_channels", C.c_int32),
                 ("stem_relu", C.c_int32), ("norm_scale", C.c_double), ("xy_scale", C.c_double),
-                ("z_scale_nm", C.c_double), ("photon_scale", C.c_double), ("bg_scale", C.c_double)]
+                ("z_scale_nm", C.c_double), ("photon_scale", C.c_double), ("bg_scale", C.c_double),
+                ("in_frames", C.c_int32)]
 
 
 class OracleCamera(C.Structure):
@@ -107,7 +108,7 @@ def threads() -> int:
 
 def make_net(channels: int, dilations: Sequence[int], head_channels: int, stem_relu: int = 1,
              norm_scale: float = 1000.0, xy_scale: float = 0.5, z_scale_nm: float = 700.0,
-             photon_scale: float = 1000.0, bg_scale: float = 100.0) -> OracleNet:
+             photon_scale: float = 1000.0, bg_scale: float = 100.0, in_frames: int = 1) -> OracleNet:
     net = OracleNet()
     net.channels = int(channels)
     net.n_layers = len(dilations)
@@ -120,6 +121,7 @@ def make_net(channels: int, dilations: Sequence[int], head_channels: int, stem_r
     net.z_scale_nm = float(z_scale_nm)
     net.photon_scale = float(photon_scale)
     net.bg_scale = float(bg_scale)
+    net.in_frames = int(in_frames)
     return net
 
 
@@ -127,7 +129,7 @@ def net_from_spec(spec) -> OracleNet:
     """spec: smlm_synth.NetSpec (plain data)."""
     return make_net(spec.channels, spec.dilations, spec.head_channels, spec.stem_relu,
                     spec.norm_scale, spec.xy_scale, spec.z_scale_nm, spec.photon_scale,
-                    spec.bg_scale)
+                    spec.bg_scale, getattr(spec, "in_frames", 1))
 
 
 class _Cam:

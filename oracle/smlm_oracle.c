@@ -56,6 +56,10 @@ typedef struct {
   double z_scale_nm;     /* 700 */
   double photon_scale;   /* reading G6 */
   double bg_scale;       /* reading G6 */
+  int32_t in_frames;     /* 0 or 1: one frame per input; 3: temporal context, the stem sees the frames
+                            f-1, f, f+1 as three input channels ("contextual three-frame
+                            information"; reading G24 in DESIGN.md: indices
+                            clamped to [0, n-1] of the call) */
 } oracle_net;
 
 typedef struct {
@@ -79,9 +83,11 @@ int smlm_oracle_threads(void) {
 #endif
 }
 
+static int in_frames_of(const oracle_net *net) { return net->in_frames == 3 ? 3 : 1; }
+
 int64_t smlm_oracle_blob_size(const oracle_net *net) {
-  int64_t C = net->channels, L = net->n_layers, nh = net->head_channels;
-  return (C * 9 + C) + L * (C * C * 9 + C) + (nh * C + nh);
+  int64_t C = net->channels, L = net->n_layers, nh = net->head_channels, IF = in_frames_of(net);
+  return (C * IF * 9 + C) + L * (C * C * 9 + C) + (nh * C + nh);
 }
 
 /* O1 normalise: xhat = ((adu - offset) / gain) / norm_scale  (reading G5). */
@@ -96,21 +102,23 @@ static void normalise(const uint16_t *frame, int H, int W, const oracle_camera *
     }
 }
 
-/* O2 stem: a0[y,x,co] = act(b0[co] + sum_{ky,kx} W0[co,0,ky,kx] * xhat[y+ky-1, x+kx-1]),
- * out-of-frame xhat := 0; act = ReLU iff stem_relu (reading G3). */
-static void stem(const double *xhat, int H, int W, int C, const float *w /*[C][1][3][3]*/,
-                 const float *b, int relu, double *a0 /*[H][W][C]*/) {
+/* O2 stem: a0[y,x,co] = act(b0[co] + sum_{ch,ky,kx} W0[co,ch,ky,kx] * xhat[ch][y+ky-1, x+kx-1]),
+ * out-of-frame xhat := 0; act = ReLU iff stem_relu (reading G3); ch < IF input channels
+ * (IF = 1: the frame itself; IF = 3: the normalised frames f-1, f, f+1, reading G24). */
+static void stem(const double *xhat /*[IF][H][W]*/, int IF, int H, int W, int C,
+                 const float *w /*[C][IF][3][3]*/, const float *b, int relu, double *a0 /*[H][W][C]*/) {
 #pragma omp parallel for schedule(static)
   for (int y = 0; y < H; ++y)
     for (int x = 0; x < W; ++x)
       for (int co = 0; co < C; ++co) {
         double acc = (double)b[co];
-        for (int ky = 0; ky < 3; ++ky)
-          for (int kx = 0; kx < 3; ++kx) {
-            int yy = y + ky - 1, xx = x + kx - 1;
-            if (yy < 0 || yy >= H || xx < 0 || xx >= W) continue;
-            acc += (double)w[(co * 3 + ky) * 3 + kx] * xhat[(int64_t)yy * W + xx];
-          }
+        for (int ch = 0; ch < IF; ++ch)
+          for (int ky = 0; ky < 3; ++ky)
+            for (int kx = 0; kx < 3; ++kx) {
+              int yy = y + ky - 1, xx = x + kx - 1;
+              if (yy < 0 || yy >= H || xx < 0 || xx >= W) continue;
+              acc += (double)w[((co * IF + ch) * 3 + ky) * 3 + kx] * xhat[((int64_t)ch * H + yy) * W + xx];
+            }
         if (relu && acc < 0.0) acc = 0.0;
         a0[((int64_t)y * W + x) * C + co] = acc;
       }
@@ -180,7 +188,8 @@ int smlm_oracle_forward_maps(const oracle_net *net, const float *weights, const 
   if (C < 1 || C > 256 || L < 0 || L > ORACLE_MAX_LAYERS || (nh != 5 && nh != 6) || H < 1 || W < 1)
     return -1;
   int64_t px = (int64_t)H * W;
-  double *xhat = (double *)malloc(sizeof(double) * px);
+  const int IF = in_frames_of(net);
+  double *xhat = (double *)malloc(sizeof(double) * px * IF);
   double *a = (double *)malloc(sizeof(double) * px * C);
   double *a2 = (double *)malloc(sizeof(double) * px * C);
   double *wt = (double *)malloc(sizeof(double) * 9 * C * C);
@@ -190,9 +199,14 @@ int smlm_oracle_forward_maps(const oracle_net *net, const float *weights, const 
   }
   for (int64_t f = 0; f < n; ++f) {
     const float *wp = weights;
-    normalise(frames + f * px, H, W, cam, net->norm_scale, xhat);
-    stem(xhat, H, W, C, wp, wp + C * 9, net->stem_relu, a);
-    wp += C * 9 + C;
+    for (int ch = 0; ch < IF; ++ch) { /* IF = 3: frames f-1, f, f+1, clamped to the call (G24) */
+      int64_t g = IF == 1 ? f : f + ch - 1;
+      if (g < 0) g = 0;
+      if (g > n - 1) g = n - 1;
+      normalise(frames + g * px, H, W, cam, net->norm_scale, xhat + ch * px);
+    }
+    stem(xhat, IF, H, W, C, wp, wp + C * IF * 9, net->stem_relu, a);
+    wp += C * IF * 9 + C;
     if (trunk_dump) memcpy(trunk_dump + (f * (L + 1) + 0) * px * C, a, sizeof(double) * px * C);
     for (int l = 0; l < L; ++l) {
       /* OIHW [co][ci][ky][kx] -> [ky][kx][ci][co] */

@@ -18,13 +18,14 @@ class NetSpec:
     channels: int                 # C
     dilations: Tuple[int, ...]    # d_l, l = 0..L-1
     head_channels: int            # 5: p,dx,dy,N,bg   6: p,dx,dy,z,N,bg
-    precision: str                # "fp32" | "bf16"
+    precision: str                # "fp32" | "bf16" | "fp16" (fp16: the 8(f)-4 activation-precision variant)
     stem_relu: int = 1            # reading G3
     norm_scale: float = 1000.0    # BASELINE.json configs[0]: (x-100)/1000
     xy_scale: float = 0.5         # tanh*0.5
     z_scale_nm: float = 700.0     # reading G6
     photon_scale: float = 1000.0  # reading G6
     bg_scale: float = 100.0       # reading G6
+    in_frames: int = 1            # 3: temporal context, frames f-1, f, f+1 as stem input channels (G24)
 
     @property
     def n_layers(self) -> int:
@@ -37,12 +38,12 @@ class NetSpec:
 
     def n_params(self) -> int:
         C, L, nh = self.channels, self.n_layers, self.head_channels
-        return (C * 9 + C) + L * (C * C * 9 + C) + (nh * C + nh)
+        return (C * self.in_frames * 9 + C) + L * (C * C * 9 + C) + (nh * C + nh)
 
     def flop_per_px(self) -> int:
         """2 x MAC: stem 18C, each layer 18C^2, head 2C n_h."""
         C, L, nh = self.channels, self.n_layers, self.head_channels
-        return 18 * C + 18 * C * C * L + 2 * C * nh
+        return 18 * C * self.in_frames + 18 * C * C * L + 2 * C * nh
 
 
 @dataclass(frozen=True)

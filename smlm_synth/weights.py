@@ -44,7 +44,7 @@ def blob_offsets(net: NetSpec) -> dict:
     C, L, nh = net.channels, net.n_layers, net.head_channels
     off = {}
     p = 0
-    off["stem_w"] = p; p += C * 9
+    off["stem_w"] = p; p += C * net.in_frames * 9
     off["stem_b"] = p; p += C
     for l in range(L):
         off[f"w{l}"] = p; p += C * C * 9
@@ -60,7 +60,7 @@ def he_normal_blob(net: NetSpec, seed: int) -> np.ndarray:
     C, L, nh = net.channels, net.n_layers, net.head_channels
     rng = np.random.default_rng([int(seed), 0x57E1])
     parts = []
-    parts.append(rng.normal(0.0, np.sqrt(2.0 / 9.0), size=C * 9))
+    parts.append(rng.normal(0.0, np.sqrt(2.0 / (9.0 * net.in_frames)), size=C * net.in_frames * 9))
     parts.append(np.zeros(C))
     for _ in range(L):
         parts.append(rng.normal(0.0, np.sqrt(2.0 / (9.0 * C)), size=C * C * 9))

@@ -48,7 +48,8 @@ def _rand_blob(spec, seed, bias=True):
 def _split(spec, blob):
     off = blob_offsets(spec)
     C, nh = spec.channels, spec.head_channels
-    out = {"stem_w": blob[off["stem_w"]:off["stem_w"] + C * 9].reshape(C, 1, 3, 3).astype(np.float64),
+    IF = spec.in_frames
+    out = {"stem_w": blob[off["stem_w"]:off["stem_w"] + C * IF * 9].reshape(C, IF, 3, 3).astype(np.float64),
            "stem_b": blob[off["stem_b"]:off["stem_b"] + C].astype(np.float64), "w": [], "b": []}
     for l in range(spec.n_layers):
         out["w"].append(blob[off[f"w{l}"]:off[f"w{l}"] + C * C * 9].reshape(C, C, 3, 3).astype(np.float64))
@@ -395,3 +396,71 @@ def test_halo_46_is_exact_and_45_is_not():
     R = spec.radius
     assert np.max(np.abs(whole[:, :120 - R, :120 - R] - crop[:, :120 - R, :120 - R])) == 0.0
     assert np.max(np.abs(whole[:, :120 - R + 1, :120 - R + 1] - crop[:, :120 - R + 1, :120 - R + 1])) > 0.0
+
+
+# --------------------------------------------------------------------------- 3-frame temporal context (G24)
+def _context_stack(frames):
+    """[n][H][W] -> [n][3][H][W]: frames f-1, f, f+1 with indices clamped to the call."""
+    n = len(frames)
+    idx = np.clip(np.arange(n)[:, None] + np.array([-1, 0, 1])[None], 0, n - 1)
+    return frames[idx]
+
+
+def test_three_frame_stem_matches_torch_conv2d():
+    """in_frames = 3: the stem is a 3 -> C convolution over the
+    normalised frames f-1, f, f+1 (clamped).  Library routine: torch conv2d in fp64 on the
+    explicitly built 3-channel input; catches a wrong channel order, a wrong clamp and a
+    wrong weight stride."""
+    import torch
+    import torch.nn.functional as F
+    spec = NetSpec(6, (1, 2), 5, "fp32", in_frames=3)
+    blob = _rand_blob(spec, 21)
+    rng = np.random.default_rng(4)
+    frames = rng.integers(50, 4000, size=(5, 17, 19)).astype(np.uint16)
+    net = O.net_from_spec(spec)
+    cam = O.make_camera(100.0, 90.0, 1.3)
+    o, dump = O.forward_maps(net, blob, frames, cam, dump_trunk=True)
+    p = _split(spec, blob)
+    x = torch.from_numpy(((_context_stack(frames).astype(np.float64) - 90.0) / 1.3) / spec.norm_scale)
+    a = torch.relu(F.conv2d(x, torch.from_numpy(p["stem_w"]), torch.from_numpy(p["stem_b"]), padding=1))
+    assert np.max(np.abs(dump[:, 0].transpose(0, 3, 1, 2) - a.numpy())) < 1e-12
+    for l, d in enumerate(spec.dilations):
+        a = a + torch.relu(F.conv2d(a, torch.from_numpy(p["w"][l]), torch.from_numpy(p["b"][l]), padding=d, dilation=d))
+    ot = F.conv2d(a, torch.from_numpy(p["head_w"])[:, :, None, None], torch.from_numpy(p["head_b"])).numpy()
+    assert np.max(np.abs(o - ot)) < 1e-10
+
+
+def test_three_frame_stem_reduces_to_single_frame_and_pins_channel_order():
+    """Weights on the centre channel only == the 1-frame network on the same frames; weights
+    on channel 0 (or 2) only == the 1-frame network on the sequence shifted by one frame with
+    the first (last) frame repeated: pins which channel is f-1 and the clamp at both ends."""
+    spec1 = NetSpec(4, (1, 2), 5, "fp32")
+    spec3 = NetSpec(4, (1, 2), 5, "fp32", in_frames=3)
+    b1 = _rand_blob(spec1, 33)
+    rng = np.random.default_rng(6)
+    frames = rng.integers(50, 4000, size=(4, 11, 12)).astype(np.uint16)
+    cam = O.make_camera(100.0, 100.0, 1.0)
+    o1 = O.forward_maps(O.net_from_spec(spec1), b1, frames, cam)
+    C = spec1.channels
+    for ch, seq in ((1, frames), (0, frames[[0, 0, 1, 2]]), (2, frames[[1, 2, 3, 3]])):
+        w3 = np.zeros((C, 3, 3, 3), dtype=np.float32)
+        w3[:, ch] = b1[:C * 9].reshape(C, 3, 3)
+        b3 = np.concatenate([w3.ravel(), b1[C * 9:]])
+        assert b3.size == blob_size(spec3)
+        o3 = O.forward_maps(O.net_from_spec(spec3), b3, frames, cam)
+        ref = o1 if ch == 1 else O.forward_maps(O.net_from_spec(spec1), b1, seq, cam)
+        assert np.array_equal(o3, ref), f"channel {ch}"
+
+
+def test_three_frame_stem_bruteforce_scatter():
+    spec = NetSpec(3, (2,), 5, "fp32", in_frames=3)
+    blob = _rand_blob(spec, 8)
+    rng = np.random.default_rng(2)
+    frames = rng.integers(0, 3000, size=(3, 9, 10)).astype(np.uint16)
+    o, dump = O.forward_maps(O.net_from_spec(spec), blob, frames, O.make_camera(100.0, 100.0, 1.7), dump_trunk=True)
+    p = _split(spec, blob)
+    ctx = _context_stack(frames)
+    for f in range(3):
+        xhat = ((ctx[f].astype(np.float64) - 100.0) / 1.7) / spec.norm_scale
+        a = np.maximum(_scatter_conv(xhat, p["stem_w"], p["stem_b"], 1), 0)
+        assert np.max(np.abs(dump[f, 0].transpose(2, 0, 1) - a)) < 1e-12
