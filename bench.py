@@ -41,6 +41,26 @@ def load_peaks():
     return dict(FALLBACK_PEAKS), "fallback"
 
 
+def lookup_traffic(cfg, C, views, bound):
+    """(bytes per full-size launch, provenance) of the plain K2 launch from profiles/traffic_r2.json."""
+    path = os.path.join(ROOT, "profiles", "traffic_r2.json")
+    if bound != "tensor" or not os.path.exists(path):
+        return None, "no capture"
+    with open(path, "r", encoding="utf-8") as fh:
+        doc = json.load(fh)
+    wl = {4: "cfg1"}.get(cfg.index, f"cfg{cfg.index}")        # cfg 4 launches are cfg 1's (same net, same shape)
+    cap = doc.get("captures", {}).get(f"{wl}/views{views}")
+    if not cap:
+        return None, f"no capture for {wl}/views{views} in profiles/traffic_r2.json"
+    k = cap["per_kernel_mean"].get(f"conv_umma_kernel<{C},-,->")
+    if not k:
+        return None, "capture holds no plain K2 launch"
+    note = (f"profiles/traffic_r2.json {wl}/views{views}: mean of {k['n']} plain K2 launches of {views} views "
+            f"(ncu --set full, {cap.get('source', '')}); the HEAD launch and the tail launch of a step are listed "
+            f"there separately")
+    return k["dram_bytes"], note
+
+
 def workload(cfg, n_frames=None):
     n = cfg.frames.n_frames if n_frames is None else n_frames
     # bounded generation time: at most 2^25 distinct pixels (cfg 3: 8 distinct 2048x2048 frames)
@@ -188,6 +208,11 @@ def main(argv=None):
     ap.add_argument("--conv-impl", default="auto", choices=["auto", "tcgen05", "direct"])
     ap.add_argument("--micro-batch", type=int, default=0)
     ap.add_argument("--fusion", default="auto", choices=["auto", "none", "all"])
+    ap.add_argument("--tile", type=int, default=-1, help="override the config's tile size (0: whole frames)")
+    ap.add_argument("--tile-merge", default="none", choices=["none", "row"],
+                    help="row: one window per tile row (SMLM_TILE_MERGE_ROW)")
+    ap.add_argument("--precision", default="", choices=["", "bf16", "fp16"],
+                    help="activation storage type of the variants study (SURVEY.md 8(f)-4); default: the config's")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = every rank localises the config's full stack (replicas); "
@@ -198,6 +223,12 @@ def main(argv=None):
                          "reduction over gloo with synthetic per-rank timings")
     args = ap.parse_args(argv)
     cfg = get_config(args.config)
+    if args.tile >= 0 or args.precision:
+        import dataclasses
+        if args.tile >= 0:
+            cfg = dataclasses.replace(cfg, tile=args.tile)
+        if args.precision:
+            cfg = dataclasses.replace(cfg, net=dataclasses.replace(cfg.net, precision=args.precision))
     if args.impl == "reference":
         return run_reference(args, cfg)
     args.warmup = max(args.warmup, 3)
@@ -232,6 +263,7 @@ def main(argv=None):
     conv_impl = {"auto": P.CONV_AUTO, "tcgen05": P.CONV_TCGEN05, "direct": P.CONV_DIRECT}[args.conv_impl]
     desc = P.desc_from_spec(cfg.net, tile=cfg.tile, micro_batch=args.micro_batch, conv_impl=conv_impl,
                             writeback_frames=cfg.writeback_batch,
+                            tile_merge={"none": P.TILE_MERGE_NONE, "row": P.TILE_MERGE_ROW}[args.tile_merge],
                             fusion={"auto": P.FUSE_AUTO, "none": P.FUSE_NONE, "all": P.FUSE_ALL}[args.fusion])
     loc = P.Localizer(desc, weights)
     cap = int(n_frames * max(4 * cfg.frames.emitters_per_frame, 1024))
@@ -321,6 +353,16 @@ def main(argv=None):
 
     peaks, peak_kind = load_peaks()
     C, L = cfg.net.channels, cfg.net.n_layers
+    # views of a full-size launch (api.cu auto_micro_batch: <= 64, <= 1.5 GB per activation buffer)
+    if args.micro_batch:
+        loc_views_per_launch = args.micro_batch
+    elif cfg.tile:   # the largest launch set: all interior tiles (window = tile + 2 halo) of the chunk's frames
+        ext = cfg.tile + 2 * (cfg.net.radius + 1)
+        mb = int(min(64, max(1, (1536 << 20) // (ext * ext * C * 2))))
+        inner = max(1, (-(-H // cfg.tile) - 2)) * max(1, (-(-W // cfg.tile) - 2))
+        loc_views_per_launch = max(1, min(mb // inner, n_frames)) * inner
+    else:
+        loc_views_per_launch = int(min(64, max(1, (1536 << 20) // (H * W * C * 2)), n_frames))
     # dominant kernel: the dilated 3x3 conv layer (K2).  Algorithmic work per launch =
     # 18 C^2 FLOP per pixel per layer x the pixels one launch processes.
     flop_total = 18.0 * C * C * H * W * n_frames * L * args.steps
@@ -329,17 +371,16 @@ def main(argv=None):
         achieved = flop_total / (conv_ms * 1e-3) / 1e12
         peak = float(peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]))
         bound = "tensor"
-        if cfg.net.precision != "bf16" or args.conv_impl == "direct":
+        if cfg.net.precision not in ("bf16", "fp16") or args.conv_impl == "direct":
             bound = "alu"
-        # DRAM traffic per launch from the ncu --set full capture of this kernel in this launch
-        # configuration (profiles/kernels_r1_final_full.md: cfg 1, 64 frames per launch,
-        # dram__bytes_read.sum + dram__bytes_write.sum = 435 + 354 MB); null for other shapes.
-        traffic = None
+        # DRAM traffic per launch: dram__bytes_read.sum + dram__bytes_write.sum of this kernel
+        # in this launch shape, from the tracked ncu --set full record (profiles/traffic_r2.json,
+        # written by paper_2410_02314_b200/profile_tools.py from the capture named there);
+        # null when no capture of this (workload, views per launch) exists.
         alg_bytes_per_launch = 4.0 * C * H * W * (n_frames * args.steps * L / conv_n)
-        if cfg.index in (1, 4) and bound == "tensor" and abs(alg_bytes_per_launch - 805.3e6) < 1e6:
-            traffic = 789.0e6
+        traffic, traffic_note = lookup_traffic(cfg, C, loc_views_per_launch, bound)
         roofline = {"bound": bound, "kernel": "conv3x3_dilated (K2)", "achieved": achieved, "peak": peak,
-                    "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
+                    "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_note,
                     "algorithmic_bytes_per_launch": alg_bytes_per_launch,
                     "hbm_GBs_algorithmic": alg_bytes_per_launch * conv_n / (conv_ms * 1e-3) / 1e9,
                     "hbm_frac_algorithmic": alg_bytes_per_launch * conv_n / (conv_ms * 1e-3) / 1e9
@@ -374,9 +415,10 @@ def main(argv=None):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
         "scaling": args.scaling, "vs_baseline": None,
-        "dtype": "bf16" if cfg.net.precision == "bf16" else "f32", "data": "synthetic",
+        "dtype": {"bf16": "bf16", "fp16": "f16"}.get(cfg.net.precision, "f32"), "data": "synthetic",
         "config": {"workload": cfg.name, "frames_per_step": n_frames, "H": H, "W": W, "channels": C,
-                   "layers": L, "head_channels": cfg.net.head_channels, "tile": cfg.tile,
+                   "layers": L, "head_channels": cfg.net.head_channels, "tile": cfg.tile, "tile_merge": args.tile_merge,
+                   "precision": cfg.net.precision,
                    "distinct_frames": int(len(fs.frames)), "conv_impl": args.conv_impl, "fusion": args.fusion,
                    "l2": "inputs larger than L2 (u16 stack + activation stream per step > 126 MB)",
                    "parallelism": f"replicas x{world}"},

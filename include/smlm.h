@@ -42,7 +42,7 @@
 extern "C" {
 #endif
 
-#define SMLM_ABI_VERSION 2
+#define SMLM_ABI_VERSION 3
 #define SMLM_MAX_LAYERS 32
 
 typedef struct smlm_ctx smlm_ctx; /* opaque; owns device weights, activations, staging slots, events */
@@ -56,9 +56,18 @@ typedef enum {
   SMLM_ERR_OVERFLOW = -5 /* more emitters found than capacity (reported by smlm_check) */
 } smlm_status;
 
-enum { SMLM_FP32 = 0, SMLM_BF16 = 1 };
+/* Storage type of the activation maps and input type of the trunk's tensor-core MMAs.  FP16 is
+ * the accuracy / throughput variant of SURVEY.md 8(f)-4: 11-bit mantissa at the same tensor
+ * rate as bf16 (fp32 accumulate in both). */
+enum { SMLM_FP32 = 0, SMLM_BF16 = 1, SMLM_FP16 = 2 };
 
-/* Trunk convolution kernel choice for SMLM_BF16 (fp32 mode always uses the CUDA-core kernel). */
+/* How the windows of a tiled call (tile > 0) are formed.
+ *   NONE  one window per tile x tile core (+ halo): BASELINE.json configs[3] as written.
+ *   ROW   the cores of one tile row share one window (core = tile rows x the whole frame
+ *         width): their x halos are computed once instead of twice.  Same emitter list. */
+enum { SMLM_TILE_MERGE_NONE = 0, SMLM_TILE_MERGE_ROW = 1 };
+
+/* Trunk convolution kernel choice for SMLM_BF16 / SMLM_FP16 (fp32 mode always uses the CUDA-core kernel). */
 enum {
   SMLM_CONV_AUTO = 0,   /* tcgen05 implicit GEMM */
   SMLM_CONV_TCGEN05 = 1,
@@ -81,9 +90,9 @@ typedef struct {
   uint32_t version;     /* SMLM_ABI_VERSION */
   int32_t channels;     /* C: multiple of 16, 16..64 */
   int32_t n_layers;     /* L: 0..SMLM_MAX_LAYERS dilated layers */
-  int32_t dilations[SMLM_MAX_LAYERS]; /* d_l in 1..8 */
+  int32_t dilations[SMLM_MAX_LAYERS]; /* d_l in 1..16 */
   int32_t head_channels; /* 5: p,dx,dy,N,bg    6: p,dx,dy,z,N,bg */
-  int32_t precision;     /* SMLM_FP32 | SMLM_BF16 (bf16 storage + bf16 tensor-core trunk, fp32 accumulate) */
+  int32_t precision;     /* SMLM_FP32 | SMLM_BF16 | SMLM_FP16 (16-bit storage + tensor-core trunk, fp32 accumulate) */
   int32_t stem_relu;     /* 1: ReLU after the stem conv */
   float norm_scale;      /* 1000 */
   float xy_scale;        /* 0.5 */
@@ -99,6 +108,11 @@ typedef struct {
                                per this many frames, overlapped with compute (0 = library
                                default, 256; the last flush is at the end of the call) */
   int32_t fusion;        /* SMLM_FUSE_*: which steps share a kernel on the tcgen05 path */
+  int32_t in_frames;     /* 0 or 1: the stem sees frame f.  3: temporal context ("contextual
+                            three-frame information"): the stem is a 3 -> C convolution over the
+                            normalised frames f-1, f, f+1 of the call, indices clamped to
+                            [0, n_frames-1].  Not available through smlm_localize_ring. */
+  int32_t tile_merge;    /* SMLM_TILE_MERGE_* */
 } smlm_net_desc;
 
 /* Camera model.  Scalars are used where a map pointer is NULL.  Maps are [H][W] float32,
@@ -123,7 +137,7 @@ typedef struct {
 /*
  * smlm_create: validate `desc`, copy `weights` to the device, pre-pack the trunk weights
  * for the tensor cores.  `weights` is a HOST pointer to one little-endian fp32 blob:
- *     stem W[C][1][3][3], b[C];  for l < L: W_l[C][C][3][3] (OIHW), b_l[C];  head W[n_h][C], b[n_h]
+ *     stem W[C][in_frames][3][3], b[C];  for l < L: W_l[C][C][3][3] (OIHW), b_l[C];  head W[n_h][C], b[n_h]
  * (cross-correlation).  Both inputs may be freed when the call returns.  Synchronous.
  * Errors: INVALID_ARG (NULL, bad sizes), UNSUPPORTED_DEVICE, CUDA, OOM.  *out_ctx = NULL on error.
  */

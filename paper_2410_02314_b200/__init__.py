@@ -3,10 +3,10 @@ of single-molecule frames plus on-GPU post-processing, as a C-ABI library
 (include/smlm.h) with a thin ctypes binding.  See DESIGN.md."""
 from .binding import (ABI_VERSION, BF16, CONV_AUTO, CONV_DIRECT, CONV_TCGEN05, EMITTER_DTYPE,
                       ERR_CUDA, ERR_INVALID_ARG, ERR_OOM, ERR_OVERFLOW, ERR_UNSUPPORTED_DEVICE,
-                      EXPORTS, FP32, FUSE_ALL, FUSE_AUTO, FUSE_NONE, KERNEL_CONV, KERNEL_POST, KERNEL_STEM, OK, CameraParams, Localizer, NetDesc, Ring, SmlmError,
+                      EXPORTS, FP16, FP32, TILE_MERGE_NONE, TILE_MERGE_ROW, FUSE_ALL, FUSE_AUTO, FUSE_NONE, KERNEL_CONV, KERNEL_POST, KERNEL_STEM, OK, CameraParams, Localizer, NetDesc, Ring, SmlmError,
                       desc_from_spec, emitters_to_numpy, lib, make_desc)
 
 __all__ = ["ABI_VERSION", "BF16", "CONV_AUTO", "CONV_DIRECT", "CONV_TCGEN05", "EMITTER_DTYPE",
            "ERR_CUDA", "ERR_INVALID_ARG", "ERR_OOM", "ERR_OVERFLOW", "ERR_UNSUPPORTED_DEVICE",
-           "EXPORTS", "FP32", "FUSE_ALL", "FUSE_AUTO", "FUSE_NONE", "KERNEL_CONV", "KERNEL_POST", "KERNEL_STEM", "OK", "CameraParams", "Localizer", "NetDesc", "Ring", "SmlmError",
+           "EXPORTS", "FP16", "FP32", "TILE_MERGE_NONE", "TILE_MERGE_ROW", "FUSE_ALL", "FUSE_AUTO", "FUSE_NONE", "KERNEL_CONV", "KERNEL_POST", "KERNEL_STEM", "OK", "CameraParams", "Localizer", "NetDesc", "Ring", "SmlmError",
            "desc_from_spec", "emitters_to_numpy", "lib", "make_desc"]

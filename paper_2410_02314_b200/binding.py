@@ -15,10 +15,11 @@ import numpy as np
 from . import build as _build
 
 MAX_LAYERS = 32
-FP32, BF16 = 0, 1
+FP32, BF16, FP16 = 0, 1, 2
+TILE_MERGE_NONE, TILE_MERGE_ROW = 0, 1
 CONV_AUTO, CONV_TCGEN05, CONV_DIRECT = 0, 1, 2
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED_DEVICE, ERR_CUDA, ERR_OOM, ERR_OVERFLOW = 0, -1, -2, -3, -4, -5
-ABI_VERSION = 2
+ABI_VERSION = 3
 FUSE_AUTO, FUSE_NONE, FUSE_ALL = 0, 1, 2
 KERNEL_STEM, KERNEL_CONV, KERNEL_POST = 0, 1, 2
 
@@ -37,7 +38,8 @@ class NetDesc(C.Structure):
                 ("norm_scale", C.c_float), ("xy_scale", C.c_float), ("z_scale_nm", C.c_float),
                 ("photon_scale", C.c_float), ("bg_scale", C.c_float), ("tile", C.c_int32),
                 ("micro_batch", C.c_int32), ("conv_impl", C.c_int32),
-                ("writeback_frames", C.c_int32), ("fusion", C.c_int32)]
+                ("writeback_frames", C.c_int32), ("fusion", C.c_int32), ("in_frames", C.c_int32),
+                ("tile_merge", C.c_int32)]
 
 
 class CameraParams(C.Structure):
@@ -107,7 +109,8 @@ def make_desc(channels: int, dilations: Sequence[int], head_channels: int, preci
               stem_relu: int = 1, norm_scale: float = 1000.0, xy_scale: float = 0.5,
               z_scale_nm: float = 700.0, photon_scale: float = 1000.0, bg_scale: float = 100.0,
               tile: int = 0, micro_batch: int = 0, conv_impl: int = CONV_AUTO,
-              writeback_frames: int = 0, fusion: int = FUSE_AUTO) -> NetDesc:
+              writeback_frames: int = 0, fusion: int = FUSE_AUTO, in_frames: int = 1,
+              tile_merge: int = TILE_MERGE_NONE) -> NetDesc:
     d = NetDesc()
     d.struct_size = C.sizeof(NetDesc)
     d.version = ABI_VERSION
@@ -123,13 +126,16 @@ def make_desc(channels: int, dilations: Sequence[int], head_channels: int, preci
     d.tile, d.micro_batch, d.conv_impl = int(tile), int(micro_batch), int(conv_impl)
     d.writeback_frames = int(writeback_frames)
     d.fusion = int(fusion)
+    d.in_frames = int(in_frames)
+    d.tile_merge = int(tile_merge)
     return d
 
 
 def desc_from_spec(spec, **overrides) -> NetDesc:
     """spec: smlm_synth.NetSpec (plain data)."""
     kw = dict(channels=spec.channels, dilations=spec.dilations, head_channels=spec.head_channels,
-              precision=BF16 if spec.precision == "bf16" else FP32, stem_relu=spec.stem_relu,
+              precision={"bf16": BF16, "fp16": FP16}.get(spec.precision, FP32), stem_relu=spec.stem_relu,
+              in_frames=getattr(spec, "in_frames", 1),
               norm_scale=spec.norm_scale, xy_scale=spec.xy_scale, z_scale_nm=spec.z_scale_nm,
               photon_scale=spec.photon_scale, bg_scale=spec.bg_scale)
     kw.update(overrides)
@@ -164,7 +170,8 @@ class Localizer:
         self.desc = desc
         w = np.ascontiguousarray(weights, dtype="<f4")
         Cc, L, nh = desc.channels, desc.n_layers, desc.head_channels
-        need = (Cc * 9 + Cc) + L * (Cc * Cc * 9 + Cc) + (nh * Cc + nh)
+        IF = 3 if desc.in_frames == 3 else 1
+        need = (Cc * IF * 9 + Cc) + L * (Cc * Cc * 9 + Cc) + (nh * Cc + nh)
         if w.size != need:
             raise ValueError(f"weight blob has {w.size} floats, the net needs {need}")
         st = lib().smlm_create(C.byref(desc), w.ctypes.data, C.byref(self._h))

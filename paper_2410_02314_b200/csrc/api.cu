@@ -29,20 +29,6 @@ constexpr int kCounterWords = 2 + kSnapRing;
 
 thread_local std::string g_create_error;
 
-uint16_t f32_to_bf16_bits(float f) {  // round to nearest even
-  uint32_t u;
-  std::memcpy(&u, &f, 4);
-  if ((u & 0x7fffffffu) > 0x7f800000u) return (uint16_t)((u >> 16) | 0x40);
-  u += 0x7fffu + ((u >> 16) & 1u);
-  return (uint16_t)(u >> 16);
-}
-float bf16_round(float f) {
-  uint32_t u = (uint32_t)f32_to_bf16_bits(f) << 16;
-  float r;
-  std::memcpy(&r, &u, 4);
-  return r;
-}
-
 struct Layer {
   float* w_direct = nullptr;  // [9][C][C] (tap, ci, co)
   void* w_umma = nullptr;     // packed bf16 image for conv_umma
@@ -55,7 +41,9 @@ struct Layer {
 
 struct smlm_ctx {
   smlm_net_desc d{};
-  bool bf16 = false;
+  bool bf16 = false;  // 16-bit storage (bf16 or fp16)
+  int dt = ACT_F32;   // ActType of the maps
+  int in_frames = 1;
   bool use_umma = false;
   int n_sm = 0;
   int radius = 0;  // receptive-field radius of the maps: 1 + sum(dilations)
@@ -185,18 +173,18 @@ smlm_status run_trunk(smlm_ctx* c, const uint16_t* dev_frames, int frame_base, c
   if (have_logit) *have_logit = false;
   const size_t nl = c->layers.size();
   // K1 folded into the first trunk layer (STEM variant) when the tcgen05 path runs it
-  const bool fuse_stem = c->use_umma && c->fuse_stem && nl > 0 &&
+  const bool fuse_stem = c->use_umma && c->fuse_stem && nl > 0 && c->dt == ACT_BF16 && c->in_frames == 1 &&
                          conv_umma_supports(c->d.channels, c->layers[0].dil, true);
   cudaEvent_t te = nullptr;
   smlm_status tr = SMLM_OK;
   if (!fuse_stem || trunk_dump) {  // (the trunk dump wants a_0 itself)
     if ((tr = time_begin(c, SMLM_KERNEL_STEM, st, &te)) != SMLM_OK) return tr;
-    CK(c, launch_stem(c->bf16, dev_frames, frame_base, vs, s, np, c->w_stem, c->b_stem,
+    CK(c, launch_stem(c->dt, dev_frames, frame_base, vs, s, np, c->w_stem, c->b_stem,
                       c->d.stem_relu, c->act[0], st));
     c->launches++;
     if ((tr = time_end(c, te, st)) != SMLM_OK) return tr;
     if (trunk_dump) {
-      CK(c, launch_dump_act(c->bf16, c->act[0], s, trunk_dump, dump_view_stride, st));
+      CK(c, launch_dump_act(c->dt, c->act[0], s, trunk_dump, dump_view_stride, st));
       c->launches++;
     }
   }
@@ -222,14 +210,14 @@ smlm_status run_trunk(smlm_ctx* c, const uint16_t* dev_frames, int frame_base, c
         c->stem_args.np = np;
         c->stem_args.relu = c->d.stem_relu;
       }
-      cudaError_t e = launch_conv_umma(c->act[cur], c->act[cur ^ 1], s, L.dil, L.w_umma, L.lc,
+      cudaError_t e = launch_conv_umma(c->dt == ACT_F16, c->act[cur], c->act[cur ^ 1], s, L.dil, L.w_umma, L.lc,
                                        head ? &c->head_args : nullptr, stem ? &c->stem_args : nullptr,
                                        c->n_sm, st, err, sizeof err);
       if (head && have_logit) *have_logit = true;
       if (e != cudaSuccess)
         return fail(c, SMLM_ERR_CUDA, "conv_umma: %s %s", cudaGetErrorString(e), err);
     } else {
-      CK(c, launch_conv_direct(c->bf16, c->act[cur], c->act[cur ^ 1], s, L.dil, L.w_direct, L.bias, st));
+      CK(c, launch_conv_direct(c->dt, c->act[cur], c->act[cur ^ 1], s, L.dil, L.w_direct, L.bias, st));
     }
     c->launches++;
     if ((tr = time_end(c, e1, st)) != SMLM_OK) return tr;
@@ -237,7 +225,7 @@ smlm_status run_trunk(smlm_ctx* c, const uint16_t* dev_frames, int frame_base, c
     if (after_stem && fuse_stem && l == 0) CK(c, cudaEventRecord(after_stem, st));
     cur ^= 1;
     if (trunk_dump) {
-      CK(c, launch_dump_act(c->bf16, c->act[cur], s, trunk_dump + (l + 1) * dump_level_stride,
+      CK(c, launch_dump_act(c->dt, c->act[cur], s, trunk_dump + (l + 1) * dump_level_stride,
                             dump_view_stride, st));
       c->launches++;
     }
@@ -362,15 +350,19 @@ smlm_status smlm_create(const smlm_net_desc* desc, const void* weights, smlm_ctx
   if (C < 16 || C > 64 || C % 16) return fail(nullptr, SMLM_ERR_INVALID_ARG, "channels must be 16, 32, 48 or 64");
   if (L < 0 || L > SMLM_MAX_LAYERS) return fail(nullptr, SMLM_ERR_INVALID_ARG, "n_layers out of range");
   if (nh != 5 && nh != 6) return fail(nullptr, SMLM_ERR_INVALID_ARG, "head_channels must be 5 or 6");
-  if (desc->precision != SMLM_FP32 && desc->precision != SMLM_BF16)
+  if (desc->precision != SMLM_FP32 && desc->precision != SMLM_BF16 && desc->precision != SMLM_FP16)
     return fail(nullptr, SMLM_ERR_INVALID_ARG, "bad precision");
+  if (desc->in_frames != 0 && desc->in_frames != 1 && desc->in_frames != 3)
+    return fail(nullptr, SMLM_ERR_INVALID_ARG, "in_frames must be 1 or 3");
+  if (desc->tile_merge != SMLM_TILE_MERGE_NONE && desc->tile_merge != SMLM_TILE_MERGE_ROW)
+    return fail(nullptr, SMLM_ERR_INVALID_ARG, "bad tile_merge");
   if (desc->conv_impl < SMLM_CONV_AUTO || desc->conv_impl > SMLM_CONV_DIRECT)
     return fail(nullptr, SMLM_ERR_INVALID_ARG, "bad conv_impl");
   if (desc->precision == SMLM_FP32 && desc->conv_impl == SMLM_CONV_TCGEN05)
-    return fail(nullptr, SMLM_ERR_INVALID_ARG, "the tcgen05 kernel is bf16 only");
+    return fail(nullptr, SMLM_ERR_INVALID_ARG, "the tcgen05 kernel needs a 16-bit precision");
   for (int l = 0; l < L; ++l)
-    if (desc->dilations[l] < 1 || desc->dilations[l] > 8)
-      return fail(nullptr, SMLM_ERR_INVALID_ARG, "dilations must be in 1..8");
+    if (desc->dilations[l] < 1 || desc->dilations[l] > 16)
+      return fail(nullptr, SMLM_ERR_INVALID_ARG, "dilations must be in 1..16");
   if (!(desc->norm_scale > 0.0f)) return fail(nullptr, SMLM_ERR_INVALID_ARG, "norm_scale must be > 0");
   if (desc->tile < 0 || desc->micro_batch < 0 || desc->writeback_frames < 0)
     return fail(nullptr, SMLM_ERR_INVALID_ARG, "negative tile / micro_batch / writeback_frames");
@@ -390,7 +382,9 @@ smlm_status smlm_create(const smlm_net_desc* desc, const void* weights, smlm_ctx
   smlm_ctx* c = new (std::nothrow) smlm_ctx;
   if (!c) return fail(nullptr, SMLM_ERR_OOM, "host allocation failed");
   c->d = *desc;
-  c->bf16 = desc->precision == SMLM_BF16;
+  c->bf16 = desc->precision != SMLM_FP32;
+  c->dt = desc->precision == SMLM_BF16 ? ACT_BF16 : (desc->precision == SMLM_FP16 ? ACT_F16 : ACT_F32);
+  c->in_frames = desc->in_frames == 3 ? 3 : 1;
   c->use_umma = c->bf16 && desc->conv_impl != SMLM_CONV_DIRECT;
   c->fuse = desc->fusion != SMLM_FUSE_NONE;
   c->fuse_stem = desc->fusion == SMLM_FUSE_ALL;
@@ -407,15 +401,17 @@ smlm_status smlm_create(const smlm_net_desc* desc, const void* weights, smlm_ctx
   };
   auto body = [&]() -> smlm_status {
     const float* w = static_cast<const float*>(weights);
-    std::vector<float> tmp(9 * C);
+    const int IF = c->in_frames, T9 = 9 * IF;  // stem W[C][IF][3][3] -> [IF * 9][C] (channel, ky, kx) major
+    std::vector<float> tmp((size_t)T9 * C);
     for (int co = 0; co < C; ++co)
-      for (int t = 0; t < 9; ++t) tmp[t * C + co] = w[co * 9 + t];
+      for (int t = 0; t < T9; ++t) tmp[(size_t)t * C + co] = w[(size_t)co * T9 + t];
     if ((st = upload(tmp, &c->w_stem)) != SMLM_OK) return st;
-    for (int t = 0; t < 9; ++t)
-      for (int co = 0; co < C; ++co) c->stem_args.w[t][co] = tmp[t * C + co];
-    for (int co = 0; co < C; ++co) c->stem_args.b[co] = w[9 * C + co];
-    if ((st = upload(std::vector<float>(w + 9 * C, w + 10 * C), &c->b_stem)) != SMLM_OK) return st;
-    w += 10 * C;
+    if (IF == 1)
+      for (int t = 0; t < 9; ++t)
+        for (int co = 0; co < C; ++co) c->stem_args.w[t][co] = tmp[t * C + co];
+    for (int co = 0; co < C; ++co) c->stem_args.b[co] = w[T9 * C + co];
+    if ((st = upload(std::vector<float>(w + T9 * C, w + (T9 + 1) * C), &c->b_stem)) != SMLM_OK) return st;
+    w += (T9 + 1) * C;
     c->layers.resize(L);
     std::vector<float> wd((size_t)9 * C * C);
     std::vector<uint8_t> pack(c->use_umma ? umma_packed_weight_bytes(C) : 0);
@@ -426,14 +422,14 @@ smlm_status smlm_create(const smlm_net_desc* desc, const void* weights, smlm_ctx
         for (int ci = 0; ci < C; ++ci)
           for (int t = 0; t < 9; ++t) {
             float v = w[((size_t)co * C + ci) * 9 + t];
-            wd[((size_t)t * C + ci) * C + co] = c->bf16 ? bf16_round(v) : v;
+            wd[((size_t)t * C + ci) * C + co] = round_to_act(v, c->dt);
           }
       if ((st = upload(wd, &Ly.w_direct)) != SMLM_OK) return st;
       if ((st = upload(std::vector<float>(w + (size_t)9 * C * C, w + (size_t)9 * C * C + C), &Ly.bias)) != SMLM_OK)
         return st;
       for (int co = 0; co < C; ++co) Ly.lc.bias[co] = w[(size_t)9 * C * C + co];
       if (c->use_umma) {
-        umma_pack_weights_host(C, w, pack.data());
+        umma_pack_weights_host(C, w, pack.data(), c->dt == ACT_F16);
         CK(nullptr, cudaMalloc(&Ly.w_umma, pack.size()));
         CK(nullptr, cudaMemcpy(Ly.w_umma, pack.data(), pack.size(), cudaMemcpyHostToDevice));
       }
@@ -549,6 +545,7 @@ struct Call {
   HeadParams hp{};
   bool tiled = false;
   int tile = 0, halo = 0, mb = 0, F = 1;
+  int tile_w = 0;  // SMLM_TILE_MERGE_ROW: the frame width (one window per tile row), else 0
   std::vector<Range> ycls, xcls;
   smlm_emitter* out = nullptr;   // caller's list
   smlm_emitter* list = nullptr;  // where K3 appends (== out, or the ctx's device list)
@@ -609,9 +606,13 @@ smlm_status call_begin(Call& k, smlm_ctx* c, int64_t n, int32_t H, int32_t W, co
   k.tile = c->d.tile;
   k.tiled = k.tile > 0 && (k.tile < H || k.tile < W);
   k.halo = c->radius + 1;  // maps need `radius`; the 3x3 test reads one more pixel
+  // SMLM_TILE_MERGE_ROW: the cores of one tile row share one window (core = tile rows x W)
+  k.tile_w = (k.tiled && c->d.tile_merge == SMLM_TILE_MERGE_ROW && k.tile < H) ? W : 0;
+  if (k.tiled && c->d.tile_merge == SMLM_TILE_MERGE_ROW && k.tile >= H) k.tiled = false;  // one row of tiles = the frame
   if (k.tiled) {
     k.ycls = tile_classes(H, k.tile, k.halo);
-    k.xcls = tile_classes(W, k.tile, k.halo);
+    if (k.tile_w) k.xcls.push_back({0, 1, W});
+    else k.xcls = tile_classes(W, k.tile, k.halo);
   } else {
     k.ycls.push_back({0, 1, H});
     k.xcls.push_back({0, 1, W});
@@ -637,7 +638,7 @@ smlm_status call_begin(Call& k, smlm_ctx* c, int64_t n, int32_t H, int32_t W, co
 
   const size_t frame_elems = (size_t)H * W;
   if (host_frames && n > 0) {
-    size_t se = (size_t)k.F * frame_elems;
+    size_t se = (size_t)(k.F + (c->in_frames == 3 ? 2 : 0)) * frame_elems;  // + frames f0-1 and f0+nf
     if (se > c->slot_elems) {
       CK(c, cudaDeviceSynchronize());  // a previous call may still read the old slots
       if (c->slots) cudaFree(c->slots);
@@ -693,19 +694,26 @@ smlm_status call_frames(Call& k, const uint16_t* frames, int64_t f_first, int64_
       slot = (int)(k.chunk % kSlots);
       if (c->slot_used[slot]) CK(c, cudaStreamWaitEvent(c->copy_stream, c->ev_consumed[slot], 0));
       uint16_t* dst = c->slots + (size_t)slot * c->slot_elems;
-      CK(c, cudaMemcpyAsync(dst, frames + (size_t)(f0 - f_first) * frame_elems, (size_t)nf * frame_elems * 2,
+      // temporal context: the chunk's neighbours f0-1 and f0+nf travel with it (the call's
+      // frames are all in `frames`: smlm_localize_ring refuses in_frames = 3)
+      int64_t c0 = f0, c1 = f0 + nf;
+      if (c->in_frames == 3) {
+        c0 = std::max<int64_t>(f0 - 1, f_first);
+        c1 = std::min<int64_t>(f0 + nf + 1, f_first + n);
+      }
+      CK(c, cudaMemcpyAsync(dst, frames + (size_t)(c0 - f_first) * frame_elems, (size_t)(c1 - c0) * frame_elems * 2,
                             cudaMemcpyHostToDevice, c->copy_stream));
       CK(c, cudaEventRecord(c->ev_copied[slot], c->copy_stream));
       CK(c, cudaStreamWaitEvent(st, c->ev_copied[slot], 0));
       c->slot_used[slot] = true;
       dev_frames = dst;
-      frame_base = (int)f0;
+      frame_base = (int)c0;
     }
     // launch sets of this chunk
     struct Set { ViewSet vs; ActShape s; };
     std::vector<Set> sets;
     if (!k.tiled) {
-      ViewSet vs{(int)f0, H, W, 0, 0, 0, 1, 0, 1};
+      ViewSet vs{(int)f0, H, W, 0, 0, 0, 1, 0, 1, 0, c->in_frames, (int)k.n_total};
       sets.push_back({vs, ActShape{nf, C, H, W}});
     } else {
       for (auto& a : k.ycls)
@@ -717,7 +725,7 @@ smlm_status call_frames(Call& k, const uint16_t* frames, int64_t f_first, int64_
           for (int ty = a.t0; ty < a.t0 + a.n; ty += by)
             for (int tx = b.t0; tx < b.t0 + b.n; tx += bx) {
               int ny = std::min(by, a.t0 + a.n - ty), nx = std::min(bx, b.t0 + b.n - tx);
-              ViewSet vs{(int)f0, H, W, k.tile, k.halo, ty, ny, tx, nx};
+              ViewSet vs{(int)f0, H, W, k.tile, k.halo, ty, ny, tx, nx, k.tile_w, c->in_frames, (int)k.n_total};
               sets.push_back({vs, ActShape{nf * ny * nx, C, a.ext, b.ext}});
             }
         }
@@ -734,7 +742,7 @@ smlm_status call_frames(Call& k, const uint16_t* frames, int64_t f_first, int64_
       if (have_logit)
         CK(c, launch_post_logits(c->logit, c->cand, sets[si].s, sets[si].vs, k.hp, k.list, counter, k.capacity, st));
       else
-        CK(c, launch_head_post(c->bf16, c->act[res], sets[si].s, sets[si].vs, c->w_head, c->b_head, k.hp,
+        CK(c, launch_head_post(c->dt, c->act[res], sets[si].s, sets[si].vs, c->w_head, c->b_head, k.hp,
                                k.list, counter, k.capacity, st));
       c->launches++;
       if ((r = time_end(c, te, st)) != SMLM_OK) return r;
@@ -797,6 +805,8 @@ smlm_status smlm_localize_ring(smlm_ctx* c, smlm_ring* ring, const smlm_camera_p
   if (!c) return SMLM_ERR_INVALID_ARG;
   if (!ring) return fail(c, SMLM_ERR_INVALID_ARG, "NULL ring");
   if (!ring->pinned) return fail(c, SMLM_ERR_INVALID_ARG, "the ring is pageable (SMLM_RING_PAGEABLE is for tests)");
+  if (c->in_frames == 3)
+    return fail(c, SMLM_ERR_INVALID_ARG, "in_frames = 3 needs the whole stack (smlm_localize): ring chunks have no neighbours");
   ring_rewind(ring);
   Call k;
   smlm_status r = call_begin(k, c, ring->n_frames, ring->H, ring->W, cam, threshold, out, out_count, true,
@@ -845,14 +855,14 @@ smlm_status smlm_debug_forward_maps(smlm_ctx* c, const uint16_t* frames, int64_t
   }
   for (int64_t f0 = 0; f0 < n; f0 += mb) {
     int nf = (int)std::min<int64_t>(mb, n - f0);
-    ViewSet vs{(int)f0, H, W, 0, 0, 0, 1, 0, 1};
+    ViewSet vs{(int)f0, H, W, 0, 0, 0, 1, 0, 1, 0, c->in_frames, (int)n};
     ActShape s{nf, C, H, W};
     int res = 0;
     float* dump = trunk ? trunk + (size_t)f0 * (L + 1) * px * C : nullptr;
     r = run_trunk(c, frames, 0, vs, s, np, st, &res, dump, (size_t)(L + 1) * px * C, px * C, nullptr, false,
                   0.0f, nullptr);
     if (r != SMLM_OK) break;
-    cudaError_t e = launch_head_maps(c->bf16, c->act[res], s, c->w_head, c->b_head, nh,
+    cudaError_t e = launch_head_maps(c->dt, c->act[res], s, c->w_head, c->b_head, nh,
                                      maps + (size_t)f0 * nh * px, st);
     c->launches++;
     if (e != cudaSuccess) {

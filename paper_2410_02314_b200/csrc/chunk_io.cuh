@@ -1,7 +1,8 @@
 // 8-channel chunk load/store for the chunk-planar activation layout (smlm_internal.cuh).
-// bf16: one 16-byte vector per (pixel, chunk); float: two.
+// bf16 / fp16: one 16-byte vector per (pixel, chunk); float: two.
 #pragma once
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -43,6 +44,30 @@ struct Chunk<__nv_bfloat16> {
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
       __nv_bfloat162 h = __floats2bfloat162_rn(v[2 * i], v[2 * i + 1]);  // .x = low half
+      w[i] = *reinterpret_cast<uint32_t*>(&h);
+    }
+    reinterpret_cast<uint4*>(base)[idx] = make_uint4(w[0], w[1], w[2], w[3]);
+  }
+};
+
+template <>
+struct Chunk<__half> {
+  static constexpr int kBytes = 16;
+  __device__ static inline void load(const void* base, size_t idx, float v[8]) {
+    uint4 q = reinterpret_cast<const uint4*>(base)[idx];
+    const uint32_t w[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&w[i]));
+      v[2 * i] = f.x;
+      v[2 * i + 1] = f.y;
+    }
+  }
+  __device__ static inline void store(void* base, size_t idx, const float v[8]) {
+    uint32_t w[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      __half2 h = __floats2half2_rn(v[2 * i], v[2 * i + 1]);  // .x = low half
       w[i] = *reinterpret_cast<uint32_t*>(&h);
     }
     reinterpret_cast<uint4*>(base)[idx] = make_uint4(w[0], w[1], w[2], w[3]);

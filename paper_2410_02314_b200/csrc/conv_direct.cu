@@ -105,20 +105,27 @@ cudaError_t init_tc() {
 cudaError_t conv_direct_init(int C) {
   cudaError_t e;
   switch (C) {
-    case 16: e = init_tc<float, 16>(); if (e == cudaSuccess) e = init_tc<__nv_bfloat16, 16>(); break;
-    case 32: e = init_tc<float, 32>(); if (e == cudaSuccess) e = init_tc<__nv_bfloat16, 32>(); break;
-    case 48: e = init_tc<float, 48>(); if (e == cudaSuccess) e = init_tc<__nv_bfloat16, 48>(); break;
-    case 64: e = init_tc<float, 64>(); if (e == cudaSuccess) e = init_tc<__nv_bfloat16, 64>(); break;
+#define INIT3(CC)                                                     \
+  e = init_tc<float, CC>();                                           \
+  if (e == cudaSuccess) e = init_tc<__nv_bfloat16, CC>();             \
+  if (e == cudaSuccess) e = init_tc<__half, CC>();                    \
+  break;
+    case 16: INIT3(16)
+    case 32: INIT3(32)
+    case 48: INIT3(48)
+    case 64: INIT3(64)
+#undef INIT3
     default: e = cudaErrorInvalidValue;
   }
   return e;
 }
 
-cudaError_t launch_conv_direct(bool bf16, const void* in, void* out, ActShape s, int dil,
+cudaError_t launch_conv_direct(int dt, const void* in, void* out, ActShape s, int dil,
                                const float* w, const float* b, cudaStream_t st) {
   if (s.B <= 0) return cudaSuccess;
-  return bf16 ? launch_t<__nv_bfloat16>(in, out, s, dil, w, b, st)
-              : launch_t<float>(in, out, s, dil, w, b, st);
+  if (dt == ACT_BF16) return launch_t<__nv_bfloat16>(in, out, s, dil, w, b, st);
+  if (dt == ACT_F16) return launch_t<__half>(in, out, s, dil, w, b, st);
+  return launch_t<float>(in, out, s, dil, w, b, st);
 }
 
 }  // namespace smlm

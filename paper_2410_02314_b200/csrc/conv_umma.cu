@@ -42,6 +42,7 @@
 // shared memory as the UMMA "K-major, no swizzle" operand: core matrix = 8 pixels x 16 B,
 // contiguous, so a horizontal tap is a 16-byte-granular shift of the descriptor start address.
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 
 #include <cstdio>
@@ -68,9 +69,9 @@ constexpr int kTmemCols = 512;
 constexpr int kLaneCols = 256;  // TMEM columns reserved per lane (3C <= 192)
 constexpr int kMaxDevices = 64;
 constexpr int kLaneBars = 2 * kMaxStages + 2;  // mbarriers per lane (SmemLayout)
-constexpr int kMaxDilation = 8;
+constexpr int kMaxDilation = 16;  // the paper's dilation set is (2, 4, 8, 16)
 
-// zero source for the padded parts of a row segment: at most (127 + 8) pixels x 16 B
+// zero source for the padded parts of a row segment: at most (127 + 16) pixels x 16 B
 __device__ __align__(16) uint4 g_zeros[160];
 
 // ------------------------------------------------------------------------------ PTX wrappers
@@ -176,9 +177,35 @@ __device__ __forceinline__ uint64_t umma_desc(uint32_t addr, uint32_t lbo, uint3
   return (uint64_t)((addr >> 4) & 0x3FFFu) | ((uint64_t)((lbo >> 4) & 0x3FFFu) << 16) |
          ((uint64_t)((sbo >> 4) & 0x3FFFu) << 32) | (1ull << 46);
 }
-// instruction descriptor (cute::UMMA::InstrDescriptor), kind::f16: D fp32, A/B bf16, K-major
-__host__ __device__ constexpr uint32_t umma_idesc(int M, int N) {
-  return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
+// instruction descriptor (cute::UMMA::InstrDescriptor), kind::f16: D fp32, A/B bf16 (format 1)
+// or fp16 (format 0), K-major
+__host__ __device__ constexpr uint32_t umma_idesc(int M, int N, bool f16) {
+  return (1u << 4) | (f16 ? 0u : ((1u << 7) | (1u << 10))) | ((uint32_t)(N >> 3) << 17) |
+         ((uint32_t)(M >> 4) << 24);
+}
+
+// Two 16-bit activations in one 32-bit word (low half = even channel): bf16, or fp16 in the
+// F16 instantiation (smlm_net_desc.precision = SMLM_FP16: 11-bit mantissa,
+// same tensor rate).
+template <bool F16>
+__device__ __forceinline__ void unpack2(uint32_t w, float& lo, float& hi) {
+  if (F16) {
+    const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&w));
+    lo = f.x;
+    hi = f.y;
+  } else {
+    lo = __uint_as_float(w << 16);
+    hi = __uint_as_float(w & 0xffff0000u);
+  }
+}
+template <bool F16>
+__device__ __forceinline__ uint32_t pack2(float lo, float hi) {
+  if (F16) {
+    __half2 h = __floats2half2_rn(lo, hi);
+    return *reinterpret_cast<uint32_t*>(&h);
+  }
+  __nv_bfloat162 h = __floats2bfloat162_rn(lo, hi);
+  return *reinterpret_cast<uint32_t*>(&h);
 }
 
 // ------------------------------------------------------------------------------ work iterator
@@ -367,7 +394,7 @@ __host__ __device__ inline SmemLayout smem_layout(int C, int d, int nstage, bool
 // the detection logit o_p for every pixel, the other heads for pixels with o_p > lthr; the
 // activation map itself is not stored.
 // STEM: the layer is the first one; its input a_0 is computed in the kernel (see above).
-template <int C, bool HEAD, bool STEM>
+template <int C, bool HEAD, bool STEM, bool F16>
 __global__ void __launch_bounds__(kThreads, 1)
     conv_umma_kernel(const __nv_bfloat16* __restrict__ in, __nv_bfloat16* __restrict__ out, Geo geo,
                      const uint8_t* __restrict__ wpack, int nstage, const __grid_constant__ LayerConst lc,
@@ -521,7 +548,7 @@ __global__ void __launch_bounds__(kThreads, 1)
     const int ln = role >> 1;
     asm volatile("griddepcontrol.wait;" ::: "memory");
     mbar_wait(wbar, 0);
-    constexpr uint32_t idesc = umma_idesc(kTileM, 3 * C);
+    constexpr uint32_t idesc = umma_idesc(kTileM, 3 * C, F16);
     const uint32_t plane16 = (uint32_t)(kTileM + 2 * d);  // (bytes between channel chunks of A) / 16
     constexpr uint32_t wplane16 = 5u * C;                 // same for B
     // descriptor = {hi: SBO = 128 B, version 1; lo: LBO << 16 | start address >> 4}
@@ -828,13 +855,14 @@ __global__ void __launch_bounds__(kThreads, 1)
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
               const int c0 = (kc0 + kk) * 8 + 2 * i;
-              float r0 = __uint_as_float(rw[i] << 16), r1 = __uint_as_float(rw[i] & 0xffff0000u);
+              float r0, r1;
+              unpack2<F16>(rw[i], r0, r1);
               float v0 = r0 + fmaxf(__uint_as_float(acc[kk * 8 + 2 * i]) + lc.bias[c0], 0.0f);
               float v1 = r1 + fmaxf(__uint_as_float(acc[kk * 8 + 2 * i + 1]) + lc.bias[c0 + 1], 0.0f);
-              __nv_bfloat162 hb = __floats2bfloat162_rn(v0, v1);
-              ow[i] = *reinterpret_cast<uint32_t*>(&hb);
+              ow[i] = pack2<F16>(v0, v1);
               if (HEAD) {
-                const float a0 = __uint_as_float(ow[i] << 16), a1 = __uint_as_float(ow[i] & 0xffff0000u);
+                float a0, a1;
+                unpack2<F16>(ow[i], a0, a1);
 #pragma unroll
                 for (int h = 0; h < 6; ++h) hp[h] = fmaf(a0, ha.w[c0][h], hp[h]);
 #pragma unroll
@@ -911,7 +939,14 @@ uint16_t bf16_bits(float f) {
   return (uint16_t)(u >> 16);
 }
 
-template <int C, bool HEAD, bool STEM>
+uint16_t f16_bits(float f) {
+  const __half h = __float2half_rn(f);
+  uint16_t u;
+  std::memcpy(&u, &h, 2);
+  return u;
+}
+
+template <int C, bool HEAD, bool STEM, bool F16>
 cudaError_t launch_chs(const void* in, void* out, Geo geo, const void* wpack, const LayerConst& lc, int nstage,
                        int grid, size_t smem, const HeadArgs& ha, const StemArgs& sa, cudaStream_t st) {
   static bool attr_done[kMaxDevices] = {};  // the attribute is per device
@@ -919,7 +954,7 @@ cudaError_t launch_chs(const void* in, void* out, Geo geo, const void* wpack, co
   cudaGetDevice(&dev);
   if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
   if (!attr_done[dev]) {
-    cudaError_t e = cudaFuncSetAttribute(conv_umma_kernel<C, HEAD, STEM>,
+    cudaError_t e = cudaFuncSetAttribute(conv_umma_kernel<C, HEAD, STEM, F16>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) return e;
     attr_done[dev] = true;
@@ -934,18 +969,23 @@ cudaError_t launch_chs(const void* in, void* out, Geo geo, const void* wpack, co
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, conv_umma_kernel<C, HEAD, STEM>, (const __nv_bfloat16*)in,
+  return cudaLaunchKernelEx(&cfg, conv_umma_kernel<C, HEAD, STEM, F16>, (const __nv_bfloat16*)in,
                             (__nv_bfloat16*)out, geo, (const uint8_t*)wpack, nstage, lc, ha, sa);
 }
 template <int C>
-cudaError_t launch_c(const void* in, void* out, Geo geo, const void* wpack, const LayerConst& lc, int nstage,
-                     int grid, size_t smem, const HeadArgs* ha, const StemArgs* sa, cudaStream_t st) {
+cudaError_t launch_c(bool f16, const void* in, void* out, Geo geo, const void* wpack, const LayerConst& lc,
+                     int nstage, int grid, size_t smem, const HeadArgs* ha, const StemArgs* sa, cudaStream_t st) {
   static const HeadArgs h0{};
   static const StemArgs s0{};
-  if (ha && sa) return launch_chs<C, true, true>(in, out, geo, wpack, lc, nstage, grid, smem, *ha, *sa, st);
-  if (ha) return launch_chs<C, true, false>(in, out, geo, wpack, lc, nstage, grid, smem, *ha, s0, st);
-  if (sa) return launch_chs<C, false, true>(in, out, geo, wpack, lc, nstage, grid, smem, h0, *sa, st);
-  return launch_chs<C, false, false>(in, out, geo, wpack, lc, nstage, grid, smem, h0, s0, st);
+  if (f16) {  // the STEM variant exists in bf16 only (api.cu keeps K1 a kernel of its own in fp16)
+    if (sa) return cudaErrorInvalidValue;
+    if (ha) return launch_chs<C, true, false, true>(in, out, geo, wpack, lc, nstage, grid, smem, *ha, s0, st);
+    return launch_chs<C, false, false, true>(in, out, geo, wpack, lc, nstage, grid, smem, h0, s0, st);
+  }
+  if (ha && sa) return launch_chs<C, true, true, false>(in, out, geo, wpack, lc, nstage, grid, smem, *ha, *sa, st);
+  if (ha) return launch_chs<C, true, false, false>(in, out, geo, wpack, lc, nstage, grid, smem, *ha, s0, st);
+  if (sa) return launch_chs<C, false, true, false>(in, out, geo, wpack, lc, nstage, grid, smem, h0, *sa, st);
+  return launch_chs<C, false, false, false>(in, out, geo, wpack, lc, nstage, grid, smem, h0, s0, st);
 }
 
 // stages: as many as fit next to the resident weights (<= kMaxStages; >= 2 for any overlap of
@@ -963,7 +1003,17 @@ size_t umma_packed_weight_bytes(int C) { return (size_t)30 * C * C; }
 
 // Shared-memory image of one layer's weights: for kx, input chunk kc: 5C rows of 16 B
 // (8 input channels), rows = output channels of ky = 1, 0, 2, 1, 0.
-void umma_pack_weights_host(int C, const float* w /*[C][C][3][3]*/, void* dst) {
+float round_to_act(float v, int dt) {
+  uint32_t u;
+  if (dt == ACT_BF16) u = (uint32_t)bf16_bits(v) << 16;
+  else if (dt == ACT_F16) return __half2float(__float2half_rn(v));
+  else return v;
+  float r;
+  std::memcpy(&r, &u, 4);
+  return r;
+}
+
+void umma_pack_weights_host(int C, const float* w /*[C][C][3][3]*/, void* dst, bool f16) {
   static const int ky_seq[5] = {1, 0, 2, 1, 0};
   uint16_t* o = static_cast<uint16_t*>(dst);
   for (int kx = 0; kx < 3; ++kx)
@@ -972,8 +1022,8 @@ void umma_pack_weights_host(int C, const float* w /*[C][C][3][3]*/, void* dst) {
         const int ky = ky_seq[n / C], co = n % C;
         for (int j = 0; j < 8; ++j) {
           const int ci = kc * 8 + j;
-          o[(((size_t)(kx * (C / 8) + kc) * 5 * C) + n) * 8 + j] =
-              bf16_bits(w[(((size_t)co * C + ci) * 3 + ky) * 3 + kx]);
+          const float v = w[(((size_t)co * C + ci) * 3 + ky) * 3 + kx];
+          o[(((size_t)(kx * (C / 8) + kc) * 5 * C) + n) * 8 + j] = f16 ? f16_bits(v) : bf16_bits(v);
         }
       }
 }
@@ -982,7 +1032,7 @@ bool conv_umma_supports(int C, int dil, bool stem) {
   return C >= 16 && C <= 64 && C % 16 == 0 && dil >= 1 && dil <= kMaxDilation && pick_stages(C, dil, stem, true) > 0;
 }
 
-cudaError_t launch_conv_umma(const void* in, void* out, ActShape s, int dil, const void* wpack,
+cudaError_t launch_conv_umma(bool f16, const void* in, void* out, ActShape s, int dil, const void* wpack,
                              const LayerConst& lc, const HeadArgs* head, const StemArgs* stem, int n_sm,
                              cudaStream_t st, char* err, size_t errlen) {
   if (dil < 1 || dil > kMaxDilation || s.C % 16 || s.C < 16 || s.C > 64) {
@@ -1009,10 +1059,10 @@ cudaError_t launch_conv_umma(const void* in, void* out, ActShape s, int dil, con
   int grid = (int)(want < 1 ? 1 : (want > n_sm ? n_sm : want));
   const size_t smem = L.total + 1024;
   switch (s.C) {
-    case 16: return launch_c<16>(in, out, geo, wpack, lc, nstage, grid, smem, head, stem, st);
-    case 32: return launch_c<32>(in, out, geo, wpack, lc, nstage, grid, smem, head, stem, st);
-    case 48: return launch_c<48>(in, out, geo, wpack, lc, nstage, grid, smem, head, stem, st);
-    case 64: return launch_c<64>(in, out, geo, wpack, lc, nstage, grid, smem, head, stem, st);
+    case 16: return launch_c<16>(f16, in, out, geo, wpack, lc, nstage, grid, smem, head, stem, st);
+    case 32: return launch_c<32>(f16, in, out, geo, wpack, lc, nstage, grid, smem, head, stem, st);
+    case 48: return launch_c<48>(f16, in, out, geo, wpack, lc, nstage, grid, smem, head, stem, st);
+    case 64: return launch_c<64>(f16, in, out, geo, wpack, lc, nstage, grid, smem, head, stem, st);
   }
   return cudaErrorInvalidValue;
 }

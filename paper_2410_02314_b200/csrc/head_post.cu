@@ -339,13 +339,15 @@ cudaError_t head_maps_tc(const void* act, ActShape s, const float* w, const floa
 
 }  // namespace
 
-cudaError_t launch_head_post(bool bf16, const void* act, ActShape s, ViewSet vs,
+cudaError_t launch_head_post(int dt, const void* act, ActShape s, ViewSet vs,
                              const float* w_head, const float* b_head, HeadParams hp,
                              smlm_emitter* out, unsigned long long* counter,
                              unsigned long long capacity, cudaStream_t st) {
   if (s.B <= 0) return cudaSuccess;
-  if (bf16) {
+  if (dt == ACT_BF16) {
     SMLM_DISPATCH_C(__nv_bfloat16, head_post_tc, act, s, vs, w_head, b_head, hp, out, counter, capacity, st)
+  } else if (dt == ACT_F16) {
+    SMLM_DISPATCH_C(__half, head_post_tc, act, s, vs, w_head, b_head, hp, out, counter, capacity, st)
   } else {
     SMLM_DISPATCH_C(float, head_post_tc, act, s, vs, w_head, b_head, hp, out, counter, capacity, st)
   }
@@ -360,22 +362,26 @@ cudaError_t launch_post_logits(const float* logit, const float* cand, ActShape s
   return cudaGetLastError();
 }
 
-cudaError_t launch_head_maps(bool bf16, const void* act, ActShape s, const float* w_head,
+cudaError_t launch_head_maps(int dt, const void* act, ActShape s, const float* w_head,
                              const float* b_head, int n_h, float* maps, cudaStream_t st) {
   if (s.B <= 0) return cudaSuccess;
-  if (bf16) {
+  if (dt == ACT_BF16) {
     SMLM_DISPATCH_C(__nv_bfloat16, head_maps_tc, act, s, w_head, b_head, n_h, maps, st)
+  } else if (dt == ACT_F16) {
+    SMLM_DISPATCH_C(__half, head_maps_tc, act, s, w_head, b_head, n_h, maps, st)
   } else {
     SMLM_DISPATCH_C(float, head_maps_tc, act, s, w_head, b_head, n_h, maps, st)
   }
 }
 
-cudaError_t launch_dump_act(bool bf16, const void* act, ActShape s, float* dst, size_t view_stride,
+cudaError_t launch_dump_act(int dt, const void* act, ActShape s, float* dst, size_t view_stride,
                             cudaStream_t st) {
   if (s.B <= 0) return cudaSuccess;
   dim3 grid((s.W + NT - 1) / NT, s.H, s.B);
-  if (bf16)
+  if (dt == ACT_BF16)
     dump_act_kernel<__nv_bfloat16><<<grid, NT, 0, st>>>((const __nv_bfloat16*)act, s, dst, view_stride);
+  else if (dt == ACT_F16)
+    dump_act_kernel<__half><<<grid, NT, 0, st>>>((const __half*)act, s, dst, view_stride);
   else
     dump_act_kernel<float><<<grid, NT, 0, st>>>((const float*)act, s, dst, view_stride);
   return cudaGetLastError();

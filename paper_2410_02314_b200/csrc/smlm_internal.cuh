@@ -37,7 +37,14 @@ struct ViewSet {
   int tile;          // 0: whole frames
   int halo;          // tile mode: window = core +- halo, clipped to the frame
   int ty0, ny, tx0, nx;
+  int tile_w;        // core width (0: = tile).  SMLM_TILE_MERGE_ROW sets it to the frame width: the
+                     // tiles of one tile row share one window and their x halos are computed once
+  int in_frames;     // 3: the stem reads frames f-1, f, f+1 (0 / 1: frame f only)
+  int n_total;       // frames of the call: the clamp bound of the temporal context
 };
+
+// Storage type of the activation maps (smlm_net_desc.precision).
+enum ActType { ACT_F32 = 0, ACT_BF16 = 1, ACT_F16 = 2 };
 
 struct View {
   int frame;
@@ -58,9 +65,10 @@ __host__ __device__ inline View view_of(const ViewSet& vs, int v, int Hw, int Ww
   int per = vs.ny * vs.nx;
   int f = v / per, t = v - f * per;
   int ty = vs.ty0 + t / vs.nx, tx = vs.tx0 + t % vs.nx;
-  int y0 = ty * vs.tile, x0 = tx * vs.tile;
+  int tw = vs.tile_w > 0 ? vs.tile_w : vs.tile;
+  int y0 = ty * vs.tile, x0 = tx * tw;
   int y1 = y0 + vs.tile < vs.Hf ? y0 + vs.tile : vs.Hf;
-  int x1 = x0 + vs.tile < vs.Wf ? x0 + vs.tile : vs.Wf;
+  int x1 = x0 + tw < vs.Wf ? x0 + tw : vs.Wf;
   r.frame = vs.frame0 + f;
   r.wy0 = y0 - vs.halo > 0 ? y0 - vs.halo : 0;
   r.wx0 = x0 - vs.halo > 0 ? x0 - vs.halo : 0;
@@ -88,20 +96,21 @@ struct NormParams {
 
 // K1: uint16 unpack + normalise + 3x3 stem conv (+ReLU) -> act.
 // frames: device u16, frame f of the call at frames + (f - frame_base) * Hf * Wf.
-cudaError_t launch_stem(bool bf16, const uint16_t* frames, int frame_base, ViewSet vs, ActShape s,
-                        NormParams np, const float* w_stem /*[9][C]*/, const float* b_stem,
+cudaError_t launch_stem(int dt, const uint16_t* frames, int frame_base, ViewSet vs, ActShape s,
+                        NormParams np, const float* w_stem /*[in_frames * 9][C]*/, const float* b_stem,
                         int relu, void* act, cudaStream_t st);
 
-// K2' reference trunk layer on CUDA cores (fp32 math; storage float or bf16).
-// w: [9][C_in][C_out] float (already rounded to bf16 values in bf16 mode).
-cudaError_t launch_conv_direct(bool bf16, const void* in, void* out, ActShape s, int dil,
+// K2' reference trunk layer on CUDA cores (fp32 math; storage float, bf16 or fp16).
+// w: [9][C_in][C_out] float (already rounded to the storage type's values in the 16-bit modes).
+cudaError_t launch_conv_direct(int dt, const void* in, void* out, ActShape s, int dil,
                                const float* w, const float* b, cudaStream_t st);
 cudaError_t conv_direct_init(int C);  // opt in to the shared memory the kernel needs
 
-// K2 trunk layer on tcgen05 tensor cores (bf16 storage, fp32 accumulate in TMEM).
+// K2 trunk layer on tcgen05 tensor cores (bf16 or fp16 storage, fp32 accumulate in TMEM).
 size_t umma_packed_weight_bytes(int C);
-// w_oihw [C][C][3][3] fp32 -> the kernel's shared-memory image (bf16, RNE), host side.
-void umma_pack_weights_host(int C, const float* w_oihw, void* dst);
+// w_oihw [C][C][3][3] fp32 -> the kernel's shared-memory image (bf16 or fp16, RNE), host side.
+void umma_pack_weights_host(int C, const float* w_oihw, void* dst, bool f16);
+float round_to_act(float v, int dt);  // host: RNE to the storage type's value set
 // STEM variant (first layer, K1 folded in): a_0 is computed in the kernel from the frames.
 // The per-layer constants travel as kernel parameters: parameters live in constant memory,
 // so a weight with a compile-time index is a free operand of the FMA that uses it (no
@@ -133,12 +142,12 @@ struct HeadArgs {
 bool conv_umma_supports(int C, int dil, bool stem);
 // head != nullptr: last layer, HEAD variant (`out` is not written).  stem != nullptr: first
 // layer, STEM variant (`in` is not read).
-cudaError_t launch_conv_umma(const void* in, void* out, ActShape s, int dil, const void* wpack,
+cudaError_t launch_conv_umma(bool f16, const void* in, void* out, ActShape s, int dil, const void* wpack,
                              const LayerConst& lc, const HeadArgs* head, const StemArgs* stem, int n_sm,
                              cudaStream_t st, char* err, size_t errlen);
 
 // K3: 1x1 heads + threshold + 3x3 NMS + decode + warp-aggregated compaction.
-cudaError_t launch_head_post(bool bf16, const void* act, ActShape s, ViewSet vs,
+cudaError_t launch_head_post(int dt, const void* act, ActShape s, ViewSet vs,
                              const float* w_head /*[n_h][C]*/, const float* b_head, HeadParams hp,
                              smlm_emitter* out, unsigned long long* counter,
                              unsigned long long capacity, cudaStream_t st);
@@ -150,10 +159,10 @@ cudaError_t launch_post_logits(const float* logit, const float* cand, ActShape s
                                unsigned long long capacity, cudaStream_t st);
 
 // debug: heads only -> fp32 maps [B][n_h][H][W] (pre-activation)
-cudaError_t launch_head_maps(bool bf16, const void* act, ActShape s, const float* w_head,
+cudaError_t launch_head_maps(int dt, const void* act, ActShape s, const float* w_head,
                              const float* b_head, int n_h, float* maps, cudaStream_t st);
 // debug: act -> float dst[b * view_stride + (y*W + x)*C + c]
-cudaError_t launch_dump_act(bool bf16, const void* act, ActShape s, float* dst, size_t view_stride,
+cudaError_t launch_dump_act(int dt, const void* act, ActShape s, float* dst, size_t view_stride,
                             cudaStream_t st);
 // debug: detection + decode on caller maps [n][n_h][H][W]
 cudaError_t launch_post_from_maps(const float* maps, int n, int H, int W, HeadParams hp,

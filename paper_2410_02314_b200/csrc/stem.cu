@@ -1,4 +1,4 @@
-// K1: uint16 unpack + offset/gain normalisation + 3x3 stem convolution (1 -> C) (+ReLU),
+// K1: uint16 unpack + offset/gain normalisation + 3x3 stem convolution (IN -> C) (+ReLU),
 // fused (BASELINE.json north_star (a); smlm.h: xhat = ((adu - offset)/gain)/norm_scale,
 // a0 = act(conv3x3(xhat; W0) + b0), zero padding 1 at the FRAME border).
 //
@@ -6,6 +6,8 @@
 // C channels; a warp covers 32 consecutive pixels of a row per store, so each store is one
 // dense 512 B run in the chunk-planar layout.  The normalised (TY+2) x (TX+2) input patch is staged in
 // shared memory once per block (the divisions happen once per pixel, not once per tap).
+// IN = 3 (smlm_net_desc.in_frames): the input channels are the frames f-1, f, f+1 of the
+// call, indices clamped to [0, n_total - 1]; taps are accumulated in (channel, ky, kx) order.
 #include "chunk_io.cuh"
 #include "smlm_internal.cuh"
 
@@ -27,17 +29,17 @@ __device__ __forceinline__ unsigned long long ffma2(unsigned long long a, unsign
 
 // Persistent blocks: tile t = (view, row, 128-px segment); warp w of block j takes tiles
 // (j * NW + w), + gridDim.x * NW, ...  With 5 blocks per SM the tail is one row-tile.
-template <typename T, int C>
+template <typename T, int C, int IN>
 __global__ void __launch_bounds__(32 * NW)
     stem_kernel(const uint16_t* __restrict__ frames, int frame_base, ViewSet vs, ActShape s,
-                NormParams np, const float* __restrict__ w /*[9][C]*/,
+                NormParams np, const float* __restrict__ w /*[IN * 9][C]*/,
                 const float* __restrict__ bias, int relu, T* __restrict__ act) {
-  __shared__ float xs[NW][3][TX + 2];
-  __shared__ __align__(16) float2 ws2[9][C];  // every weight twice: the broadcast operand of fma.rn.f32x2
+  __shared__ float xs[NW][3 * IN][TX + 2];
+  __shared__ __align__(16) float2 ws2[9 * IN][C];  // every weight twice: the broadcast operand of fma.rn.f32x2
   __shared__ __align__(16) float bs[C];
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  for (int i = tid; i < 9 * C; i += 32 * NW) ws2[i / C][i % C] = make_float2(w[i], w[i]);
+  for (int i = tid; i < 9 * IN * C; i += 32 * NW) ws2[i / C][i % C] = make_float2(w[i], w[i]);
   for (int i = tid; i < C; i += 32 * NW) bs[i] = bias[i];
   __syncthreads();
 
@@ -50,29 +52,37 @@ __global__ void __launch_bounds__(32 * NW)
     const int y = (int)(ty % s.H), b = (int)(ty / s.H);
     const int x0 = seg * TX;
     const View v = view_of(vs, b, s.H, s.W);
-    const uint16_t* frame = frames + (size_t)(v.frame - frame_base) * vs.Hf * vs.Wf;
-    // all loads of the 3 x 130 patch first (independent, one round trip), then the arithmetic
-    float adu[NLD], om[NLD], gm[NLD];
-    bool ok[NLD];
-#pragma unroll
-    for (int r = 0; r < NLD; ++r) {
-      const int i = lane + r * 32;
-      const int ly = i / (TX + 2), lx = i - ly * (TX + 2);
-      const int fy = v.wy0 + y + ly - 1, fx = v.wx0 + x0 + lx - 1;  // frame coordinates
-      ok[r] = i < PATCH && fy >= 0 && fy < vs.Hf && fx >= 0 && fx < vs.Wf;
-      const size_t q = ok[r] ? (size_t)fy * vs.Wf + fx : 0;
-      adu[r] = ok[r] ? (float)__ldg(frame + q) : 0.0f;
-      om[r] = (ok[r] && np.offset_map) ? __ldg(np.offset_map + q) : np.offset;
-      gm[r] = (ok[r] && np.offset_map) ? __ldg(np.gain_map + q) : np.gain;
-    }
     __syncwarp();  // the previous tile's reads of xs[warp] are done
 #pragma unroll
-    for (int r = 0; r < NLD; ++r) {
-      const int i = lane + r * 32;
-      if (i >= PATCH) continue;
-      float xn = 0.0f;
-      if (ok[r]) xn = ((adu[r] - om[r]) / gm[r]) / np.norm_scale;  // the oracle's operation order (G5)
-      xs[warp][i / (TX + 2)][i % (TX + 2)] = xn;
+    for (int ch = 0; ch < IN; ++ch) {
+      int g = v.frame;
+      if (IN == 3) {  // temporal context: frames f-1, f, f+1, clamped to the call
+        g += ch - 1;
+        g = g < 0 ? 0 : (g > vs.n_total - 1 ? vs.n_total - 1 : g);
+      }
+      const uint16_t* frame = frames + (size_t)(g - frame_base) * vs.Hf * vs.Wf;
+      // all loads of the 3 x 130 patch first (independent, one round trip), then the arithmetic
+      float adu[NLD], om[NLD], gm[NLD];
+      bool ok[NLD];
+#pragma unroll
+      for (int r = 0; r < NLD; ++r) {
+        const int i = lane + r * 32;
+        const int ly = i / (TX + 2), lx = i - ly * (TX + 2);
+        const int fy = v.wy0 + y + ly - 1, fx = v.wx0 + x0 + lx - 1;  // frame coordinates
+        ok[r] = i < PATCH && fy >= 0 && fy < vs.Hf && fx >= 0 && fx < vs.Wf;
+        const size_t q = ok[r] ? (size_t)fy * vs.Wf + fx : 0;
+        adu[r] = ok[r] ? (float)__ldg(frame + q) : 0.0f;
+        om[r] = (ok[r] && np.offset_map) ? __ldg(np.offset_map + q) : np.offset;
+        gm[r] = (ok[r] && np.offset_map) ? __ldg(np.gain_map + q) : np.gain;
+      }
+#pragma unroll
+      for (int r = 0; r < NLD; ++r) {
+        const int i = lane + r * 32;
+        if (i >= PATCH) continue;
+        float xn = 0.0f;
+        if (ok[r]) xn = ((adu[r] - om[r]) / gm[r]) / np.norm_scale;  // the oracle's operation order (G5)
+        xs[warp][ch * 3 + i / (TX + 2)][i % (TX + 2)] = xn;
+      }
     }
     __syncwarp();
 
@@ -80,11 +90,11 @@ __global__ void __launch_bounds__(32 * NW)
     // fma.rn.f32x2 (two independent IEEE fp32 FMAs, same bits as fmaf) updates one channel of
     // a pair, which halves the FMA instruction count of this issue-bound loop; every store of
     // the warp is one dense 512-byte run.
-    unsigned long long xp[PX / 2][9];
+    unsigned long long xp[PX / 2][9 * IN];
 #pragma unroll
     for (int pp = 0; pp < PX / 2; ++pp)
 #pragma unroll
-      for (int ky = 0; ky < 3; ++ky)
+      for (int ky = 0; ky < 3 * IN; ++ky)  // (channel, ky) rows of the patch
 #pragma unroll
         for (int kx = 0; kx < 3; ++kx)
           xp[pp][ky * 3 + kx] = pack2(xs[warp][ky][lane + 64 * pp + kx], xs[warp][ky][lane + 64 * pp + 32 + kx]);
@@ -99,7 +109,7 @@ __global__ void __launch_bounds__(32 * NW)
         for (int pp = 0; pp < PX / 2; ++pp) acc[pp][c] = pack2(bv, bv);
       }
 #pragma unroll
-      for (int tp = 0; tp < 9; ++tp)
+      for (int tp = 0; tp < 9 * IN; ++tp)
 #pragma unroll
         for (int c = 0; c < 8; c += 2) {
           const ulonglong2 wv = *reinterpret_cast<const ulonglong2*>(&ws2[tp][k * 8 + c]);
@@ -126,9 +136,9 @@ __global__ void __launch_bounds__(32 * NW)
   }
 }
 
-template <typename T, int C>
-cudaError_t launch_tc(const uint16_t* frames, int frame_base, ViewSet vs, ActShape s, NormParams np,
-                      const float* w, const float* b, int relu, void* act, cudaStream_t st) {
+template <typename T, int C, int IN>
+cudaError_t launch_tci(const uint16_t* frames, int frame_base, ViewSet vs, ActShape s, NormParams np,
+                       const float* w, const float* b, int relu, void* act, cudaStream_t st) {
   static int waves[64] = {};  // resident blocks per device (occupancy is a per-device fact)
   int dev = 0;
   cudaGetDevice(&dev);
@@ -136,15 +146,22 @@ cudaError_t launch_tc(const uint16_t* frames, int frame_base, ViewSet vs, ActSha
   if (!waves[dev]) {
     int n_sm = 0, per_sm = 0;
     cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, stem_kernel<T, C>, 32 * NW, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, stem_kernel<T, C, IN>, 32 * NW, 0);
     waves[dev] = n_sm * (per_sm > 0 ? per_sm : 1);
   }
   const int blocks_per_wave = waves[dev];
   const long long ntiles = (long long)s.B * s.H * ((s.W + TX - 1) / TX);
   const long long want = (ntiles + NW - 1) / NW;
   const int grid = (int)(want < blocks_per_wave ? want : blocks_per_wave);
-  stem_kernel<T, C><<<grid, 32 * NW, 0, st>>>(frames, frame_base, vs, s, np, w, b, relu, (T*)act);
+  stem_kernel<T, C, IN><<<grid, 32 * NW, 0, st>>>(frames, frame_base, vs, s, np, w, b, relu, (T*)act);
   return cudaGetLastError();
+}
+
+template <typename T, int C>
+cudaError_t launch_tc(const uint16_t* frames, int frame_base, ViewSet vs, ActShape s, NormParams np,
+                      const float* w, const float* b, int relu, void* act, cudaStream_t st) {
+  if (vs.in_frames == 3) return launch_tci<T, C, 3>(frames, frame_base, vs, s, np, w, b, relu, act, st);
+  return launch_tci<T, C, 1>(frames, frame_base, vs, s, np, w, b, relu, act, st);
 }
 
 template <typename T>
@@ -161,12 +178,13 @@ cudaError_t launch_t(const uint16_t* frames, int frame_base, ViewSet vs, ActShap
 
 }  // namespace
 
-cudaError_t launch_stem(bool bf16, const uint16_t* frames, int frame_base, ViewSet vs, ActShape s,
+cudaError_t launch_stem(int dt, const uint16_t* frames, int frame_base, ViewSet vs, ActShape s,
                         NormParams np, const float* w_stem, const float* b_stem, int relu,
                         void* act, cudaStream_t st) {
   if (s.B <= 0) return cudaSuccess;
-  return bf16 ? launch_t<__nv_bfloat16>(frames, frame_base, vs, s, np, w_stem, b_stem, relu, act, st)
-              : launch_t<float>(frames, frame_base, vs, s, np, w_stem, b_stem, relu, act, st);
+  if (dt == ACT_BF16) return launch_t<__nv_bfloat16>(frames, frame_base, vs, s, np, w_stem, b_stem, relu, act, st);
+  if (dt == ACT_F16) return launch_t<__half>(frames, frame_base, vs, s, np, w_stem, b_stem, relu, act, st);
+  return launch_t<float>(frames, frame_base, vs, s, np, w_stem, b_stem, relu, act, st);
 }
 
 }  // namespace smlm

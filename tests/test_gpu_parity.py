@@ -374,7 +374,7 @@ def test_edge_cases_empty_overflow_pageable_threshold():
             loc.localize(torch.from_numpy(fs.frames.copy()), loc.camera(), 0.3, buf, 10)
         assert ei.value.status == P.ERR_INVALID_ARG
     # bad descriptors
-    for kw in (dict(channels=24), dict(head_channels=4), dict(dilations=(9,)), dict(precision=7)):
+    for kw in (dict(channels=24), dict(head_channels=4), dict(dilations=(17,)), dict(precision=7), dict(in_frames=2), dict(tile_merge=5)):
         base = dict(channels=16, dilations=(1,), head_channels=5, precision=P.FP32)
         base.update(kw)
         d = P.make_desc(**base)
