@@ -6,7 +6,12 @@ from .binding import (ABI_VERSION, BF16, CONV_AUTO, CONV_DIRECT, CONV_TCGEN05, E
                       EXPORTS, FP16, FP32, TILE_MERGE_NONE, TILE_MERGE_ROW, FUSE_ALL, FUSE_AUTO, FUSE_NONE, KERNEL_CONV, KERNEL_POST, KERNEL_STEM, OK, CameraParams, Localizer, NetDesc, Ring, SmlmError,
                       desc_from_spec, emitters_to_numpy, lib, make_desc)
 
-__all__ = ["ABI_VERSION", "BF16", "CONV_AUTO", "CONV_DIRECT", "CONV_TCGEN05", "EMITTER_DTYPE",
+from .dloc_binding import (DLOC_EMITTER_DTYPE, DLOC_EXPORTS, DLOC_HEADS, DlocDesc, DlocLocalizer, dloc_desc,
+                           dloc_desc_from_spec, dloc_emitters_to_numpy)
+
+__all__ = ["DLOC_EMITTER_DTYPE", "DLOC_EXPORTS", "DLOC_HEADS", "DlocDesc", "DlocLocalizer", "dloc_desc",
+           "dloc_desc_from_spec", "dloc_emitters_to_numpy",
+           "ABI_VERSION", "BF16", "CONV_AUTO", "CONV_DIRECT", "CONV_TCGEN05", "EMITTER_DTYPE",
            "ERR_CUDA", "ERR_INVALID_ARG", "ERR_OOM", "ERR_OVERFLOW", "ERR_UNSUPPORTED_DEVICE",
            "EXPORTS", "FP16", "FP32", "TILE_MERGE_NONE", "TILE_MERGE_ROW", "FUSE_ALL", "FUSE_AUTO", "FUSE_NONE", "KERNEL_CONV", "KERNEL_POST", "KERNEL_STEM", "OK", "CameraParams", "Localizer", "NetDesc", "Ring", "SmlmError",
            "desc_from_spec", "emitters_to_numpy", "lib", "make_desc"]

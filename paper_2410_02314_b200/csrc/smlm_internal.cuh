@@ -21,9 +21,11 @@ namespace smlm {
 // ---------------------------------------------------------------------------------------
 struct ActShape {
   int B, C, H, W;
+  int CT = 0;  // channels per view of the buffer the map lives in (0: = C).  > C when the map is a
+               // slice of a concatenation buffer (dloc.cu): the planes of a view stay contiguous
   __host__ __device__ size_t elems() const { return (size_t)B * C * H * W; }
   __host__ __device__ size_t chunk_index(int b, int k, int y, int x) const {
-    return ((((size_t)b * (C >> 3) + k) * H + y) * W + x);
+    return ((((size_t)b * ((CT > 0 ? CT : C) >> 3) + k) * H + y) * W + x);
   }
 };
 

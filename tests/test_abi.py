@@ -33,6 +33,37 @@ def test_library_exports_every_declared_function():
     assert sorted(binding.EXPORTS) == names, "binding.EXPORTS and smlm.h disagree"
 
 
+def test_dloc_header_exports_and_layout():
+    """include/dloc.h: every declared function is exported; struct layouts match the binding."""
+    lib = C.CDLL(build.build())
+    src = open(os.path.join(ROOT, "include", "dloc.h"), "r", encoding="utf-8").read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    names = sorted(set(re.findall(r"\b(dloc_[a-z_0-9]+)\s*\(", src)))
+    assert sorted(P.DLOC_EXPORTS) == names
+    for n in names:
+        assert hasattr(lib, n), f"{n} declared in dloc.h but not exported"
+    prog = r'''
+#include <stdio.h>
+#include <stddef.h>
+#include "dloc.h"
+int main(void) {
+  printf("%zu %zu %zu %zu %zu %zu\n", sizeof(dloc_net_desc), offsetof(dloc_net_desc, dilations),
+         offsetof(dloc_net_desc, in_frames), offsetof(dloc_net_desc, sigma_xy_px), offsetof(dloc_net_desc, conv_impl),
+         sizeof(dloc_emitter));
+  return 0;
+}
+'''
+    with tempfile.TemporaryDirectory() as d:
+        src_c = os.path.join(d, "t.c")
+        exe = os.path.join(d, "t")
+        open(src_c, "w").write(prog)
+        subprocess.run(["gcc", "-std=c99", "-I", os.path.join(ROOT, "include"), src_c, "-o", exe], check=True)
+        got = [int(v) for v in subprocess.run([exe], capture_output=True, text=True, check=True).stdout.split()]
+    D = P.DlocDesc
+    assert got == [C.sizeof(D), D.dilations.offset, D.in_frames.offset, D.sigma_xy_px.offset, D.conv_impl.offset,
+                   P.DLOC_EMITTER_DTYPE.itemsize]
+
+
 def test_struct_layout_matches_header():
     prog = r'''
 #include <stdio.h>
