@@ -76,14 +76,20 @@ enum {
 
 /* Kernel fusion on the tcgen05 path ("post-processing is consolidated
  * within GPU memory to minimize data transfer").
- *   AUTO  the last trunk layer's epilogue evaluates the heads (K3 folded in): the final
- *         activation map is never stored; K3 reads a 4 B/px logit map and 32-byte records of
- *         the above-threshold pixels.  K1 stays a kernel of its own (measured faster).
- *   ALL   additionally the stem (K1) is computed inside the first trunk layer's kernel: a_0
- *         never reaches HBM either.
+ *   AUTO  HEAD + PAIRS:
+ *         HEAD   the last trunk layer's epilogue evaluates the heads (K3 folded in): the final
+ *                activation map is never stored; K3 reads a 4 B/px logit map and 32-byte records
+ *                of the above-threshold pixels;
+ *         PAIRS  consecutive trunk layers with dilations (d, 2d) run as one kernel on a
+ *                thread-block cluster; the map between them stays in shared memory (C <= 48,
+ *                rows of at most 1024 pixels; other layers run one per kernel).
+ *         K1 stays a kernel of its own (measured faster).
+ *   ALL   additionally the stem (K1) is computed inside the first trunk layer's kernel when
+ *         that layer is not part of a pair: a_0 never reaches HBM either.
+ *   HEAD  HEAD only (every trunk layer its own kernel).
  *   NONE  one kernel per step (the cross-check twin).
- * All three use the same arithmetic and rounding points and give bit-identical results. */
-enum { SMLM_FUSE_AUTO = 0, SMLM_FUSE_NONE = 1, SMLM_FUSE_ALL = 2 };
+ * All use the same arithmetic and rounding points and give bit-identical results. */
+enum { SMLM_FUSE_AUTO = 0, SMLM_FUSE_NONE = 1, SMLM_FUSE_ALL = 2, SMLM_FUSE_HEAD = 3 };
 
 typedef struct {
   uint32_t struct_size; /* sizeof(smlm_net_desc) */

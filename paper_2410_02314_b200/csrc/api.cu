@@ -60,6 +60,7 @@ struct smlm_ctx {
   float* cand = nullptr;   // 32-byte candidate records (other heads) of above-threshold pixels
   bool fuse = true;        // desc.fusion != SMLM_FUSE_NONE: K3's heads in the last layer's epilogue
   bool fuse_stem = false;  // desc.fusion == SMLM_FUSE_ALL: K1 inside the first layer's kernel
+  bool fuse_pairs = true;  // AUTO / ALL: layers (d, 2d) as one kernel (conv_pair.cu)
 
   uint16_t* slots = nullptr;  // kSlots x slot_elems
   size_t slot_elems = 0;
@@ -172,9 +173,15 @@ smlm_status run_trunk(smlm_ctx* c, const uint16_t* dev_frames, int frame_base, c
                       cudaEvent_t after_stem, bool want_logit, float lthr, bool* have_logit) {
   if (have_logit) *have_logit = false;
   const size_t nl = c->layers.size();
+  // layers l, l+1 run as one kernel (conv_pair.cu) when their dilations are (d, 2d); pairs are
+  // formed greedily from the first layer on (the trunk dump wants every level: no pairs then)
+  auto pair_at = [&](size_t l) {
+    return c->use_umma && c->fuse_pairs && !trunk_dump && l + 1 < nl && c->layers[l + 1].dil == 2 * c->layers[l].dil &&
+           conv_pair_supports(c->d.channels, c->layers[l].dil, c->layers[l + 1].dil, s.W);
+  };
   // K1 folded into the first trunk layer (STEM variant) when the tcgen05 path runs it
   const bool fuse_stem = c->use_umma && c->fuse_stem && nl > 0 && c->dt == ACT_BF16 && c->in_frames == 1 &&
-                         conv_umma_supports(c->d.channels, c->layers[0].dil, true);
+                         !pair_at(0) && conv_umma_supports(c->d.channels, c->layers[0].dil, true);
   cudaEvent_t te = nullptr;
   smlm_status tr = SMLM_OK;
   if (!fuse_stem || trunk_dump) {  // (the trunk dump wants a_0 itself)
@@ -194,7 +201,22 @@ smlm_status run_trunk(smlm_ctx* c, const uint16_t* dev_frames, int frame_base, c
     const Layer& L = c->layers[l];
     cudaEvent_t e1 = nullptr;
     if ((tr = time_begin(c, SMLM_KERNEL_CONV, st, &e1)) != SMLM_OK) return tr;
-    if (c->use_umma) {
+    const bool pair = pair_at(l);
+    if (pair) {
+      char err[256] = {0};
+      const bool head = want_logit && c->fuse && l + 2 == nl;
+      if (head) {
+        c->head_args.lthr = lthr;
+        c->head_args.logit = c->logit;
+        c->head_args.cand = c->cand;
+      }
+      const Layer& L2 = c->layers[l + 1];
+      cudaError_t e = launch_conv_pair(c->dt == ACT_F16, c->act[cur], c->act[cur ^ 1], s, L.dil, L.w_umma, L2.w_umma,
+                                       L.lc, L2.lc, head ? &c->head_args : nullptr, c->n_sm, st, err, sizeof err);
+      if (head && have_logit) *have_logit = true;
+      if (e != cudaSuccess) return fail(c, SMLM_ERR_CUDA, "conv_pair: %s %s", cudaGetErrorString(e), err);
+      ++l;
+    } else if (c->use_umma) {
       char err[256] = {0};
       const bool head = want_logit && c->fuse && l + 1 == nl;
       const bool stem = fuse_stem && l == 0;
@@ -366,7 +388,7 @@ smlm_status smlm_create(const smlm_net_desc* desc, const void* weights, smlm_ctx
   if (!(desc->norm_scale > 0.0f)) return fail(nullptr, SMLM_ERR_INVALID_ARG, "norm_scale must be > 0");
   if (desc->tile < 0 || desc->micro_batch < 0 || desc->writeback_frames < 0)
     return fail(nullptr, SMLM_ERR_INVALID_ARG, "negative tile / micro_batch / writeback_frames");
-  if (desc->fusion < SMLM_FUSE_AUTO || desc->fusion > SMLM_FUSE_ALL)
+  if (desc->fusion < SMLM_FUSE_AUTO || desc->fusion > SMLM_FUSE_HEAD)
     return fail(nullptr, SMLM_ERR_INVALID_ARG, "bad fusion");
 
   int dev = 0;
@@ -388,6 +410,7 @@ smlm_status smlm_create(const smlm_net_desc* desc, const void* weights, smlm_ctx
   c->use_umma = c->bf16 && desc->conv_impl != SMLM_CONV_DIRECT;
   c->fuse = desc->fusion != SMLM_FUSE_NONE;
   c->fuse_stem = desc->fusion == SMLM_FUSE_ALL;
+  c->fuse_pairs = desc->fusion == SMLM_FUSE_AUTO || desc->fusion == SMLM_FUSE_ALL;
   c->n_sm = prop.multiProcessorCount;
   c->l2_bytes = (size_t)prop.l2CacheSize;
   c->radius = 1;

@@ -470,3 +470,37 @@ def test_fused_stem_and_heads_equal_unfused_bit_exact(C, nh, H, W, dil, tile):
         for fusion in (P.FUSE_AUTO, P.FUSE_ALL):
             b = G.gpu_localize(spec, w, frames, ck, thr, fusion=fusion, tile=tile, **kw)
             assert len(a) == len(b) and a.tobytes() == b.tobytes(), (thr, fusion)
+
+
+# ------------------------------------------------------------------ layer pairs (conv_pair.cu) vs one kernel per layer
+@pytest.mark.parametrize("C,nh,n,H,W,dil,tile", [
+    (48, 5, 5, 256, 256, (1, 2, 4, 8) * 3, 0),       # the cfg 1 trunk: six pairs, cluster of 2
+    (48, 5, 3, 37, 130, (1, 2), 0),                  # ragged: 2 valid pixels in the second segment
+    (32, 6, 2, 64, 100, (2, 4, 8, 16), 0),           # one segment (no neighbours), the paper's dilations
+    (16, 5, 2, 21, 1000, (1, 2, 4, 8), 0),           # cluster of 8
+    (48, 5, 2, 3, 17, (4, 8), 0),                    # H < d
+    (48, 5, 1, 40, 1025, (1, 2), 0),                 # 9 segments: not a pair, must fall back
+    (48, 5, 2, 300, 300, (4, 8, 1, 2, 4), 96),       # tiles (windows of 96 + halo), a single layer after the pairs
+    (32, 5, 70, 24, 200, (1, 2, 4, 8), 0)])          # more views than clusters x rows: several runs per cluster
+def test_layer_pairs_equal_unfused_bit_exact(C, nh, n, H, W, dil, tile):
+    """SMLM_FUSE_AUTO runs layers with dilations (d, 2d) as one kernel on a thread-block cluster
+    (the map between them stays in shared memory, x halos exchanged through distributed shared
+    memory).  Same operands, accumulation order and rounding points as one kernel per layer
+    (SMLM_FUSE_HEAD), so head maps and emitter records must be identical bit by bit."""
+    spec = NetSpec(C, dil, nh, "bf16")
+    w = _rand_blob(spec, 700 + C + W, scale=(2.0 / (9 * C)) ** 0.5 * 0.6)
+    off = C * 10 + len(dil) * (C * C * 9 + C)
+    w[off + nh * C] = 0.2
+    rng = np.random.default_rng(H * 1000 + W + 1)
+    frames = rng.integers(80, 3000, size=(n, H, W)).astype(np.uint16)
+    ck = dict(pixel_size_nm=100.0, offset=100.0, gain=1.0)
+    kw = dict(conv_impl=P.CONV_TCGEN05)
+    if not tile:
+        ma = G.gpu_forward_maps(spec, w, frames, ck, fusion=P.FUSE_HEAD, **kw)
+        mb = G.gpu_forward_maps(spec, w, frames, ck, fusion=P.FUSE_AUTO, **kw)
+        assert np.array_equal(ma, mb), float(np.max(np.abs(ma - mb)))
+    for thr in (0.5, 0.0):
+        a = G.gpu_localize(spec, w, frames, ck, thr, fusion=P.FUSE_HEAD, tile=tile, **kw)
+        b = G.gpu_localize(spec, w, frames, ck, thr, fusion=P.FUSE_AUTO, tile=tile, **kw)
+        assert len(a) > 0
+        assert len(a) == len(b) and a.tobytes() == b.tobytes(), thr
