@@ -41,8 +41,8 @@ def load_peaks():
     return dict(FALLBACK_PEAKS), "fallback"
 
 
-def lookup_traffic(cfg, C, views, bound):
-    """(bytes per full-size launch, provenance) of the plain K2 launch from profiles/traffic_r2.json."""
+def lookup_traffic(cfg, C, views, bound, pair=False):
+    """(bytes per full-size launch, provenance) of the dominant K2 kernel from profiles/traffic_r2.json."""
     path = os.path.join(ROOT, "profiles", "traffic_r2.json")
     if bound != "tensor" or not os.path.exists(path):
         return None, "no capture"
@@ -52,10 +52,11 @@ def lookup_traffic(cfg, C, views, bound):
     cap = doc.get("captures", {}).get(f"{wl}/views{views}")
     if not cap:
         return None, f"no capture for {wl}/views{views} in profiles/traffic_r2.json"
-    k = cap["per_kernel_mean"].get(f"conv_umma_kernel<{C},-,->")
+    name = f"conv_pair_kernel<{C},-,->" if pair else f"conv_umma_kernel<{C},-,->"
+    k = cap["per_kernel_mean"].get(name)
     if not k:
-        return None, "capture holds no plain K2 launch"
-    note = (f"profiles/traffic_r2.json {wl}/views{views}: mean of {k['n']} plain K2 launches of {views} views "
+        return None, f"capture {wl}/views{views} holds no {name} launch"
+    note = (f"profiles/traffic_r2.json {wl}/views{views}: mean of {k['n']} {name} launches of {views} views "
             f"(ncu --set full, {cap.get('source', '')}); the HEAD launch and the tail launch of a step are listed "
             f"there separately")
     return k["dram_bytes"], note
@@ -209,8 +210,9 @@ def main(argv=None):
     ap.add_argument("--micro-batch", type=int, default=0)
     ap.add_argument("--fusion", default="auto", choices=["auto", "none", "all", "head"])
     ap.add_argument("--tile", type=int, default=-1, help="override the config's tile size (0: whole frames)")
-    ap.add_argument("--tile-merge", default="none", choices=["none", "row"],
-                    help="row: one window per tile row (SMLM_TILE_MERGE_ROW)")
+    ap.add_argument("--tile-merge", default="auto", choices=["auto", "none", "row"],
+                    help="row: one window per tile row (SMLM_TILE_MERGE_ROW); auto = row for a tiled config "
+                         "(cfg 3: 408 vs 325 frames/s, profiles/bench_r2.md)")
     ap.add_argument("--precision", default="", choices=["", "bf16", "fp16"],
                     help="activation storage type of the variants study (SURVEY.md 8(f)-4); default: the config's")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -261,9 +263,10 @@ def main(argv=None):
     weights = make_weights(cfg)
     H, W = frames.shape[1:]
     conv_impl = {"auto": P.CONV_AUTO, "tcgen05": P.CONV_TCGEN05, "direct": P.CONV_DIRECT}[args.conv_impl]
+    tile_merge = args.tile_merge if args.tile_merge != "auto" else ("row" if cfg.tile else "none")
     desc = P.desc_from_spec(cfg.net, tile=cfg.tile, micro_batch=args.micro_batch, conv_impl=conv_impl,
                             writeback_frames=cfg.writeback_batch,
-                            tile_merge={"none": P.TILE_MERGE_NONE, "row": P.TILE_MERGE_ROW}[args.tile_merge],
+                            tile_merge={"none": P.TILE_MERGE_NONE, "row": P.TILE_MERGE_ROW}[tile_merge],
                             fusion={"auto": P.FUSE_AUTO, "none": P.FUSE_NONE, "all": P.FUSE_ALL, "head": P.FUSE_HEAD}[args.fusion])
     loc = P.Localizer(desc, weights)
     cap = int(n_frames * max(4 * cfg.frames.emitters_per_frame, 1024))
@@ -298,7 +301,7 @@ def main(argv=None):
         st = loc.check()
         if st != P.OK:
             raise SystemExit(f"smlm_check: {st} {loc.last_error()}")
-        kt = {k: loc.kernel_time_ms(k) for k in (P.KERNEL_STEM, P.KERNEL_CONV, P.KERNEL_POST)} \
+        kt = {k: loc.kernel_time_ms(k) for k in (P.KERNEL_STEM, P.KERNEL_CONV, P.KERNEL_CONV_PAIR, P.KERNEL_POST)} \
             if kernel_timing else None
         loc.kernel_timing(False)
         return ms, [int(c.value) for c in counts], loc.launch_count() - l0, kt
@@ -314,7 +317,9 @@ def main(argv=None):
     # roofline pass: the same steps with every K2 launch bracketed by CUDA events on the
     # launching stream (the events serialise a little, so `value` is not taken from this pass)
     ms_rf, _, _, kt = timed(frames_dev, out_dev, args.steps, kernel_timing=True)
-    conv_ms, conv_n = kt[P.KERNEL_CONV]
+    single_ms, single_n = kt[P.KERNEL_CONV]          # launches of one trunk layer
+    pair_ms, pair_n = kt[P.KERNEL_CONV_PAIR]         # launches of two trunk layers (conv_pair.cu)
+    conv_ms, conv_n = single_ms + pair_ms, single_n + pair_n
     disk = None
     if args.disk:
         # the paper's storage -> GPU experiment: reader threads fill the pinned ring
@@ -353,18 +358,24 @@ def main(argv=None):
 
     peaks, peak_kind = load_peaks()
     C, L = cfg.net.channels, cfg.net.n_layers
-    # views of a full-size launch (api.cu auto_micro_batch: <= 64, <= 1.5 GB per activation buffer)
+    # views of a full-size launch (api.cu auto_micro_batch: <= 128, <= 1.5 GB per activation buffer)
     if args.micro_batch:
         loc_views_per_launch = args.micro_batch
-    elif cfg.tile:   # the largest launch set: all interior tiles (window = tile + 2 halo) of the chunk's frames
+    elif cfg.tile and tile_merge == "none":   # the largest launch set: all interior tiles of the chunk's frames
         ext = cfg.tile + 2 * (cfg.net.radius + 1)
-        mb = int(min(64, max(1, (1536 << 20) // (ext * ext * C * 2))))
+        mb = int(min(128, max(1, (1536 << 20) // (ext * ext * C * 2))))
         inner = max(1, (-(-H // cfg.tile) - 2)) * max(1, (-(-W // cfg.tile) - 2))
         loc_views_per_launch = max(1, min(mb // inner, n_frames)) * inner
+    elif cfg.tile:                            # row-merged tiles: windows of (tile + 2 halo) rows x the frame width
+        ext = cfg.tile + 2 * (cfg.net.radius + 1)
+        mb = int(min(128, max(1, (1536 << 20) // (ext * W * C * 2))))
+        inner = max(1, (-(-H // cfg.tile) - 2))
+        loc_views_per_launch = max(1, min(mb // inner, n_frames)) * inner
     else:
-        loc_views_per_launch = int(min(64, max(1, (1536 << 20) // (H * W * C * 2)), n_frames))
-    # dominant kernel: the dilated 3x3 conv layer (K2).  Algorithmic work per launch =
-    # 18 C^2 FLOP per pixel per layer x the pixels one launch processes.
+        loc_views_per_launch = int(min(128, max(1, (1536 << 20) // (H * W * C * 2)), n_frames))
+    # dominant kernel: the dilated 3x3 conv (K2), one layer per launch (conv_umma_kernel) or two
+    # (conv_pair_kernel).  Algorithmic work = 18 C^2 FLOP per pixel per layer;
+    # algorithmic bytes of a launch = 2C B/px in + 2C B/px out, whatever the number of layers it runs.
     flop_total = 18.0 * C * C * H * W * n_frames * L * args.steps
     roofline = None
     if conv_n > 0 and conv_ms > 0:  # tiled configs: algorithmic (whole-frame) FLOPs, halo recompute not counted
@@ -373,22 +384,35 @@ def main(argv=None):
         bound = "tensor"
         if cfg.net.precision not in ("bf16", "fp16") or args.conv_impl == "direct":
             bound = "alu"
-        # DRAM traffic per launch: dram__bytes_read.sum + dram__bytes_write.sum of this kernel
-        # in this launch shape, from the tracked ncu --set full record (profiles/traffic_r2.json,
-        # written by paper_2410_02314_b200/profile_tools.py from the capture named there);
-        # null when no capture of this (workload, views per launch) exists.
-        alg_bytes_per_launch = 4.0 * C * H * W * (n_frames * args.steps * L / conv_n)
-        traffic, traffic_note = lookup_traffic(cfg, C, loc_views_per_launch, bound)
-        roofline = {"bound": bound, "kernel": "conv3x3_dilated (K2)", "achieved": achieved, "peak": peak,
-                    "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_note,
+        # the launches of the step split by kernel: layers = single_n + 2 pair_n
+        layers_run = single_n + 2 * pair_n
+        dominant_pair = pair_ms >= single_ms
+        dom_ms, dom_n, dom_layers = (pair_ms, pair_n, 2) if dominant_pair else (single_ms, single_n, 1)
+        dom_flop = flop_total * (dom_layers * dom_n) / layers_run
+        alg_bytes_per_launch = 4.0 * C * H * W * n_frames * args.steps * L / layers_run
+        # DRAM traffic per launch: dram__bytes_read.sum + dram__bytes_write.sum of the dominant
+        # kernel in this launch shape, from the tracked ncu --set full record
+        # (profiles/traffic_r2.json, written by paper_2410_02314_b200/profile_tools.py from the
+        # capture named there); null when no capture of this (workload, views per launch) exists.
+        traffic, traffic_note = lookup_traffic(cfg, C, loc_views_per_launch, bound, dominant_pair)
+        roofline = {"bound": bound,
+                    "kernel": "conv3x3_dilated x2, layers (d, 2d) fused (conv_pair_kernel)" if dominant_pair
+                              else "conv3x3_dilated (conv_umma_kernel)",
+                    "achieved": dom_flop / (dom_ms * 1e-3) / 1e12, "peak": peak,
+                    "unit": "TFLOP/s", "frac": dom_flop / (dom_ms * 1e-3) / 1e12 / peak,
+                    "traffic": traffic, "traffic_source": traffic_note,
                     "algorithmic_bytes_per_launch": alg_bytes_per_launch,
-                    "hbm_GBs_algorithmic": alg_bytes_per_launch * conv_n / (conv_ms * 1e-3) / 1e9,
-                    "hbm_frac_algorithmic": alg_bytes_per_launch * conv_n / (conv_ms * 1e-3) / 1e9
+                    "hbm_GBs_algorithmic": alg_bytes_per_launch * dom_n / (dom_ms * 1e-3) / 1e9,
+                    "hbm_frac_algorithmic": alg_bytes_per_launch * dom_n / (dom_ms * 1e-3) / 1e9
                                             / float(peaks["hbm_gbs"]),
                     "peak_source": f"{peak_kind} bf16_tflops_sustained (kernel timed inside a long step)",
-                    "frac_of_burst": achieved / float(peaks["bf16_tflops"]),
-                    "launches": conv_n, "avg_launch_ms": conv_ms / conv_n,
-                    "share_of_step": conv_ms / ms_rf}
+                    "frac_of_burst": dom_flop / (dom_ms * 1e-3) / 1e12 / float(peaks["bf16_tflops"]),
+                    "launches": dom_n, "avg_launch_ms": dom_ms / dom_n, "layers_per_launch": dom_layers,
+                    "share_of_step": dom_ms / ms_rf,
+                    "all_trunk_launches": {"achieved": achieved, "frac": achieved / peak,
+                                           "frac_of_burst": achieved / float(peaks["bf16_tflops"]),
+                                           "single_layer_launches": single_n, "pair_launches": pair_n,
+                                           "share_of_step": conv_ms / ms_rf}}
     # K1 / K3: bytes moved per launch / CUDA-event time, against the
     # measured HBM copy bandwidth (the maps they touch are L2-resident in this pipeline, so
     # this is "bytes moved", not DRAM traffic).
@@ -417,7 +441,7 @@ def main(argv=None):
         "scaling": args.scaling, "vs_baseline": None,
         "dtype": {"bf16": "bf16", "fp16": "f16"}.get(cfg.net.precision, "f32"), "data": "synthetic",
         "config": {"workload": cfg.name, "frames_per_step": n_frames, "H": H, "W": W, "channels": C,
-                   "layers": L, "head_channels": cfg.net.head_channels, "tile": cfg.tile, "tile_merge": args.tile_merge,
+                   "layers": L, "head_channels": cfg.net.head_channels, "tile": cfg.tile, "tile_merge": tile_merge,
                    "precision": cfg.net.precision,
                    "distinct_frames": int(len(fs.frames)), "conv_impl": args.conv_impl, "fusion": args.fusion,
                    "l2": "inputs larger than L2 (u16 stack + activation stream per step > 126 MB)",

@@ -225,7 +225,8 @@ int64_t smlm_launch_count(const smlm_ctx* ctx);
  * launching stream; smlm_kernel_time_ms (after a stream sync) sums the launches of one kind
  * since timing was last enabled.  Disabled by default: the events cost ~1 us each and switch
  * off the programmatic overlap between consecutive layers. */
-enum { SMLM_KERNEL_STEM = 0, SMLM_KERNEL_CONV = 1, SMLM_KERNEL_POST = 2 };
+/* CONV: one trunk layer per launch; CONV_PAIR: two trunk layers per launch (SMLM_FUSE_* PAIRS). */
+enum { SMLM_KERNEL_STEM = 0, SMLM_KERNEL_CONV = 1, SMLM_KERNEL_POST = 2, SMLM_KERNEL_CONV_PAIR = 3 };
 smlm_status smlm_kernel_timing(smlm_ctx* ctx, int32_t enable);
 smlm_status smlm_kernel_time_ms(smlm_ctx* ctx, int32_t kind, double* total_ms, int64_t* launches);
 

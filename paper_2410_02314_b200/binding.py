@@ -21,7 +21,7 @@ CONV_AUTO, CONV_TCGEN05, CONV_DIRECT = 0, 1, 2
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED_DEVICE, ERR_CUDA, ERR_OOM, ERR_OVERFLOW = 0, -1, -2, -3, -4, -5
 ABI_VERSION = 3
 FUSE_AUTO, FUSE_NONE, FUSE_ALL, FUSE_HEAD = 0, 1, 2, 3
-KERNEL_STEM, KERNEL_CONV, KERNEL_POST = 0, 1, 2
+KERNEL_STEM, KERNEL_CONV, KERNEL_POST, KERNEL_CONV_PAIR = 0, 1, 2, 3
 
 EXPORTS = ["smlm_create", "smlm_localize", "smlm_check", "smlm_destroy", "smlm_last_error",
            "smlm_launch_count", "smlm_kernel_timing", "smlm_kernel_time_ms",
@@ -230,7 +230,7 @@ class Localizer:
         self._check(lib().smlm_kernel_timing(self._h, 1 if enable else 0))
 
     def kernel_time_ms(self, kind: int):
-        """(total ms, launches) of KERNEL_STEM / KERNEL_CONV / KERNEL_POST since timing was enabled."""
+        """(total ms, launches) of KERNEL_STEM / KERNEL_CONV / KERNEL_CONV_PAIR / KERNEL_POST since timing was enabled."""
         ms, k = C.c_double(), C.c_int64()
         self._check(lib().smlm_kernel_time_ms(self._h, int(kind), C.byref(ms), C.byref(k)))
         return ms.value, k.value

@@ -200,8 +200,8 @@ smlm_status run_trunk(smlm_ctx* c, const uint16_t* dev_frames, int frame_base, c
   for (size_t l = 0; l < nl; ++l) {
     const Layer& L = c->layers[l];
     cudaEvent_t e1 = nullptr;
-    if ((tr = time_begin(c, SMLM_KERNEL_CONV, st, &e1)) != SMLM_OK) return tr;
     const bool pair = pair_at(l);
+    if ((tr = time_begin(c, pair ? SMLM_KERNEL_CONV_PAIR : SMLM_KERNEL_CONV, st, &e1)) != SMLM_OK) return tr;
     if (pair) {
       char err[256] = {0};
       const bool head = want_logit && c->fuse && l + 2 == nl;
@@ -349,14 +349,15 @@ smlm_status store_count(smlm_ctx* c, const unsigned long long* counter, int64_t*
 
 int auto_micro_batch(const smlm_ctx* c, int Hw, int Ww) {
   if (c->d.micro_batch > 0) return c->d.micro_batch;
-  // Measured on B200 (profiles/microbatch_sweep_r1.md): keeping the two ping-pong maps
-  // L2-resident (7 frames of 256x256x48) is SLOWER than streaming large micro-batches from
-  // HBM - per-launch overheads and the two halo steps per lane range weigh more than the
-  // DRAM traffic, which stays below 65 % of HBM bandwidth.  So: up to 64 views per launch,
-  // bounded by 1.5 GB per activation buffer.
+  // Measured on B200 (profiles/microbatch_sweep_r1.md, profiles/bench_r2.md): keeping the two
+  // ping-pong maps L2-resident (7 frames of 256x256x48) is SLOWER than streaming large
+  // micro-batches from HBM - per-launch overheads (prologue, weight load, tail) and the halo
+  // steps per work range weigh more than the DRAM traffic.  So: up to 128 views per launch
+  // (round 2 sweep: 64 -> 128 views is +1.7 % on cfg 1, flat beyond), bounded by 1.5 GB per
+  // activation buffer.
   size_t per_view = (size_t)Hw * Ww * c->d.channels * elt_size(c);
   size_t b = ((size_t)1536 << 20) / std::max<size_t>(per_view, 1);
-  return (int)std::min<size_t>(std::max<size_t>(b, 1), 64);
+  return (int)std::min<size_t>(std::max<size_t>(b, 1), 128);
 }
 
 }  // namespace
@@ -527,7 +528,7 @@ smlm_status smlm_kernel_timing(smlm_ctx* c, int32_t enable) {
 }
 
 smlm_status smlm_kernel_time_ms(smlm_ctx* c, int32_t kind, double* total_ms, int64_t* launches) {
-  if (!c || !total_ms || !launches || kind < SMLM_KERNEL_STEM || kind > SMLM_KERNEL_POST)
+  if (!c || !total_ms || !launches || kind < SMLM_KERNEL_STEM || kind > SMLM_KERNEL_CONV_PAIR)
     return SMLM_ERR_INVALID_ARG;
   double tot = 0.0;
   int64_t n = 0;

@@ -119,17 +119,17 @@ __device__ __forceinline__ void wait_bar(uint32_t bar, uint32_t parity) {
   for (;;) {
     if (CLUSTER)
       asm volatile(
-          "{\n.reg .pred p;\nmbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n"
+          "{\n.reg .pred p;\nmbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2, %3;\n"
           "selp.u32 %0, 1, 0, p;\n}\n"
           : "=r"(ok)
-          : "r"(bar), "r"(parity)
+          : "r"(bar), "r"(parity), "r"(0x989680u)
           : "memory");
     else
       asm volatile(
-          "{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+          "{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n"
           "selp.u32 %0, 1, 0, p;\n}\n"
           : "=r"(ok)
-          : "r"(bar), "r"(parity)
+          : "r"(bar), "r"(parity), "r"(0x989680u)
           : "memory");
     if (ok) return;
     const long long t = clock64();

@@ -53,6 +53,9 @@ def short_name(name: str) -> str:
     if m:
         return (f"conv_umma_kernel<{m.group(1)},{'HEAD' if t(m.group(2)) else '-'},"
                 f"{'STEM' if t(m.group(3)) else '-'}" + (",f16" if m.group(4) and t(m.group(4)) else "") + ">")
+    m = re.match(r"conv_pair_kernel<(\d+),\s*(?:\(bool\))?(\w+),\s*(?:\(bool\))?(\w+)>", name)
+    if m:
+        return f"conv_pair_kernel<{m.group(1)},{'HEAD' if t(m.group(2)) else '-'},{'f16' if t(m.group(3)) else '-'}>"
     m = re.match(r"([\w:]+)(<.*?>)?\(", name)
     if m:
         return m.group(1) + (m.group(2) or "").replace("__nv_bfloat16", "bf16").replace("__half", "f16") \
@@ -144,6 +147,9 @@ def cmd_traffic(args):
             if e["kernel"].startswith("conv_umma_kernel"):
                 e["dilation"] = dil[k % len(dil)]
                 k += 1
+            elif e["kernel"].startswith("conv_pair_kernel"):   # two layers per launch
+                e["dilation"] = [dil[k % len(dil)], dil[(k + 1) % len(dil)]]
+                k += 2
     record = {"workload": args.workload, "views_per_launch": args.views, "source": args.source or args.csv,
               "launches": entries}
     by = collections.defaultdict(list)
