@@ -138,6 +138,15 @@ __device__ __forceinline__ void wait_bar(uint32_t bar, uint32_t parity) {
   }
 }
 
+__device__ __forceinline__ unsigned long long pack2f(float lo, float hi) {
+  return ((unsigned long long)__float_as_uint(hi) << 32) | __float_as_uint(lo);
+}
+__device__ __forceinline__ unsigned long long ffma2(unsigned long long a, unsigned long long b, unsigned long long c) {
+  unsigned long long d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+
 template <int C, bool HEAD, bool F16>
 __global__ void __launch_bounds__(kThreads, 1)
     conv_pair_kernel(const __nv_bfloat16* __restrict__ in, __nv_bfloat16* __restrict__ out, PGeo geo,
@@ -563,12 +572,15 @@ __global__ void __launch_bounds__(kThreads, 1)
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive(accB_free(s));
-          float hp[6] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};
+          // HEAD (K3 folded in, as conv_umma.cu): every head is the sum of two fmaf chains, one per
+          // channel half (head_post.cu evaluates the same two chains); heads are updated two at a
+          // time with fma.rn.f32x2 (two independent IEEE fp32 FMAs: the same bits as fmaf).
+          unsigned long long hq[3] = {0ull, 0ull, 0ull};  // (o_0, o_1), (o_2, o_3), (o_4, o_5)
           auto post = [&](auto HALF) {
             constexpr int kHalf = decltype(HALF)::value;
             if (HEAD && kHalf == 0) {
 #pragma unroll
-              for (int h = 0; h < 6; ++h) hp[h] = ha.b[h];
+              for (int j = 0; j < 3; ++j) hq[j] = pack2f(ha.b[2 * j], ha.b[2 * j + 1]);
             }
 #pragma unroll
             for (int kk = 0; kk < KH; ++kk) {
@@ -586,10 +598,12 @@ __global__ void __launch_bounds__(kThreads, 1)
                 if (HEAD) {
                   float a0, a1;
                   unpack2<F16>(ow[i], a0, a1);
+                  const unsigned long long aa0 = pack2f(a0, a0), aa1 = pack2f(a1, a1);
 #pragma unroll
-                  for (int h = 0; h < 6; ++h) hp[h] = fmaf(a0, ha.w[c0][h], hp[h]);
+                  for (int j = 0; j < 3; ++j) hq[j] = ffma2(aa0, pack2f(ha.w[c0][2 * j], ha.w[c0][2 * j + 1]), hq[j]);
 #pragma unroll
-                  for (int h = 0; h < 6; ++h) hp[h] = fmaf(a1, ha.w[c0 + 1][h], hp[h]);
+                  for (int j = 0; j < 3; ++j)
+                    hq[j] = ffma2(aa1, pack2f(ha.w[c0 + 1][2 * j], ha.w[c0 + 1][2 * j + 1]), hq[j]);
                 }
               }
               if (!HEAD) orow[(size_t)kk * plane_px] = make_uint4(ow[0], ow[1], ow[2], ow[3]);
@@ -600,6 +614,12 @@ __global__ void __launch_bounds__(kThreads, 1)
             else post(std::integral_constant<int, 1>{});
           }
           if (HEAD && out_valid) {
+            float hp[6];
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+              hp[2 * j] = __uint_as_float((uint32_t)hq[j]);
+              hp[2 * j + 1] = __uint_as_float((uint32_t)(hq[j] >> 32));
+            }
             if (half == 1) {
               *reinterpret_cast<float4*>(xch) = make_float4(hp[0], hp[1], hp[2], hp[3]);
               *reinterpret_cast<float2*>(xch + 4) = make_float2(hp[4], hp[5]);
