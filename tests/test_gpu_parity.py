@@ -223,8 +223,8 @@ def test_cfg4_dense_bf16(impl):
 # ------------------------------------------------------------------ maps in the launch shape bench.py times
 def _launch_shape_maps(name, cfg, fs, w, n, sample, tol=2e-2):
     """n frames cycling the distinct frames of fs through smlm_debug_forward_maps with the
-    default micro-batch (cfg 1: 64 + 64 + tail views per launch): K2's work split - lane
-    ranges of ~110 rows that start and end mid-chain - is the one of the timed run.  Sampled
+    default micro-batch (cfg 1: 128 + 128 + tail views per launch): K2's work split - cluster /
+    lane ranges of a few hundred rows that start and end mid-chain - is the one of the timed run.  Sampled
     frames are compared element by element with the oracle, and every frame with the first
     occurrence of the same distinct frame bit by bit (position in the launch must not matter)."""
     k = len(fs.frames)
@@ -242,9 +242,9 @@ def _launch_shape_maps(name, cfg, fs, w, n, sample, tol=2e-2):
     G.record(f"{name}_launch_shape_maps", frames=n, distinct=k, head_max_err=errs)
 
 
-def test_cfg1_maps_in_timed_launch_shape_130_frames():
-    cfg = get_config(1)
-    _launch_shape_maps("cfg1lc", cfg, make_frames(cfg, 2), make_weights(cfg, "lc"), 130, (0, 63, 64, 129))
+def test_cfg1_maps_in_timed_launch_shape_260_frames():
+    cfg = get_config(1)     # default micro-batch: 128 + 128 + tail views per launch, layer pairs on 2-CTA clusters
+    _launch_shape_maps("cfg1lc", cfg, make_frames(cfg, 2), make_weights(cfg, "lc"), 260, (0, 127, 128, 259))
 
 
 def test_cfg2_maps_full_frame_in_multi_view_launch():
