@@ -208,7 +208,7 @@ def main(argv=None):
     ap.add_argument("--frames", type=int, default=0, help="override the number of frames per step")
     ap.add_argument("--conv-impl", default="auto", choices=["auto", "tcgen05", "direct"])
     ap.add_argument("--micro-batch", type=int, default=0)
-    ap.add_argument("--fusion", default="auto", choices=["auto", "none", "all", "head"])
+    ap.add_argument("--fusion", default="auto", choices=["auto", "none", "all", "head", "pairs1"])
     ap.add_argument("--tile", type=int, default=-1, help="override the config's tile size (0: whole frames)")
     ap.add_argument("--tile-merge", default="auto", choices=["auto", "none", "row"],
                     help="row: one window per tile row (SMLM_TILE_MERGE_ROW); auto = row for a tiled config "
@@ -267,7 +267,7 @@ def main(argv=None):
     desc = P.desc_from_spec(cfg.net, tile=cfg.tile, micro_batch=args.micro_batch, conv_impl=conv_impl,
                             writeback_frames=cfg.writeback_batch,
                             tile_merge={"none": P.TILE_MERGE_NONE, "row": P.TILE_MERGE_ROW}[tile_merge],
-                            fusion={"auto": P.FUSE_AUTO, "none": P.FUSE_NONE, "all": P.FUSE_ALL, "head": P.FUSE_HEAD}[args.fusion])
+                            fusion={"auto": P.FUSE_AUTO, "none": P.FUSE_NONE, "all": P.FUSE_ALL, "head": P.FUSE_HEAD, "pairs1": P.FUSE_PAIRS_1CTA}[args.fusion])
     loc = P.Localizer(desc, weights)
     cap = int(n_frames * max(4 * cfg.frames.emitters_per_frame, 1024))
     cap = min(cap, n_frames * ((H + 1) // 2) * ((W + 1) // 2))

@@ -82,14 +82,17 @@ enum {
  *                of the above-threshold pixels;
  *         PAIRS  consecutive trunk layers with dilations (d, 2d) run as one kernel on a
  *                thread-block cluster; the map between them stays in shared memory (C <= 48,
- *                rows of at most 1024 pixels; other layers run one per kernel).
+ *                rows of at most 1024 pixels; other layers run one per kernel).  Rows with an
+ *                even number of 128-pixel segments use tcgen05 cta_group::2 (one M = 256 MMA
+ *                per CTA pair, weights split between the two CTAs).
  *         K1 stays a kernel of its own (measured faster).
  *   ALL   additionally the stem (K1) is computed inside the first trunk layer's kernel when
  *         that layer is not part of a pair: a_0 never reaches HBM either.
  *   HEAD  HEAD only (every trunk layer its own kernel).
+ *   PAIRS_1CTA  as AUTO with cta_group::1 MMAs in the pair kernel (the comparison twin).
  *   NONE  one kernel per step (the cross-check twin).
  * All use the same arithmetic and rounding points and give bit-identical results. */
-enum { SMLM_FUSE_AUTO = 0, SMLM_FUSE_NONE = 1, SMLM_FUSE_ALL = 2, SMLM_FUSE_HEAD = 3 };
+enum { SMLM_FUSE_AUTO = 0, SMLM_FUSE_NONE = 1, SMLM_FUSE_ALL = 2, SMLM_FUSE_HEAD = 3, SMLM_FUSE_PAIRS_1CTA = 4 };
 
 typedef struct {
   uint32_t struct_size; /* sizeof(smlm_net_desc) */

@@ -20,7 +20,7 @@ TILE_MERGE_NONE, TILE_MERGE_ROW = 0, 1
 CONV_AUTO, CONV_TCGEN05, CONV_DIRECT = 0, 1, 2
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED_DEVICE, ERR_CUDA, ERR_OOM, ERR_OVERFLOW = 0, -1, -2, -3, -4, -5
 ABI_VERSION = 3
-FUSE_AUTO, FUSE_NONE, FUSE_ALL, FUSE_HEAD = 0, 1, 2, 3
+FUSE_AUTO, FUSE_NONE, FUSE_ALL, FUSE_HEAD, FUSE_PAIRS_1CTA = 0, 1, 2, 3, 4
 KERNEL_STEM, KERNEL_CONV, KERNEL_POST, KERNEL_CONV_PAIR = 0, 1, 2, 3
 
 EXPORTS = ["smlm_create", "smlm_localize", "smlm_check", "smlm_destroy", "smlm_last_error",

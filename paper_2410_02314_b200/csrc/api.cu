@@ -60,7 +60,8 @@ struct smlm_ctx {
   float* cand = nullptr;   // 32-byte candidate records (other heads) of above-threshold pixels
   bool fuse = true;        // desc.fusion != SMLM_FUSE_NONE: K3's heads in the last layer's epilogue
   bool fuse_stem = false;  // desc.fusion == SMLM_FUSE_ALL: K1 inside the first layer's kernel
-  bool fuse_pairs = true;  // AUTO / ALL: layers (d, 2d) as one kernel (conv_pair.cu)
+  bool fuse_pairs = true;  // AUTO / ALL / PAIRS_1CTA: layers (d, 2d) as one kernel (conv_pair.cu)
+  bool pair_cg2 = true;    // ... with tcgen05 cta_group::2 where a row has an even number of segments
 
   uint16_t* slots = nullptr;  // kSlots x slot_elems
   size_t slot_elems = 0;
@@ -212,7 +213,7 @@ smlm_status run_trunk(smlm_ctx* c, const uint16_t* dev_frames, int frame_base, c
       }
       const Layer& L2 = c->layers[l + 1];
       cudaError_t e = launch_conv_pair(c->dt == ACT_F16, c->act[cur], c->act[cur ^ 1], s, L.dil, L.w_umma, L2.w_umma,
-                                       L.lc, L2.lc, head ? &c->head_args : nullptr, c->n_sm, st, err, sizeof err);
+                                       L.lc, L2.lc, head ? &c->head_args : nullptr, c->pair_cg2, c->n_sm, st, err, sizeof err);
       if (head && have_logit) *have_logit = true;
       if (e != cudaSuccess) return fail(c, SMLM_ERR_CUDA, "conv_pair: %s %s", cudaGetErrorString(e), err);
       ++l;
@@ -389,7 +390,7 @@ smlm_status smlm_create(const smlm_net_desc* desc, const void* weights, smlm_ctx
   if (!(desc->norm_scale > 0.0f)) return fail(nullptr, SMLM_ERR_INVALID_ARG, "norm_scale must be > 0");
   if (desc->tile < 0 || desc->micro_batch < 0 || desc->writeback_frames < 0)
     return fail(nullptr, SMLM_ERR_INVALID_ARG, "negative tile / micro_batch / writeback_frames");
-  if (desc->fusion < SMLM_FUSE_AUTO || desc->fusion > SMLM_FUSE_HEAD)
+  if (desc->fusion < SMLM_FUSE_AUTO || desc->fusion > SMLM_FUSE_PAIRS_1CTA)
     return fail(nullptr, SMLM_ERR_INVALID_ARG, "bad fusion");
 
   int dev = 0;
@@ -411,7 +412,8 @@ smlm_status smlm_create(const smlm_net_desc* desc, const void* weights, smlm_ctx
   c->use_umma = c->bf16 && desc->conv_impl != SMLM_CONV_DIRECT;
   c->fuse = desc->fusion != SMLM_FUSE_NONE;
   c->fuse_stem = desc->fusion == SMLM_FUSE_ALL;
-  c->fuse_pairs = desc->fusion == SMLM_FUSE_AUTO || desc->fusion == SMLM_FUSE_ALL;
+  c->fuse_pairs = desc->fusion == SMLM_FUSE_AUTO || desc->fusion == SMLM_FUSE_ALL || desc->fusion == SMLM_FUSE_PAIRS_1CTA;
+  c->pair_cg2 = desc->fusion != SMLM_FUSE_PAIRS_1CTA;
   c->n_sm = prop.multiProcessorCount;
   c->l2_bytes = (size_t)prop.l2CacheSize;
   c->radius = 1;

@@ -48,7 +48,7 @@ constexpr int kMaxSt = 4;     // stages per ring
 constexpr int kTmemCols = 512;
 constexpr int kMaxDevices = 64;
 constexpr int kMaxCluster = 8;  // portable cluster size
-constexpr int kNumBars = 23;
+constexpr int kNumBars = 23 + 2 * kMaxSt;  // + the peer's stage-full relays (cta_group::2)
 
 // zero source for the padded parts of an input row segment: at most (127 + 8) pixels x 16 B
 __device__ __align__(16) uint4 g_pzeros[160];
@@ -94,9 +94,13 @@ struct PSmem {
   uint32_t bar_off, tmem_off, total;
 };
 
-__host__ __device__ inline PSmem pair_smem(int C, int d, int nA, int nB, bool head) {
+// cta_group::2: of every 5C-row weight plane a CTA holds the rows its half of the three N = 3C
+// windows needs: rows [pr NH, pr NH + 2C + NH), NH = 3C/2, pr = rank in the pair
+__host__ __device__ constexpr uint32_t pair_wrows(int C, bool cg2) { return cg2 ? 2u * C + 3u * C / 2u : 5u * C; }
+
+__host__ __device__ inline PSmem pair_smem(int C, int d, int nA, int nB, bool head, bool cg2) {
   PSmem L;
-  L.w_bytes = 30u * C * C;
+  L.w_bytes = 3u * (C / 8) * pair_wrows(C, cg2) * 16u;
   L.wA_off = 0;
   L.wB_off = L.w_bytes;
   L.stA_bytes = (((uint32_t)(C / 8) * (kTileM + 2 * d) * 16u) + 127u) & ~127u;
@@ -147,7 +151,32 @@ __device__ __forceinline__ unsigned long long ffma2(unsigned long long a, unsign
   return d;
 }
 
-template <int C, bool HEAD, bool F16>
+// cta_group::2: one MMA over the CTA pair (ranks 2k, 2k+1 of the cluster = two adjacent
+// segments): D[256 x N], A rows 0-127 / 128-255 and D from the leader's / the peer's shared
+// memory and TMEM at the same addresses, B's N columns split between the two CTAs.
+__device__ __forceinline__ void tc_mma2(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "setp.ne.b32 p, 1, 0;\n"
+      "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n"
+      "}\n" ::"r"(d_tmem),
+      "l"(a_desc), "l"(b_desc), "r"(idesc)
+      : "memory");
+}
+__device__ __forceinline__ void tc_commit2_mc(uint32_t bar, uint16_t mask) {
+  asm volatile(
+      "tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar),
+      "h"(mask)
+      : "memory");
+}
+// relay "this CTA's stage is full" to the leader: the relaying warp has no stores of its own in
+// flight, so the cluster-scope release is cheap here
+__device__ __forceinline__ void mbar_arrive_cluster_release(uint32_t cbar) {
+  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cbar) : "memory");
+}
+
+template <int C, bool HEAD, bool F16, bool CG2>
 __global__ void __launch_bounds__(kThreads, 1)
     conv_pair_kernel(const __nv_bfloat16* __restrict__ in, __nv_bfloat16* __restrict__ out, PGeo geo,
                      const uint8_t* __restrict__ wpackA, const uint8_t* __restrict__ wpackB, int nA, int nB,
@@ -155,7 +184,7 @@ __global__ void __launch_bounds__(kThreads, 1)
                      const __grid_constant__ HeadArgs ha) {
   extern __shared__ uint8_t smem_raw[];
   const int d = geo.d, dB = 2 * geo.d;
-  const PSmem L = pair_smem(C, d, nA, nB, HEAD);
+  const PSmem L = pair_smem(C, d, nA, nB, HEAD, CG2);
   const uint32_t sraw = smem_u32(smem_raw);
   const uint32_t sbase = (sraw + 1023u) & ~1023u;  // the launch reserves 1 KB of slack for this
   uint8_t* smem = smem_raw + (sbase - sraw);
@@ -166,6 +195,10 @@ __global__ void __launch_bounds__(kThreads, 1)
   const int nnb = 1 + (has_left ? 1 : 0) + (has_right ? 1 : 0);
   const int cid = blockIdx.x / nseg, ncl = gridDim.x / nseg;
   const int x0 = rank * kTileM;
+  // cta_group::2: the even rank of a pair issues the MMAs of both CTAs
+  const int pr = rank & 1;
+  const bool leader = !CG2 || pr == 0;
+  const uint32_t leader_rank = (uint32_t)(rank & ~1);
 
   auto bar = [&](int i) { return sbase + L.bar_off + 8u * (uint32_t)i; };
   const uint32_t wbar = bar(0);
@@ -176,6 +209,11 @@ __global__ void __launch_bounds__(kThreads, 1)
   const uint32_t accA_full = bar(1 + 4 * kMaxSt), accA_free = bar(2 + 4 * kMaxSt);
   auto accB_full = [&](int s) { return bar(3 + 4 * kMaxSt + s); };
   auto accB_free = [&](int s) { return bar(5 + 4 * kMaxSt + s); };
+  auto fullAp = [&](int s) { return bar(7 + 4 * kMaxSt + s); };  // leader: the peer's input stage s is full
+  auto fullBp = [&](int s) { return bar(7 + 5 * kMaxSt + s); };  // leader: the peer's mid stage s is full
+  // B's MMA commits arrive once per CTA (cta_group::1) or once per pair (cta_group::2) that
+  // touches this CTA's neighbourhood {rank-1, rank, rank+1}
+  const int ncommit = CG2 ? 1 + ((pr == 0 ? has_left : has_right) ? 1 : 0) : nnb;
   auto stA = [&](int s) { return sbase + L.stA_off + (uint32_t)s * L.stA_bytes; };
   auto stB = [&](int s) { return sbase + L.stB_off + (uint32_t)s * L.stB_bytes; };
   volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + L.tmem_off);
@@ -194,22 +232,31 @@ __global__ void __launch_bounds__(kThreads, 1)
       // warps of this CTA - and the stages of the neighbours, which this CTA also writes,
       // must be free too
       mbar_init(fullB(s), kEpiWarps);
-      mbar_init(emptyB(s), (1 + kEpiWarps) * nnb);
+      mbar_init(emptyB(s), ncommit + kEpiWarps * nnb);
+      mbar_init(fullAp(s), 1);
+      mbar_init(fullBp(s), 1);
     }
     mbar_init(accA_full, 1);
-    mbar_init(accA_free, kEpiWarps);
+    mbar_init(accA_free, CG2 ? 2 * kEpiWarps : kEpiWarps);  // cta_group::2: both CTAs' epilogues, on the leader
     for (int s = 0; s < 2; ++s) {
       mbar_init(accB_full(s), 1);
-      mbar_init(accB_free(s), kEpiWarps);
+      mbar_init(accB_free(s), CG2 ? 2 * kEpiWarps : kEpiWarps);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
   if (warp == 18) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(sbase + L.tmem_off),
-                 "n"(kTmemCols)
-                 : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    if (CG2) {  // the same warp of both CTAs, the same destination offset
+      asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(sbase + L.tmem_off),
+                   "n"(kTmemCols)
+                   : "memory");
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+    } else {
+      asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(sbase + L.tmem_off),
+                   "n"(kTmemCols)
+                   : "memory");
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
   }
   // the mid stages start as zeros: positions outside the frame (left of segment 0, right of the
   // last segment) are never written and ARE the zero padding of layer B
@@ -230,10 +277,18 @@ __global__ void __launch_bounds__(kThreads, 1)
     // =========================== TMA producer (layer A's input rows, both layers' weights)
     if (elect_one()) {
       mbar_expect_tx(wbar, 2u * L.w_bytes);
-      for (uint32_t off = 0; off < L.w_bytes; off += 16384u) {
-        const uint32_t n = L.w_bytes - off < 16384u ? L.w_bytes - off : 16384u;
-        bulk_load(sbase + L.wA_off + off, wpackA + off, n, wbar);
-        bulk_load(sbase + L.wB_off + off, wpackB + off, n, wbar);
+      if (CG2) {  // per (kx, input chunk) plane: the rows of this CTA's halves of the three windows
+        const uint32_t prow = pair_wrows(C, true) * 16u, skip = (uint32_t)pr * (3u * C / 2u) * 16u;
+        for (uint32_t pl = 0; pl < 3u * (C / 8); ++pl) {
+          bulk_load(sbase + L.wA_off + pl * prow, wpackA + pl * (5u * C * 16u) + skip, prow, wbar);
+          bulk_load(sbase + L.wB_off + pl * prow, wpackB + pl * (5u * C * 16u) + skip, prow, wbar);
+        }
+      } else {
+        for (uint32_t off = 0; off < L.w_bytes; off += 16384u) {
+          const uint32_t n = L.w_bytes - off < 16384u ? L.w_bytes - off : 16384u;
+          bulk_load(sbase + L.wA_off + off, wpackA + off, n, wbar);
+          bulk_load(sbase + L.wB_off + off, wpackB + off, n, wbar);
+        }
       }
     }
     __syncwarp();
@@ -284,9 +339,11 @@ __global__ void __launch_bounds__(kThreads, 1)
     // =========================== MMA issuer of layer A
     asm volatile("griddepcontrol.wait;" ::: "memory");
     wait_bar<false>(wbar, 0);
-    constexpr uint32_t idesc = umma_idesc(kTileM, 3 * C, F16);
+    constexpr uint32_t idesc = umma_idesc(CG2 ? 2 * kTileM : kTileM, 3 * C, F16);
     const uint32_t plane16 = planeA >> 4;
-    constexpr uint32_t wplane16 = 5u * C;
+    constexpr uint32_t wplane16 = pair_wrows(C, CG2);
+    const uint16_t pair_mask = (uint16_t)(3u << leader_rank);
+    const uint32_t relayA = CG2 && !leader ? mapa(fullAp(0), leader_rank) : 0u;
     constexpr uint32_t desc_hi = (128u >> 4) | (1u << 14);
     const uint32_t a_lo_base = (plane16 << 16) | (((sbase + L.stA_off) >> 4) & 0x3FFFu);
     const uint32_t b_lo_base = (wplane16 << 16) | (((sbase + L.wA_off) >> 4) & 0x3FFFu);
@@ -301,6 +358,17 @@ __global__ void __launch_bounds__(kThreads, 1)
       for (int t = 0; t < run.n + 6; ++t, row += d) {
         const bool in_valid = row >= 0 && row < geo.H;
         if (in_valid) wait_bar<false>(fullA((int)st), full_par);
+        if (CG2 && !leader) {
+          // the peer of a pair issues nothing: it tells the leader that its stage has landed
+          if (in_valid && elect_one()) mbar_arrive_cluster(relayA + 8u * st);
+          __syncwarp();
+          if (in_valid && ++st == (uint32_t)nA) {
+            st = 0;
+            full_par ^= 1u;
+          }
+          continue;
+        }
+        if (CG2 && in_valid) wait_bar<false>(fullAp((int)st), full_par);
         wait_bar<false>(accA_free, free_par);
         free_par ^= 1u;
         tc_fence_after();
@@ -315,12 +383,15 @@ __global__ void __launch_bounds__(kThreads, 1)
               for (int ks = 0; ks < C / 16; ++ks) {
                 const uint32_t al = a_lo + (uint32_t)(2 * ks) * plane16 + (uint32_t)(kx * d);
                 const uint32_t bl = b_lo + (uint32_t)(kx * (C / 8) + 2 * ks) * wplane16;
-                tc_mma(dcol, ((uint64_t)desc_hi << 32) | al, ((uint64_t)desc_hi << 32) | bl, idesc, 1u);
+                if (CG2) tc_mma2(dcol, ((uint64_t)desc_hi << 32) | al, ((uint64_t)desc_hi << 32) | bl, idesc);
+                else tc_mma(dcol, ((uint64_t)desc_hi << 32) | al, ((uint64_t)desc_hi << 32) | bl, idesc, 1u);
               }
             }
-            tc_commit(emptyA((int)st));
+            if (CG2) tc_commit2_mc(emptyA((int)st), pair_mask);
+            else tc_commit(emptyA((int)st));
           }
-          tc_commit(accA_full);
+          if (CG2) tc_commit2_mc(accA_full, pair_mask);
+          else tc_commit(accA_full);
         }
         __syncwarp();
         if (in_valid && ++st == (uint32_t)nA) {
@@ -334,16 +405,22 @@ __global__ void __launch_bounds__(kThreads, 1)
     // =========================== MMA issuer of layer B (two interleaved chains)
     asm volatile("griddepcontrol.wait;" ::: "memory");
     wait_bar<false>(wbar, 0);
-    constexpr uint32_t idesc = umma_idesc(kTileM, 3 * C, F16);
+    constexpr uint32_t idesc = umma_idesc(CG2 ? 2 * kTileM : kTileM, 3 * C, F16);
     const uint32_t plane16 = planeB >> 4;
-    constexpr uint32_t wplane16 = 5u * C;
+    constexpr uint32_t wplane16 = pair_wrows(C, CG2);
+    const uint16_t pair_mask = (uint16_t)(3u << leader_rank);
+    const uint32_t relayB = CG2 && !leader ? mapa(fullBp(0), leader_rank) : 0u;
     constexpr uint32_t desc_hi = (128u >> 4) | (1u << 14);
     const uint32_t a_lo_base = (plane16 << 16) | (((sbase + L.stB_off) >> 4) & 0x3FFFu);
     const uint32_t b_lo_base = (wplane16 << 16) | (((sbase + L.wB_off) >> 4) & 0x3FFFu);
     const uint32_t stage16 = L.stB_bytes >> 4;
     const uint32_t dcol0 = __shfl_sync(0xffffffffu, tmem_base, 0) + 3u * C;
-    const uint16_t mask = (uint16_t)((1u << rank) | (has_left ? 1u << (rank - 1) : 0u) |
-                                     (has_right ? 1u << (rank + 1) : 0u));
+    // who hears that this CTA's (cta_group::2: this pair's) MMAs are done with a mid stage: the
+    // CTAs that write into it
+    const uint16_t mask = CG2 ? (uint16_t)((3u << leader_rank) | (leader_rank > 0 ? 1u << (leader_rank - 1) : 0u) |
+                                           ((int)leader_rank + 2 < nseg ? 1u << (leader_rank + 2) : 0u))
+                              : (uint16_t)((1u << rank) | (has_left ? 1u << (rank - 1) : 0u) |
+                                           (has_right ? 1u << (rank + 1) : 0u));
     PRuns runs;
     runs.init(geo, cid, ncl);
     PRun run;
@@ -359,6 +436,16 @@ __global__ void __launch_bounds__(kThreads, 1)
           // the neighbours' st.async data, observed through the barrier, before the MMAs read it
           asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         }
+        if (CG2 && !leader) {
+          if (in_valid && elect_one()) mbar_arrive_cluster(relayB + 8u * st);
+          __syncwarp();
+          if (in_valid && ++st == (uint32_t)nB) {
+            st = 0;
+            full_par ^= 1u;
+          }
+          continue;
+        }
+        if (CG2 && in_valid) wait_bar<false>(fullBp((int)st), full_par);
         wait_bar<false>(accB_free(s), s ? free_par1 : free_par0);
         if (s) free_par1 ^= 1u;
         else free_par0 ^= 1u;
@@ -376,13 +463,16 @@ __global__ void __launch_bounds__(kThreads, 1)
               for (int ks = 0; ks < C / 16; ++ks) {
                 const uint32_t al = a_lo + (uint32_t)(2 * ks) * plane16 + (uint32_t)(kx * dB);
                 const uint32_t bl = b_lo + (uint32_t)(kx * (C / 8) + 2 * ks) * wplane16;
-                tc_mma(dcol, ((uint64_t)desc_hi << 32) | al, ((uint64_t)desc_hi << 32) | bl, idesc, 1u);
+                if (CG2) tc_mma2(dcol, ((uint64_t)desc_hi << 32) | al, ((uint64_t)desc_hi << 32) | bl, idesc);
+                else tc_mma(dcol, ((uint64_t)desc_hi << 32) | al, ((uint64_t)desc_hi << 32) | bl, idesc, 1u);
               }
             }
-            if (nnb > 1) tc_commit_mc(emptyB((int)st), mask);
+            if (CG2) tc_commit2_mc(emptyB((int)st), mask);
+            else if (nnb > 1) tc_commit_mc(emptyB((int)st), mask);
             else tc_commit(emptyB((int)st));
           }
-          tc_commit(accB_full(s));
+          if (CG2) tc_commit2_mc(accB_full(s), pair_mask);
+          else tc_commit(accB_full(s));
         }
         __syncwarp();
         if (in_valid && ++st == (uint32_t)nB) {
@@ -423,7 +513,13 @@ __global__ void __launch_bounds__(kThreads, 1)
       tc_wait_st();
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(accA_free);
+      // cta_group::2: the accumulator-free signals of both CTAs go to the leader, who issues
+      const uint32_t accA_free_t = CG2 && !leader ? mapa(accA_free, leader_rank) : accA_free;
+      auto arrive_accA_free = [&]() {
+        if (CG2 && !leader) mbar_arrive_cluster(accA_free_t);
+        else mbar_arrive(accA_free);
+      };
+      if (lane == 0) arrive_accA_free();
       // where this thread's pixel goes: own stage at dB + px; the first / last dB pixels of the
       // segment are also the right / left halo of the left / right neighbour's stage
       const bool to_left = has_left && px < dB, to_right = has_right && px >= kTileM - dB;
@@ -458,7 +554,7 @@ __global__ void __launch_bounds__(kThreads, 1)
           tc_wait_st();
           tc_fence_before();
           __syncwarp();
-          if (lane == 0) mbar_arrive(accA_free);
+          if (lane == 0) arrive_accA_free();
           // the residual of the mid row that the NEXT step finishes is this step's input row:
           // copy its centre pixels out now (conv_umma.cu, kEarly policy); the stage goes back
           // to the producer together with the mid stage's arrival below
@@ -531,9 +627,14 @@ __global__ void __launch_bounds__(kThreads, 1)
       tc_wait_st();
       tc_fence_before();
       __syncwarp();
+      const uint32_t accB_free_t0 = CG2 && !leader ? mapa(accB_free(0), leader_rank) : accB_free(0);
+      auto arrive_accB_free = [&](int c) {
+        if (CG2 && !leader) mbar_arrive_cluster(accB_free_t0 + 8u * (uint32_t)c);
+        else mbar_arrive(accB_free(c));
+      };
       if (lane == 0) {
-        mbar_arrive(accB_free(0));
-        mbar_arrive(accB_free(1));
+        arrive_accB_free(0);
+        arrive_accB_free(1);
       }
       asm volatile("griddepcontrol.wait;" ::: "memory");
       const size_t plane_px = (size_t)geo.H * geo.W;
@@ -571,7 +672,7 @@ __global__ void __launch_bounds__(kThreads, 1)
           tc_wait_st();
           tc_fence_before();
           __syncwarp();
-          if (lane == 0) mbar_arrive(accB_free(s));
+          if (lane == 0) arrive_accB_free(s);
           // HEAD (K3 folded in, as conv_umma.cu): every head is the sum of two fmaf chains, one per
           // channel half (head_post.cu evaluates the same two chains); heads are updated two at a
           // time with fma.rn.f32x2 (two independent IEEE fp32 FMAs: the same bits as fmaf).
@@ -672,17 +773,20 @@ __global__ void __launch_bounds__(kThreads, 1)
   cluster_sync_all();
   if (warp == 18) {
     tc_fence_after();
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(kTmemCols) : "memory");
+    if (CG2)
+      asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(kTmemCols) : "memory");
+    else
+      asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(kTmemCols) : "memory");
   }
 }
 
 // stages: mid needs 3 (being written / read by the MMAs / waiting for its residual copy); the
 // rest of the shared memory goes to the input ring, then to mid
-bool pick_pair_stages(int C, int d, bool head, int* nA, int* nB) {
+bool pick_pair_stages(int C, int d, bool head, bool cg2, int* nA, int* nB) {
   const uint32_t budget = 227u * 1024u - 1024u;
   static const int pref[][2] = {{4, 4}, {4, 3}, {3, 3}, {3, 2}, {2, 2}};
   for (const auto& p : pref) {
-    if (pair_smem(C, d, p[0], p[1], head).total <= budget) {
+    if (pair_smem(C, d, p[0], p[1], head, cg2).total <= budget) {
       *nA = p[0];
       *nB = p[1];
       return true;
@@ -691,7 +795,16 @@ bool pick_pair_stages(int C, int d, bool head, int* nA, int* nB) {
   return false;
 }
 
-template <int C, bool HEAD, bool F16>
+// cta_group::2 (one M = 256 MMA per CTA pair, B operand split between the two CTAs) needs an
+// even number of segments per row.  Measured (profiles/conv_pair_r2.md): the shared-memory
+// pipe drops from 95 % to 66 % busy, but layer A's serial loop MMA -> epilogue reads its TMEM
+// slot -> next MMA now crosses the SM pair twice per step (multicast commit out, remote
+// mbarrier arrive back), so at full clocks the kernel is ~7 % SLOWER than cta_group::1; in the
+// sustained, power-capped step it is ~1.6 % FASTER (fewer operand bytes per FLOP).  The
+// sustained step is what counts: on by default, SMLM_FUSE_PAIRS_1CTA selects cta_group::1.
+bool pair_uses_cg2(int nseg, bool allow) { return allow && nseg % 2 == 0; }
+
+template <int C, bool HEAD, bool F16, bool CG2>
 cudaError_t launch_pair_t(const void* in, void* out, PGeo geo, const void* wA, const void* wB, const LayerConst& lcA,
                           const LayerConst& lcB, int nA, int nB, size_t smem, const HeadArgs& ha, int n_sm,
                           cudaStream_t st) {
@@ -700,7 +813,7 @@ cudaError_t launch_pair_t(const void* in, void* out, PGeo geo, const void* wA, c
   int dev = 0;
   cudaGetDevice(&dev);
   if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
-  auto kern = conv_pair_kernel<C, HEAD, F16>;
+  auto kern = conv_pair_kernel<C, HEAD, F16, CG2>;
   if (!attr_done[dev]) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) return e;
@@ -737,17 +850,17 @@ cudaError_t launch_pair_t(const void* in, void* out, PGeo geo, const void* wA, c
                             (const uint8_t*)wB, nA, nB, lcA, lcB, ha);
 }
 
-template <int C>
+template <int C, bool CG2>
 cudaError_t launch_pair_c(bool f16, const void* in, void* out, PGeo geo, const void* wA, const void* wB,
                           const LayerConst& lcA, const LayerConst& lcB, int nA, int nB, size_t smem, const HeadArgs* ha,
                           int n_sm, cudaStream_t st) {
   static const HeadArgs h0{};
   if (f16) {
-    if (ha) return launch_pair_t<C, true, true>(in, out, geo, wA, wB, lcA, lcB, nA, nB, smem, *ha, n_sm, st);
-    return launch_pair_t<C, false, true>(in, out, geo, wA, wB, lcA, lcB, nA, nB, smem, h0, n_sm, st);
+    if (ha) return launch_pair_t<C, true, true, CG2>(in, out, geo, wA, wB, lcA, lcB, nA, nB, smem, *ha, n_sm, st);
+    return launch_pair_t<C, false, true, CG2>(in, out, geo, wA, wB, lcA, lcB, nA, nB, smem, h0, n_sm, st);
   }
-  if (ha) return launch_pair_t<C, true, false>(in, out, geo, wA, wB, lcA, lcB, nA, nB, smem, *ha, n_sm, st);
-  return launch_pair_t<C, false, false>(in, out, geo, wA, wB, lcA, lcB, nA, nB, smem, h0, n_sm, st);
+  if (ha) return launch_pair_t<C, true, false, CG2>(in, out, geo, wA, wB, lcA, lcB, nA, nB, smem, *ha, n_sm, st);
+  return launch_pair_t<C, false, false, CG2>(in, out, geo, wA, wB, lcA, lcB, nA, nB, smem, h0, n_sm, st);
 }
 
 }  // namespace
@@ -756,12 +869,13 @@ bool conv_pair_supports(int C, int dA, int dB, int W) {
   int nA, nB;
   // TMEM: 9 slots of C columns; cluster = segments of a row
   return C >= 16 && C <= 48 && C % 16 == 0 && dA >= 1 && dB == 2 * dA && dB <= 16 && W >= 1 &&
-         (W + kTileM - 1) / kTileM <= kMaxCluster && pick_pair_stages(C, dA, true, &nA, &nB);
+         (W + kTileM - 1) / kTileM <= kMaxCluster &&
+         pick_pair_stages(C, dA, true, false, &nA, &nB);  // (cta_group::2 needs less shared memory)
 }
 
 cudaError_t launch_conv_pair(bool f16, const void* in, void* out, ActShape s, int dA, const void* wpackA,
                              const void* wpackB, const LayerConst& lcA, const LayerConst& lcB, const HeadArgs* head,
-                             int n_sm, cudaStream_t st, char* err, size_t errlen) {
+                             bool allow_cg2, int n_sm, cudaStream_t st, char* err, size_t errlen) {
   if (!conv_pair_supports(s.C, dA, 2 * dA, s.W)) {
     snprintf(err, errlen, "unsupported layer pair");
     return cudaErrorInvalidValue;
@@ -776,13 +890,19 @@ cudaError_t launch_conv_pair(bool f16, const void* in, void* out, ActShape s, in
   geo.Lmax = (s.H + dA - 1) / dA;
   geo.total = (long long)s.B * dA * geo.Lmax;
   int nA = 0, nB = 0;
-  pick_pair_stages(s.C, dA, head != nullptr, &nA, &nB);
-  const size_t smem = pair_smem(s.C, dA, nA, nB, head != nullptr).total + 1024;
+  const bool cg2 = pair_uses_cg2(geo.nseg, allow_cg2);
+  pick_pair_stages(s.C, dA, head != nullptr, cg2, &nA, &nB);
+  const size_t smem = pair_smem(s.C, dA, nA, nB, head != nullptr, cg2).total + 1024;
+#define SMLM_PAIR_CASE(CC)                                                                                          \
+  case CC:                                                                                                          \
+    return cg2 ? launch_pair_c<CC, true>(f16, in, out, geo, wpackA, wpackB, lcA, lcB, nA, nB, smem, head, n_sm, st)  \
+               : launch_pair_c<CC, false>(f16, in, out, geo, wpackA, wpackB, lcA, lcB, nA, nB, smem, head, n_sm, st);
   switch (s.C) {
-    case 16: return launch_pair_c<16>(f16, in, out, geo, wpackA, wpackB, lcA, lcB, nA, nB, smem, head, n_sm, st);
-    case 32: return launch_pair_c<32>(f16, in, out, geo, wpackA, wpackB, lcA, lcB, nA, nB, smem, head, n_sm, st);
-    case 48: return launch_pair_c<48>(f16, in, out, geo, wpackA, wpackB, lcA, lcB, nA, nB, smem, head, n_sm, st);
+    SMLM_PAIR_CASE(16)
+    SMLM_PAIR_CASE(32)
+    SMLM_PAIR_CASE(48)
   }
+#undef SMLM_PAIR_CASE
   return cudaErrorInvalidValue;
 }
 

@@ -150,11 +150,12 @@ cudaError_t launch_conv_umma(bool f16, const void* in, void* out, ActShape s, in
 
 // K2 pair (conv_pair.cu): layers l and l+1 with dilations (d, 2d) in one kernel; the map between
 // them stays in shared memory.  Bit-identical to two launch_conv_umma calls.  head != nullptr:
-// layer l+1 is the last one (HEAD variant, `out` is not written).
+// layer l+1 is the last one (HEAD variant, `out` is not written).  allow_cg2: rows with an even
+// number of segments use tcgen05 cta_group::2 (one M = 256 MMA per CTA pair).
 bool conv_pair_supports(int C, int dA, int dB, int W);
 cudaError_t launch_conv_pair(bool f16, const void* in, void* out, ActShape s, int dA, const void* wpackA,
                              const void* wpackB, const LayerConst& lcA, const LayerConst& lcB, const HeadArgs* head,
-                             int n_sm, cudaStream_t st, char* err, size_t errlen);
+                             bool allow_cg2, int n_sm, cudaStream_t st, char* err, size_t errlen);
 
 // K3: 1x1 heads + threshold + 3x3 NMS + decode + warp-aggregated compaction.
 cudaError_t launch_head_post(int dt, const void* act, ActShape s, ViewSet vs,

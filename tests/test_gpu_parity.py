@@ -497,10 +497,12 @@ def test_layer_pairs_equal_unfused_bit_exact(C, nh, n, H, W, dil, tile):
     kw = dict(conv_impl=P.CONV_TCGEN05)
     if not tile:
         ma = G.gpu_forward_maps(spec, w, frames, ck, fusion=P.FUSE_HEAD, **kw)
-        mb = G.gpu_forward_maps(spec, w, frames, ck, fusion=P.FUSE_AUTO, **kw)
-        assert np.array_equal(ma, mb), float(np.max(np.abs(ma - mb)))
+        for fusion in (P.FUSE_AUTO, P.FUSE_PAIRS_1CTA):
+            mb = G.gpu_forward_maps(spec, w, frames, ck, fusion=fusion, **kw)
+            assert np.array_equal(ma, mb), (fusion, float(np.max(np.abs(ma - mb))))
     for thr in (0.5, 0.0):
         a = G.gpu_localize(spec, w, frames, ck, thr, fusion=P.FUSE_HEAD, tile=tile, **kw)
-        b = G.gpu_localize(spec, w, frames, ck, thr, fusion=P.FUSE_AUTO, tile=tile, **kw)
         assert len(a) > 0
-        assert len(a) == len(b) and a.tobytes() == b.tobytes(), thr
+        for fusion in (P.FUSE_AUTO, P.FUSE_PAIRS_1CTA):     # cta_group::2 where the row has an even number of segments / ::1
+            b = G.gpu_localize(spec, w, frames, ck, thr, fusion=fusion, tile=tile, **kw)
+            assert len(a) == len(b) and a.tobytes() == b.tobytes(), (thr, fusion)
