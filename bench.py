@@ -154,6 +154,124 @@ def run_reference(args, cfg):
     return 0
 
 
+def dloc_flop_per_px(spec):
+    """2 x MAC per full-resolution pixel (dloc.h): the DCD blocks and dec0 at full resolution,
+    enc1 / dec1 at 1/4 of the pixels, enc2 at 1/16."""
+    C = spec.c0
+    f = 0.0
+    for name, co, ci, k in spec.layers():
+        scale = {"enc1": 0.25, "dec1": 0.25, "enc2": 1.0 / 16}.get(name, 1.0)
+        f += 2.0 * co * ci * k * k * scale
+    return f
+
+
+def run_dloc(args, cfg):
+    """The paper's own topology through dloc_localize: same step, timing and JSON contract as
+    the headline path (one step = one call over the whole stack; value device-resident, e2e
+    from pinned host frames to a pinned host list)."""
+    import dataclasses
+    import torch
+    import paper_2410_02314_b200 as P
+    from paper_2410_02314_b200 import dloc_binding as DB
+    from smlm_synth import DlocSpec, dloc_he_normal_blob
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    if int(os.environ.get("RANK", "0")) != 0:
+        return 0
+    torch.cuda.set_device(0)
+    spec = DlocSpec(precision=args.precision or "bf16")
+    n_frames = args.frames or cfg.frames.n_frames
+    fs, frames = workload(cfg, n_frames)
+    H, W = frames.shape[1:]
+    weights = dloc_he_normal_blob(spec, 7, head_gain=0.5)
+    conv_impl = {"auto": P.CONV_AUTO, "tcgen05": P.CONV_TCGEN05, "direct": P.CONV_DIRECT}[args.conv_impl]
+    loc = DB.DlocLocalizer(DB.dloc_desc_from_spec(spec, micro_batch=args.micro_batch, conv_impl=conv_impl), weights)
+    cap = n_frames * ((H + 1) // 2) * ((W + 1) // 2)
+    cap = min(cap, int(n_frames * max(8 * cfg.frames.emitters_per_frame, 4096)))
+    cam = loc.camera(fs.pixel_size_nm, fs.offset, fs.gain)
+    frames_host = torch.from_numpy(frames).pin_memory()
+    frames_dev = frames_host.cuda()
+    out_dev = torch.zeros(cap * 48, dtype=torch.uint8, device="cuda")
+    out_host = torch.zeros(cap * 48, dtype=torch.uint8).pin_memory()
+    stream = torch.cuda.Stream()
+    thr = 0.5
+
+    def timed(frames_t, out_t, steps, kernel_timing=False):
+        loc.kernel_timing(kernel_timing)
+        torch.cuda.synchronize()
+        l0 = loc.launch_count()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        counts = []
+        with torch.cuda.stream(stream):
+            e0.record(stream)
+            for _ in range(steps):
+                counts.append(loc.localize(frames_t, cam, thr, out_t, cap, stream=stream))
+            e1.record(stream)
+        torch.cuda.synchronize()
+        if loc.check() != P.OK:
+            raise SystemExit(f"dloc_check: {loc.check()} {loc.last_error()}")
+        kt = loc.conv_time_ms() if kernel_timing else None
+        loc.kernel_timing(False)
+        return e0.elapsed_time(e1), [int(getattr(c, "value", c)) for c in counts], loc.launch_count() - l0, kt
+
+    timed(frames_dev, out_dev, args.warmup)
+    timed(frames_host, out_host, 1)
+    sampler = ClockSampler(0)
+    sampler.start()
+    ms, counts, launches, _ = timed(frames_dev, out_dev, args.steps)
+    ms_e2e, counts_e2e, _, _ = timed(frames_host, out_host, args.steps)
+    ms_rf, _, _, (conv_ms, conv_n) = timed(frames_dev, out_dev, args.steps, kernel_timing=True)
+    sampler.stop_flag.set()
+    sampler.join(timeout=2)
+    peaks, peak_kind = load_peaks()
+    fpp = dloc_flop_per_px(spec)
+    stem_head = 2.0 * spec.c0 * spec.in_frames * 9 + 2.0 * spec.c0 * spec.head_channels   # not tensor-core work
+    conv_flop = (fpp - stem_head) * H * W * n_frames * args.steps
+    peak = float(peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]))
+    achieved = conv_flop / (conv_ms * 1e-3) / 1e12 if conv_ms > 0 else None
+    roofline = None
+    if achieved is not None:
+        roofline = {"bound": "tensor" if spec.precision != "fp32" and args.conv_impl != "direct" else "alu",
+                    "kernel": "conv_gen_umma_kernel (every convolution of the net except stem and heads)",
+                    "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                    "frac_of_burst": achieved / float(peaks["bf16_tflops"]), "traffic": None,
+                    "traffic_source": "no ncu --set full capture of this path",
+                    "peak_source": f"{peak_kind} bf16_tflops_sustained (kernels timed inside a long step)",
+                    "launches": conv_n, "avg_launch_ms": conv_ms / max(conv_n, 1), "share_of_step": conv_ms / ms_rf}
+    cpu = None
+    if not args.no_cpu_baseline:
+        from oracle import dloc as D
+        from oracle import oracle as O
+        ns = max(1, min(len(fs.frames), int(2.5e11 / (fpp * H * W))))    # ~15 s: this oracle runs at ~15 GFLOP/s
+        ocam = O.make_camera(fs.pixel_size_nm, fs.offset, fs.gain)
+        t0 = time.perf_counter()
+        o = D.forward_maps(D.net_from_spec(spec), weights, fs.frames[:ns], ocam)
+        em = D.postprocess(spec, o, ocam, thr)
+        dt = time.perf_counter() - t0
+        cpu = {"value": ns / dt, "unit": UNIT, "cores": O.threads(), "kind": "oracle",
+               "sample": f"first {ns} frame(s), {dt:.1f} s (oracle/dloc_oracle.c)", "emitters_per_s": len(em) / dt}
+    line = {"metric": METRIC, "value": n_frames * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": 1,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": {"bf16": "bf16"}.get(spec.precision, "f32"),
+            "data": "synthetic",
+            "config": {"workload": f"dloc_c{spec.c0}g{spec.growth}_b{spec.n_blocks}_on_{cfg.name}", "frames_per_step": n_frames,
+                       "H": H, "W": W, "c0": spec.c0, "growth": spec.growth, "n_blocks": spec.n_blocks,
+                       "dilations": list(spec.dilations), "head_channels": spec.head_channels,
+                       "precision": spec.precision, "conv_impl": args.conv_impl, "flop_per_px": fpp,
+                       "l2": "inputs larger than L2 (u16 stack + feature maps per step > 126 MB)",
+                       "parallelism": "replicas x1"},
+            "emitters_per_s": sum(counts) / (ms * 1e-3), "emitters_per_frame": sum(counts) / (n_frames * args.steps),
+            "e2e": {"value": n_frames * args.steps / (ms_e2e * 1e-3), "unit": UNIT,
+                    "h2d_bytes_per_step": int(frames.nbytes), "d2h_bytes_per_step": int(counts_e2e[-1] * 48 + 8),
+                    "ms_per_step": ms_e2e / args.steps, "exposed_copy_ms_per_step": (ms_e2e - ms) / args.steps},
+            "gpu_launches": launches, "clocks": sampler.summary(), "roofline": roofline, "cpu_baseline": cpu,
+            "tensor_frac_whole_step": (fpp * H * W * n_frames * args.steps / (ms * 1e-3) / 1e12)
+                                      / float(peaks["bf16_tflops"])}
+    print(json.dumps(line), flush=True)
+    loc.close()
+    return 0
+
+
 def _rank_entry(rank, world, port, argv):
     """One rank of a self-spawned run: the same environment torchrun would set."""
     os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), LOCAL_WORLD_SIZE=str(world),
@@ -205,6 +323,10 @@ def main(argv=None):
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1)
+    ap.add_argument("--net", default="stack", choices=["stack", "dloc"],
+                    help="stack: BASELINE.json's residual dilated stack (smlm.h, the headline); dloc: the paper's own "
+                         "topology (dloc.h, SURVEY.md 8(f)-2: DCD dense blocks, dilations 2-4-8-16, two-stage U-Net, "
+                         "ten heads) on the config's frames")
     ap.add_argument("--frames", type=int, default=0, help="override the number of frames per step")
     ap.add_argument("--conv-impl", default="auto", choices=["auto", "tcgen05", "direct"])
     ap.add_argument("--micro-batch", type=int, default=0)
@@ -231,6 +353,9 @@ def main(argv=None):
             cfg = dataclasses.replace(cfg, tile=args.tile)
         if args.precision:
             cfg = dataclasses.replace(cfg, net=dataclasses.replace(cfg.net, precision=args.precision))
+    if args.net == "dloc":
+        args.warmup = max(args.warmup, 3)
+        return run_dloc(args, cfg)
     if args.impl == "reference":
         return run_reference(args, cfg)
     args.warmup = max(args.warmup, 3)
