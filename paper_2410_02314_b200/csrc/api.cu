@@ -833,7 +833,12 @@ smlm_status smlm_localize_ring(smlm_ctx* c, smlm_ring* ring, const smlm_camera_p
   if (!ring->pinned) return fail(c, SMLM_ERR_INVALID_ARG, "the ring is pageable (SMLM_RING_PAGEABLE is for tests)");
   if (c->in_frames == 3)
     return fail(c, SMLM_ERR_INVALID_ARG, "in_frames = 3 needs the whole stack (smlm_localize): ring chunks have no neighbours");
-  ring_rewind(ring);
+  {
+    std::lock_guard<std::mutex> lk(ring->mu);
+    if (ring->by_hand > 0)
+      return fail(c, SMLM_ERR_INVALID_ARG, "chunks taken with smlm_ring_acquire have not been released");
+  }
+  ring_rewind(ring);  // waits for the previous pass's copies to have drained their slots
   Call k;
   smlm_status r = call_begin(k, c, ring->n_frames, ring->H, ring->W, cam, threshold, out, out_count, true,
                              ring->chunk_frames, static_cast<cudaStream_t>(cuda_stream));
@@ -841,13 +846,23 @@ smlm_status smlm_localize_ring(smlm_ctx* c, smlm_ring* ring, const smlm_camera_p
   for (int64_t ck = 0; ck < ring->n_chunks; ++ck) {
     const uint16_t* p = ring_wait_chunk(ring, ck);  // blocks on the disk only
     if (!p) return fail(c, SMLM_ERR_INVALID_ARG, "frame file: %s", ring->error.c_str());
-    if ((r = call_frames(k, p, ck * ring->chunk_frames, ring->frames_of(ck), true)) != SMLM_OK) return r;
+    if ((r = call_frames(k, p, ck * ring->chunk_frames, ring->frames_of(ck), true)) != SMLM_OK) {
+      cudaStreamSynchronize(c->copy_stream);  // a failed call must not leave a chunk handed out
+      ring_release_chunk(ring, ck);
+      return r;
+    }
     // the slot goes back to the readers when the copy stream has drained this chunk's copies
     RingRelease* rr = new (std::nothrow) RingRelease{ring, ck};
-    if (!rr) return fail(c, SMLM_ERR_OOM, "host allocation failed");
+    if (!rr) {
+      cudaStreamSynchronize(c->copy_stream);
+      ring_release_chunk(ring, ck);
+      return fail(c, SMLM_ERR_OOM, "host allocation failed");
+    }
     cudaError_t e = cudaLaunchHostFunc(c->copy_stream, ring_release_cb, rr);
     if (e != cudaSuccess) {
       delete rr;
+      cudaStreamSynchronize(c->copy_stream);
+      ring_release_chunk(ring, ck);
       return fail(c, SMLM_ERR_CUDA, "cudaLaunchHostFunc: %s", cudaGetErrorString(e));
     }
   }

@@ -74,6 +74,7 @@ const uint16_t* ring_wait_chunk(smlm_ring* r, int64_t k) {
   r->touched = true;
   r->cv.wait(lk, [&] { return r->stop || r->loaded[s] == k; });
   if (r->loaded[s] != k) return nullptr;
+  ++r->outstanding;
   return r->buf + (size_t)s * r->slot_elems();
 }
 
@@ -84,18 +85,24 @@ void ring_release_chunk(smlm_ring* r, int64_t k) {
     if (r->loaded[s] == k) {
       r->loaded[s] = -1;
       r->free_from[s] = k + r->n_slots;
+      --r->outstanding;
     }
   }
   r->cv.notify_all();
 }
 
 // Start over at chunk 0.  Nothing to do on a ring no chunk of which has been handed out; else
-// the readers' pending assignments are voided (generation bump) and the call waits for reads
-// in flight, so that no stale reader writes into a slot of the new pass.
+// wait until every chunk handed out has been released (smlm_localize_ring releases from a
+// callback of its copy stream: the host may be several calls ahead of the GPU, the previous
+// pass's copies still read the slots, and a late release of old chunk k would otherwise free
+// the slot that holds new chunk k - the host then waits for that chunk forever), void the
+// readers' pending assignments (generation bump) and wait for reads in flight, so that no
+// stale reader writes into a slot of the new pass.
 void ring_rewind(smlm_ring* r) {
   {
     std::unique_lock<std::mutex> lk(r->mu);
     if (!r->touched) return;
+    r->cv.wait(lk, [&] { return r->stop || r->outstanding == 0; });
     ++r->gen;
     r->cv.notify_all();
     r->cv.wait(lk, [&] { return r->stop || r->active_reads == 0; });
@@ -195,11 +202,20 @@ smlm_status smlm_ring_acquire(smlm_ring* r, const uint16_t** frames, int64_t* n_
   *n_frames = r->frames_of(k);
   if (first_frame) *first_frame = k * r->chunk_frames;
   r->next_acquire = k + 1;
+  {
+    std::lock_guard<std::mutex> lk(r->mu);
+    ++r->by_hand;
+  }
   return SMLM_OK;
 }
 
 smlm_status smlm_ring_release(smlm_ring* r, int64_t first_frame) {
   if (!r || first_frame < 0 || first_frame % r->chunk_frames) return SMLM_ERR_INVALID_ARG;
+  {
+    std::lock_guard<std::mutex> lk(r->mu);
+    const int64_t k = first_frame / r->chunk_frames;
+    if (r->loaded[(size_t)(k % r->n_slots)] == k && r->by_hand > 0) --r->by_hand;
+  }
   smlm::ring_release_chunk(r, first_frame / r->chunk_frames);
   return SMLM_OK;
 }

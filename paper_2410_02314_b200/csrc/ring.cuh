@@ -32,6 +32,8 @@ struct smlm_ring {
   int64_t gen = 0;       // bumped by a rewind: readers drop the chunk they were assigned before it
   int active_reads = 0;  // readers inside pread
   bool touched = false;  // a chunk has been handed out since the last rewind
+  int64_t outstanding = 0;  // chunks handed out and not yet released (a rewind waits for them)
+  int64_t by_hand = 0;      // ... of which through smlm_ring_acquire
   bool stop = false;
   std::string error;
   std::vector<std::thread> readers;
@@ -48,6 +50,8 @@ namespace smlm {
 const uint16_t* ring_wait_chunk(smlm_ring* r, int64_t k);
 // the slot of chunk k may be refilled (with chunk k + n_slots)
 void ring_release_chunk(smlm_ring* r, int64_t k);
-// all chunks start over (a ring can serve several passes over the file)
+// all chunks start over (a ring can serve several passes over the file).  Blocks until every
+// chunk handed out so far has been released: the previous pass's asynchronous H2D copies still
+// read the slots, and a release that arrived after the rewind would free a slot of the new pass.
 void ring_rewind(smlm_ring* r);
 }  // namespace smlm

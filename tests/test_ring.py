@@ -84,3 +84,36 @@ def test_localize_ring_equals_in_memory_localize(tmp_path, chunk, slots, threads
             assert len(em) == len(ref) and em.tobytes() == ref.tobytes()
         with P.Ring(path, n, H, W, chunk, pageable=True) as bad, pytest.raises(P.SmlmError):
             loc.localize_ring(bad, loc.camera(**ck), cfg.threshold, buf, cap)
+
+
+@pytest.mark.gpu
+@pytest.mark.timeout(180)
+def test_localize_ring_back_to_back_calls_without_sync(tmp_path):
+    """The host enqueues several smlm_localize_ring calls before the GPU has finished the first:
+    each call rewinds the ring while the previous pass's H2D copies and slot releases are still
+    pending.  The rewind must wait for them (a late release of old chunk k used to free the slot
+    holding new chunk k, and the host then waited for that chunk forever; seen as a hung
+    bench.py --disk).  Every call must give the in-memory result."""
+    import torch
+    import gpu_util as G
+    from smlm_synth import get_config, make_frames, make_weights
+    cfg = get_config(1)
+    fs = make_frames(cfg, 4)
+    frames = np.ascontiguousarray(np.concatenate([fs.frames] * 16))           # 64 frames of 256 x 256
+    w = make_weights(cfg)
+    ck = G.cam_kwargs(fs)
+    ref = G.gpu_localize(cfg.net, w, frames, ck, cfg.threshold, host_frames=True, host_out=True)
+    path = _write(str(tmp_path), frames)
+    n, H, W = frames.shape
+    cap = n * 2048
+    calls = 12
+    with P.Localizer(P.desc_from_spec(cfg.net), w) as loc, P.Ring(path, n, H, W, 16, n_slots=2, n_threads=3) as ring:
+        stream = torch.cuda.Stream()
+        bufs = [torch.zeros(cap * 32, dtype=torch.uint8).pin_memory() for _ in range(calls)]
+        cam = loc.camera(**ck)
+        cnts = [loc.localize_ring(ring, cam, cfg.threshold, b, cap, stream=stream) for b in bufs]
+        torch.cuda.synchronize()
+        assert loc.check() == P.OK, loc.last_error()
+        for b, c in zip(bufs, cnts):
+            em = P.emitters_to_numpy(b, c.value)
+            assert len(em) == len(ref) and em.tobytes() == ref.tobytes()
