@@ -41,7 +41,7 @@ def load_peaks():
     return dict(FALLBACK_PEAKS), "fallback"
 
 
-def lookup_traffic(cfg, C, views, bound, pair=False):
+def lookup_traffic(cfg, C, views, bound, pair=False, fusion="auto"):
     """(bytes per full-size launch, provenance) of the dominant K2 kernel from profiles/traffic_r2.json."""
     path = os.path.join(ROOT, "profiles", "traffic_r2.json")
     if bound != "tensor" or not os.path.exists(path):
@@ -52,7 +52,9 @@ def lookup_traffic(cfg, C, views, bound, pair=False):
     cap = doc.get("captures", {}).get(f"{wl}/views{views}")
     if not cap:
         return None, f"no capture for {wl}/views{views} in profiles/traffic_r2.json"
-    name = f"conv_pair_kernel<{C},-,->" if pair else f"conv_umma_kernel<{C},-,->"
+    name = f"conv_umma_kernel<{C},-,->"
+    if pair:   # cta_group::2 where a row has an even number of segments (conv_pair.cu)
+        name = f"conv_pair_kernel<{C},-,-,{'cg2' if (-(-cfg.frames.width // 128)) % 2 == 0 and fusion != 'pairs1' else 'cg1'}>"
     k = cap["per_kernel_mean"].get(name)
     if not k:
         return None, f"capture {wl}/views{views} holds no {name} launch"
@@ -519,7 +521,7 @@ def main(argv=None):
         # kernel in this launch shape, from the tracked ncu --set full record
         # (profiles/traffic_r2.json, written by paper_2410_02314_b200/profile_tools.py from the
         # capture named there); null when no capture of this (workload, views per launch) exists.
-        traffic, traffic_note = lookup_traffic(cfg, C, loc_views_per_launch, bound, dominant_pair)
+        traffic, traffic_note = lookup_traffic(cfg, C, loc_views_per_launch, bound, dominant_pair, args.fusion)
         roofline = {"bound": bound,
                     "kernel": "conv3x3_dilated x2, layers (d, 2d) fused (conv_pair_kernel)" if dominant_pair
                               else "conv3x3_dilated (conv_umma_kernel)",
