@@ -71,7 +71,9 @@ typedef struct {
   float norm_scale, xy_scale, z_scale_nm, photon_scale, bg_scale;
   float sigma_xy_px, sigma_z_nm, sigma_photons; /* D7 */
   int32_t micro_batch;  /* frames per launch set; 0 = library default */
-  int32_t conv_impl;    /* SMLM_CONV_AUTO / TCGEN05 / DIRECT (16-bit precision only) */
+  int32_t conv_impl;    /* 16-bit precision only.  SMLM_CONV_AUTO: tcgen05, the dense-block layers through the
+                           row-chain kernel (conv_chain.cu); TCGEN05: every convolution through the generic
+                           tcgen05 kernel (the twin); DIRECT: CUDA cores */
 } dloc_net_desc;
 
 /* smlm_emitter plus the four uncertainties. */

@@ -26,6 +26,8 @@ struct GLayer {
   void* wpack = nullptr;     // tensor-core image (16-bit modes, tcgen05 path)
   float* w_direct = nullptr; // [k*k][CI][CO] fp32 (values rounded to the storage type in 16-bit modes)
   float* bias = nullptr;     // [CO]
+  void* wchain = nullptr;    // conv_chain.cu's image (dense-block layers on the tcgen05 path)
+  LayerConst lc{};           // the bias again, as a kernel parameter of conv_chain
 };
 
 struct Bufs {
@@ -43,6 +45,7 @@ struct dloc_ctx {
   int dt = ACT_F32;
   int in_frames = 1;
   bool use_umma = false;
+  bool use_chain = true;  // dense-block layers through conv_chain.cu (SMLM_CONV_TCGEN05 keeps the generic kernel: the twin)
   int n_sm = 0;
   int CB = 0;
   float *w_stem = nullptr, *b_stem = nullptr;
@@ -129,6 +132,13 @@ smlm_status make_layer(dloc_ctx* c, GLayer& L, int CI, int CO_real, int k, int d
     conv_gen_pack_host(CI, L.CO, CO_real, k, w, pack.data(), c->dt == ACT_F16);
     DCK(nullptr, cudaMalloc(&L.wpack, pack.size()));
     DCK(nullptr, cudaMemcpy(L.wpack, pack.data(), pack.size(), cudaMemcpyHostToDevice));
+    if (conv_chain_supports(CI, L.CO, k, d)) {  // the dense-block layers: row-chain kernel
+      std::vector<uint8_t> cp(conv_chain_packed_bytes(CI, L.CO));
+      conv_chain_pack_host(CI, L.CO, CO_real, w, cp.data(), c->dt == ACT_F16);
+      DCK(nullptr, cudaMalloc(&L.wchain, cp.size()));
+      DCK(nullptr, cudaMemcpy(L.wchain, cp.data(), cp.size(), cudaMemcpyHostToDevice));
+      for (int i = 0; i < L.CO && i < 64; ++i) L.lc.bias[i] = b[i];
+    }
   }
   *used = (size_t)CO_real * CI * taps + CO_real;
   return SMLM_OK;
@@ -136,6 +146,8 @@ smlm_status make_layer(dloc_ctx* c, GLayer& L, int CI, int CO_real, int k, int d
 
 void free_layer(GLayer& L) {
   if (L.wpack) cudaFree(L.wpack);
+  if (L.wchain) cudaFree(L.wchain);
+  L.wchain = nullptr;
   if (L.w_direct) cudaFree(L.w_direct);
   if (L.bias) cudaFree(L.bias);
   L.wpack = nullptr;
@@ -217,8 +229,12 @@ smlm_status conv(dloc_ctx* c, const GLayer& L, const void* in, int in_ch, int ci
     ++c->tev_used;
     DCK(c, cudaEventRecord(e0, st));
   }
-  cudaError_t e = c->use_umma ? launch_conv_gen_umma(c->dt == ACT_F16, a, L.wpack, L.bias, c->n_sm, st)
-                              : launch_conv_gen_direct(c->dt, a, L.w_direct, L.bias, st);
+  cudaError_t e;
+  if (c->use_umma && L.wchain && c->use_chain && a.ci_plane0 == 0 && !out_f32)
+    e = launch_conv_chain(c->dt == ACT_F16, a, L.wchain, L.lc, c->n_sm, st);
+  else
+    e = c->use_umma ? launch_conv_gen_umma(c->dt == ACT_F16, a, L.wpack, L.bias, c->n_sm, st)
+                    : launch_conv_gen_direct(c->dt, a, L.w_direct, L.bias, st);
   if (e != cudaSuccess) return dfail(c, SMLM_ERR_CUDA, "conv_gen: %s", cudaGetErrorString(e));
   if (c->timing) DCK(c, cudaEventRecord(e1, st));
   c->launches++;
@@ -394,6 +410,7 @@ smlm_status dloc_create(const dloc_net_desc* desc, const void* weights, dloc_ctx
   c->dt = desc->precision == SMLM_BF16 ? ACT_BF16 : (desc->precision == SMLM_FP16 ? ACT_F16 : ACT_F32);
   c->in_frames = desc->in_frames;
   c->use_umma = c->dt != ACT_F32 && desc->conv_impl != SMLM_CONV_DIRECT;
+  c->use_chain = desc->conv_impl == SMLM_CONV_AUTO;
   c->n_sm = prop.multiProcessorCount;
   c->CB = C + ND * G;
   smlm_status st = SMLM_OK;

@@ -103,7 +103,8 @@ def test_dloc_fp32_reference_mode_every_feature_map(spec, n, H, W):
     assert np.max(np.abs(sig(o[:, 6:]) - sig(og[:, 6:].astype(np.float64)))) < 1e-4
 
 
-@pytest.mark.parametrize("impl", [pytest.param(P.CONV_DIRECT, id="direct"), pytest.param(P.CONV_TCGEN05, id="tcgen05")])
+@pytest.mark.parametrize("impl", [pytest.param(P.CONV_DIRECT, id="direct"), pytest.param(P.CONV_TCGEN05, id="tcgen05"),
+                                  pytest.param(P.CONV_AUTO, id="auto")])
 @pytest.mark.parametrize("spec,n,H,W", CASES)
 def test_dloc_bf16_maps_and_emitters(spec, n, H, W, impl):
     spec = dataclasses.replace(spec, precision="bf16")
@@ -140,7 +141,7 @@ def test_dloc_bf16_maps_and_emitters(spec, n, H, W, impl):
                      abs(a["sz_nm"] - e["sz_nm"]) / spec.sigma_z_nm,
                      abs(a["s_photons"] - e["s_photons"]) / spec.sigma_photons)
     assert ds < 2e-2, ds
-    name = {P.CONV_DIRECT: "direct", P.CONV_TCGEN05: "tcgen05"}[impl]
+    name = {P.CONV_DIRECT: "direct", P.CONV_TCGEN05: "tcgen05", P.CONV_AUTO: "auto"}[impl]
     G.record(f"dloc_bf16_{name}_c{spec.c0}g{spec.growth}_{H}x{W}", gate=st, head_max_err=err, sigma_head_err=err_s,
              feature_rel_err=rel, sigma_rel_err=ds, launches=launches)
 
@@ -153,12 +154,13 @@ def test_dloc_tcgen05_matches_direct_bf16_feature_maps():
     frames = _frames(2, 45, 200, 3)
     ck = dict(pixel_size_nm=100.0, offset=100.0, gain=1.0)
     oa, da = _gpu_maps(spec, w, frames, ck, dump=True, conv_impl=P.CONV_DIRECT)
-    ob, db = _gpu_maps(spec, w, frames, ck, dump=True, conv_impl=P.CONV_TCGEN05)
-    for f in range(2):
-        assert np.array_equal(da[f]["stem"], db[f]["stem"])
-        for name in da[f]:
-            d = np.abs(da[f][name] - db[f][name]) / np.maximum(np.abs(da[f][name]), 1.0)
-            assert d.max() < 2.0 ** -5 and np.mean(d > 0) < 0.5, (name, d.max(), np.mean(d > 0))   # bf16 ulps pile up with depth
+    for impl in (P.CONV_TCGEN05, P.CONV_AUTO):     # generic tcgen05 kernel / dense-block layers through conv_chain.cu
+        ob, db = _gpu_maps(spec, w, frames, ck, dump=True, conv_impl=impl)
+        for f in range(2):
+            assert np.array_equal(da[f]["stem"], db[f]["stem"])
+            for name in da[f]:
+                d = np.abs(da[f][name] - db[f][name]) / np.maximum(np.abs(da[f][name]), 1.0)
+                assert d.max() < 2.0 ** -5 and np.mean(d > 0) < 0.5, (impl, name, d.max(), np.mean(d > 0))   # bf16 ulps pile up with depth
 
 
 def test_dloc_pipeline_host_ring_micro_batches_three_frames_and_edges():
