@@ -42,7 +42,8 @@ constexpr int kMaxDevices = 64;
 __device__ __align__(16) uint4 g_czeros[160];  // zero source for the padded parts of a row segment
 
 struct CGeo {
-  int B, H, W, d;
+  int B, H, W, d;         // d: row step of a chain = vertical dilation (1 for a 1x1 convolution)
+  int dx;                 // horizontal dilation = x halo of a row segment (0 for a 1x1 convolution)
   int nseg, Lmax;
   long long total;
   int CI;                 // input channels (multiple of 16)
@@ -77,10 +78,10 @@ struct CRuns {
 struct CSmem {
   uint32_t w_bytes, stage_off, stage_bytes, bar_off, tmem_off, total;
 };
-__host__ __device__ inline CSmem chain_smem(int CI, int CO, int d, int nstage) {
+__host__ __device__ inline CSmem chain_smem(int CI, int CO, int kx_taps, int dx, int nstage) {
   CSmem L;
-  L.w_bytes = 3u * (CI / 8) * 5u * CO * 16u;
-  L.stage_bytes = (((uint32_t)(CI / 8) * (kTileM + 2 * d) * 16u) + 127u) & ~127u;
+  L.w_bytes = (uint32_t)kx_taps * (CI / 8) * 5u * CO * 16u;
+  L.stage_bytes = (((uint32_t)(CI / 8) * (kTileM + 2 * dx) * 16u) + 127u) & ~127u;
   L.stage_off = (L.w_bytes + 127u) & ~127u;
   L.bar_off = L.stage_off + 2u * nstage * L.stage_bytes;
   L.tmem_off = L.bar_off + 8u * (1 + 2 * kLaneBars);
@@ -88,13 +89,16 @@ __host__ __device__ inline CSmem chain_smem(int CI, int CO, int d, int nstage) {
   return L;
 }
 
-template <int CO, bool F16>
+// KX = 3: 3x3 convolution.  KX = 1: 1x1 convolution (the transition of a dense block) run through
+// the same walk - one tap, no x halo, the weight rows of ky = 0 and ky = 2 are zero; the layer is
+// HBM-bound by a wide margin, so the idle two thirds of each MMA's N do not show.
+template <int CO, bool F16, int KX>
 __global__ void __launch_bounds__(kThreads, 1)
     conv_chain_kernel(const uint8_t* __restrict__ in, uint8_t* __restrict__ out, CGeo geo,
                       const uint8_t* __restrict__ wpack, int nstage, const __grid_constant__ LayerConst lc, int relu) {
   extern __shared__ uint8_t smem_raw[];
-  const int d = geo.d, CI = geo.CI;
-  const CSmem L = chain_smem(CI, CO, d, nstage);
+  const int d = geo.d, dx = geo.dx, CI = geo.CI;
+  const CSmem L = chain_smem(CI, CO, KX, dx, nstage);
   const uint32_t sraw = smem_u32(smem_raw);
   const uint32_t sbase = (sraw + 1023u) & ~1023u;
   uint8_t* smem = smem_raw + (sbase - sraw);
@@ -135,7 +139,7 @@ __global__ void __launch_bounds__(kThreads, 1)
   const uint32_t tmem_base = *tmem_slot;
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   const int nlanes = 2 * gridDim.x;
-  const uint32_t plane = (uint32_t)(kTileM + 2 * d) * 16u;
+  const uint32_t plane = (uint32_t)(kTileM + 2 * dx) * 16u;
 
   if (role == 0 || role == 2) {
     // =========================== TMA producers
@@ -158,7 +162,7 @@ __global__ void __launch_bounds__(kThreads, 1)
     uint32_t st = 0, empty_par = 1;
     int last_x0 = -1, fills_left = 0;
     while (runs.next(geo, run)) {
-      const int xl = run.x0 - d, xr = run.x0 + kTileM + d;
+      const int xl = run.x0 - dx, xr = run.x0 + kTileM + dx;
       const int lo = xl > 0 ? xl : 0, hi = xr < geo.W ? xr : geo.W;
       const uint32_t pre = (uint32_t)(lo - xl) * 16u, mid = (uint32_t)(hi - lo) * 16u, post = (uint32_t)(xr - hi) * 16u;
       if (run.x0 != last_x0) {
@@ -197,7 +201,7 @@ __global__ void __launch_bounds__(kThreads, 1)
     asm volatile("griddepcontrol.wait;" ::: "memory");
     mbar_wait(wbar, 0);
     constexpr uint32_t idesc = umma_idesc(kTileM, 3 * CO, F16);
-    const uint32_t plane16 = (uint32_t)(kTileM + 2 * d);
+    const uint32_t plane16 = (uint32_t)(kTileM + 2 * dx);
     constexpr uint32_t wplane16 = 5u * CO;
     constexpr uint32_t desc_hi = (128u >> 4) | (1u << 14);
     const uint32_t a_lo_base = (plane16 << 16) | (((sbase + L.stage_off) >> 4) & 0x3FFFu);
@@ -223,9 +227,9 @@ __global__ void __launch_bounds__(kThreads, 1)
         if (elect_one()) {
           if (in_valid) {
 #pragma unroll
-            for (int kx = 0; kx < 3; ++kx) {
+            for (int kx = 0; kx < KX; ++kx) {
               for (int ks = 0; ks < nks; ++ks) {
-                const uint32_t al = a_lo + (uint32_t)(2 * ks) * plane16 + (uint32_t)(kx * d);
+                const uint32_t al = a_lo + (uint32_t)(2 * ks) * plane16 + (uint32_t)(kx * dx);
                 const uint32_t bl = b_lo + (uint32_t)(kx * (CI / 8) + 2 * ks) * wplane16;
                 tc_mma(dcol, ((uint64_t)desc_hi << 32) | al, ((uint64_t)desc_hi << 32) | bl, idesc, 1u);
               }
@@ -318,9 +322,9 @@ __global__ void __launch_bounds__(kThreads, 1)
   }
 }
 
-int pick_chain_stages(int CI, int CO, int d) {
+int pick_chain_stages(int CI, int CO, int k, int d) {
   int nstage = kMaxStages;
-  while (nstage >= 2 && chain_smem(CI, CO, d, nstage).total + 1024 > 227u * 1024u) --nstage;
+  while (nstage >= 2 && chain_smem(CI, CO, k, k == 3 ? d : 0, nstage).total + 1024 > 227u * 1024u) --nstage;
   return nstage >= 2 ? nstage : 0;
 }
 
@@ -338,7 +342,7 @@ uint16_t bits16(float f, bool f16) {
   return (uint16_t)(u >> 16);
 }
 
-template <int CO, bool F16>
+template <int CO, bool F16, int KX>
 cudaError_t launch_t(const ConvGen& a, CGeo geo, const void* wpack, const LayerConst& lc, int nstage, int grid,
                      size_t smem, cudaStream_t st) {
   static bool attr_done[kMaxDevices] = {};
@@ -346,7 +350,7 @@ cudaError_t launch_t(const ConvGen& a, CGeo geo, const void* wpack, const LayerC
   cudaGetDevice(&dev);
   if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
   if (!attr_done[dev]) {
-    cudaError_t e = cudaFuncSetAttribute(conv_chain_kernel<CO, F16>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    cudaError_t e = cudaFuncSetAttribute(conv_chain_kernel<CO, F16, KX>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) return e;
     attr_done[dev] = true;
   }
@@ -360,31 +364,36 @@ cudaError_t launch_t(const ConvGen& a, CGeo geo, const void* wpack, const LayerC
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, conv_chain_kernel<CO, F16>, (const uint8_t*)a.in, (uint8_t*)a.out, geo,
+  return cudaLaunchKernelEx(&cfg, conv_chain_kernel<CO, F16, KX>, (const uint8_t*)a.in, (uint8_t*)a.out, geo,
                             (const uint8_t*)wpack, nstage, lc, a.relu);
 }
 
 }  // namespace
 
 bool conv_chain_supports(int CI, int CO, int k, int d) {
-  return k == 3 && (CO == 16 || CO == 32) && CI % 16 == 0 && CI >= 16 && CI <= 256 && d >= 1 && d <= 16 &&
-         pick_chain_stages(CI, CO, d) > 0;
+  const bool shape = (k == 3 && (CO == 16 || CO == 32)) || (k == 1 && (CO == 16 || CO == 32 || CO == 48) && d == 1);
+  return shape && CI % 16 == 0 && CI >= 16 && CI <= 256 && d >= 1 && d <= 16 && pick_chain_stages(CI, CO, k, d) > 0;
 }
 
-size_t conv_chain_packed_bytes(int CI, int CO) { return (size_t)3 * (CI / 8) * 5 * CO * 16; }
+size_t conv_chain_packed_bytes(int CI, int CO, int k) { return (size_t)k * (CI / 8) * 5 * CO * 16; }
 
-// w_oihw [CO_real][CI][3][3] fp32 -> shared-memory image: for kx, input chunk kc: 5 CO rows of
+// w_oihw [CO_real][CI][k][k] fp32 -> shared-memory image: for kx, input chunk kc: 5 CO rows of
 // 16 B (8 input channels), rows = output channels of ky = 1, 0, 2, 1, 0; rows >= CO_real zero.
-void conv_chain_pack_host(int CI, int CO, int CO_real, const float* w, void* dst, bool f16) {
+// k = 1: one kx tap, the rows of ky = 0 and ky = 2 zero.
+void conv_chain_pack_host(int CI, int CO, int CO_real, int k, const float* w, void* dst, bool f16) {
   static const int ky_seq[5] = {1, 0, 2, 1, 0};
   uint16_t* o = static_cast<uint16_t*>(dst);
-  for (int kx = 0; kx < 3; ++kx)
+  for (int kx = 0; kx < k; ++kx)
     for (int kc = 0; kc < CI / 8; ++kc)
       for (int n = 0; n < 5 * CO; ++n) {
         const int ky = ky_seq[n / CO], co = n % CO;
         for (int j = 0; j < 8; ++j) {
           const int ci = kc * 8 + j;
-          const float v = co < CO_real ? w[(((size_t)co * CI + ci) * 3 + ky) * 3 + kx] : 0.0f;
+          float v = 0.0f;
+          if (co < CO_real) {
+            if (k == 3) v = w[(((size_t)co * CI + ci) * 3 + ky) * 3 + kx];
+            else if (ky == 1) v = w[(size_t)co * CI + ci];
+          }
           o[(((size_t)(kx * (CI / 8) + kc) * 5 * CO) + n) * 8 + j] = bits16(v, f16);
         }
       }
@@ -399,6 +408,7 @@ cudaError_t launch_conv_chain(bool f16, const ConvGen& a, const void* wpack, con
   geo.H = a.H;
   geo.W = a.W;
   geo.d = a.d;
+  geo.dx = a.k == 3 ? a.d : 0;
   geo.nseg = (a.W + kTileM - 1) / kTileM;
   geo.Lmax = (a.H + a.d - 1) / a.d;
   geo.total = (long long)a.B * geo.nseg * a.d * geo.Lmax;
@@ -406,15 +416,21 @@ cudaError_t launch_conv_chain(bool f16, const ConvGen& a, const void* wpack, con
   geo.in_planes = a.in_planes;
   geo.out_planes = a.out_planes;
   geo.co_plane0 = a.co_plane0;
-  const int nstage = pick_chain_stages(a.CI, a.CO, a.d);
-  const size_t smem = chain_smem(a.CI, a.CO, a.d, nstage).total + 1024;
+  const int nstage = pick_chain_stages(a.CI, a.CO, a.k, a.d);
+  const size_t smem = chain_smem(a.CI, a.CO, a.k, geo.dx, nstage).total + 1024;
   long long want = (geo.total + 23) / 24;
   const int grid = (int)(want < 1 ? 1 : (want > n_sm ? n_sm : want));
-  if (a.CO == 16)
-    return f16 ? launch_t<16, true>(a, geo, wpack, lc, nstage, grid, smem, st)
-               : launch_t<16, false>(a, geo, wpack, lc, nstage, grid, smem, st);
-  return f16 ? launch_t<32, true>(a, geo, wpack, lc, nstage, grid, smem, st)
-             : launch_t<32, false>(a, geo, wpack, lc, nstage, grid, smem, st);
+#define SMLM_CHAIN_CASE(CC, KK)                                                              \
+  if (a.CO == CC && a.k == KK)                                                              \
+    return f16 ? launch_t<CC, true, KK>(a, geo, wpack, lc, nstage, grid, smem, st)          \
+               : launch_t<CC, false, KK>(a, geo, wpack, lc, nstage, grid, smem, st);
+  SMLM_CHAIN_CASE(16, 3)
+  SMLM_CHAIN_CASE(32, 3)
+  SMLM_CHAIN_CASE(16, 1)
+  SMLM_CHAIN_CASE(32, 1)
+  SMLM_CHAIN_CASE(48, 1)
+#undef SMLM_CHAIN_CASE
+  return cudaErrorInvalidValue;
 }
 
 }  // namespace smlm

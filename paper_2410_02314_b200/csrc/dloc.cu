@@ -133,8 +133,8 @@ smlm_status make_layer(dloc_ctx* c, GLayer& L, int CI, int CO_real, int k, int d
     DCK(nullptr, cudaMalloc(&L.wpack, pack.size()));
     DCK(nullptr, cudaMemcpy(L.wpack, pack.data(), pack.size(), cudaMemcpyHostToDevice));
     if (conv_chain_supports(CI, L.CO, k, d)) {  // the dense-block layers: row-chain kernel
-      std::vector<uint8_t> cp(conv_chain_packed_bytes(CI, L.CO));
-      conv_chain_pack_host(CI, L.CO, CO_real, w, cp.data(), c->dt == ACT_F16);
+      std::vector<uint8_t> cp(conv_chain_packed_bytes(CI, L.CO, k));
+      conv_chain_pack_host(CI, L.CO, CO_real, k, w, cp.data(), c->dt == ACT_F16);
       DCK(nullptr, cudaMalloc(&L.wchain, cp.size()));
       DCK(nullptr, cudaMemcpy(L.wchain, cp.data(), cp.size(), cudaMemcpyHostToDevice));
       for (int i = 0; i < L.CO && i < 64; ++i) L.lc.bias[i] = b[i];

@@ -35,11 +35,12 @@ void conv_gen_pack_host(int CI, int CO, int CO_real, int k, const float* w_oihw,
 // tcgen05 implicit GEMM (16-bit maps).  bias: device float [CO].
 cudaError_t launch_conv_gen_umma(bool f16, const ConvGen& a, const void* wpack, const float* bias, int n_sm,
                                  cudaStream_t st);
-// Row-chain kernel for the dense-block layers (conv_chain.cu): 3x3, C_out = 16 or 32, input planes
-// [0, CI / 8) of a buffer, weights resident in shared memory, every input row fetched once.
+// Row-chain kernel for the dense blocks (conv_chain.cu): the 3x3 dilated layers (C_out = 16 or 32) and
+// the 1x1 transition (C_out <= 48); input planes [0, CI / 8) of a buffer, weights resident in shared
+// memory, every input row fetched once.
 bool conv_chain_supports(int CI, int CO, int k, int d);
-size_t conv_chain_packed_bytes(int CI, int CO);
-void conv_chain_pack_host(int CI, int CO, int CO_real, const float* w_oihw, void* dst, bool f16);
+size_t conv_chain_packed_bytes(int CI, int CO, int k);
+void conv_chain_pack_host(int CI, int CO, int CO_real, int k, const float* w_oihw, void* dst, bool f16);
 cudaError_t launch_conv_chain(bool f16, const ConvGen& a, const void* wpack, const LayerConst& lc, int n_sm,
                               cudaStream_t st);
 // CUDA-core twin (fp32 math; maps float, bf16 or fp16).  w: device float [k * k][CI][CO].
