@@ -165,10 +165,12 @@ void free_bufs(dloc_ctx* c) {
 
 int auto_mb(const dloc_ctx* c, int H, int W) {
   if (c->d.micro_batch > 0) return c->d.micro_batch;
-  // ~ (2 CB + 4 C0 + quarter-resolution maps) channels per pixel; keep a launch set <= 2 GB
+  // ~ (2 CB + 4 C0 + quarter-resolution maps) channels per pixel; keep a launch set <= 8 GB.
+  // Up to 64 views per launch: the dense-block launches are short (~50 us at 26 views), so
+  // prologue and tail weigh (26 -> 64 views: 8.8 k -> see profiles/bench_r2.md frames/s).
   const double per_view = (double)H * W * esz(c) * (2.0 * c->CB + 5.0 * c->d.c0 + 3.0 * c->d.c0) + 40.0 * H * W;
-  int mb = (int)((2048.0 * 1048576.0) / per_view);
-  return std::max(1, std::min(mb, 32));
+  int mb = (int)((8192.0 * 1048576.0) / per_view);
+  return std::max(1, std::min(mb, 64));
 }
 
 smlm_status ensure_bufs(dloc_ctx* c, int mb, int H, int W, bool host_frames) {
