@@ -217,7 +217,7 @@ def run_dloc(args, cfg):
         return e0.elapsed_time(e1), [int(getattr(c, "value", c)) for c in counts], loc.launch_count() - l0, kt
 
     timed(frames_dev, out_dev, args.warmup)
-    timed(frames_host, out_host, 1)
+    timed(frames_host, out_host, args.warmup)
     sampler = ClockSampler(0)
     sampler.start()
     ms, counts, launches, _ = timed(frames_dev, out_dev, args.steps)
@@ -433,9 +433,15 @@ def main(argv=None):
         loc.kernel_timing(False)
         return ms, [int(c.value) for c in counts], loc.launch_count() - l0, kt
 
-    # warm-up (device-resident and end-to-end paths)
-    timed(frames_dev, out_dev, args.warmup)
-    timed(frames_host, out_host, 1)
+    # warm-up (device-resident and end-to-end paths): W steps each, then more device-resident
+    # steps until ~1.5 s of GPU work has run, so that the power-cap governor has settled (a
+    # process started on an idle GPU measured ~3 % low in its first second)
+    ms_w = timed(frames_dev, out_dev, args.warmup)[0]
+    timed(frames_host, out_host, args.warmup)
+    per_step = max(ms_w / args.warmup, 1e-3)
+    extra = int(min(200, max(0.0, 1500.0 - ms_w) / per_step))
+    if extra > 0:
+        timed(frames_dev, out_dev, extra)
 
     sampler = ClockSampler(local)
     sampler.start()
