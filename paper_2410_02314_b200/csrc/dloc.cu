@@ -26,8 +26,12 @@ struct GLayer {
   void* wpack = nullptr;     // tensor-core image (16-bit modes, tcgen05 path)
   float* w_direct = nullptr; // [k*k][CI][CO] fp32 (values rounded to the storage type in 16-bit modes)
   float* bias = nullptr;     // [CO]
-  void* wchain = nullptr;    // conv_chain.cu's image (dense-block layers on the tcgen05 path)
-  LayerConst lc{};           // the bias again, as a kernel parameter of conv_chain
+  // conv_chain.cu (tcgen05 path): one pass per group of `chain_co` output channels - the dense
+  // layers (growth 16: one pass), the transitions (one pass of C0), and dec0 (C0 / 16 passes of 16
+  // channels: its whole weight image does not fit in shared memory, a 16-channel slice does)
+  std::vector<void*> wchain;
+  std::vector<LayerConst> lc;  // the bias slices, as kernel parameters
+  int chain_co = 0;
 };
 
 struct Bufs {
@@ -132,12 +136,19 @@ smlm_status make_layer(dloc_ctx* c, GLayer& L, int CI, int CO_real, int k, int d
     conv_gen_pack_host(CI, L.CO, CO_real, k, w, pack.data(), c->dt == ACT_F16);
     DCK(nullptr, cudaMalloc(&L.wpack, pack.size()));
     DCK(nullptr, cudaMemcpy(L.wpack, pack.data(), pack.size(), cudaMemcpyHostToDevice));
-    if (conv_chain_supports(CI, L.CO, k, d)) {  // the dense-block layers: row-chain kernel
-      std::vector<uint8_t> cp(conv_chain_packed_bytes(CI, L.CO, k));
-      conv_chain_pack_host(CI, L.CO, CO_real, k, w, cp.data(), c->dt == ACT_F16);
-      DCK(nullptr, cudaMalloc(&L.wchain, cp.size()));
-      DCK(nullptr, cudaMemcpy(L.wchain, cp.data(), cp.size(), cudaMemcpyHostToDevice));
-      for (int i = 0; i < L.CO && i < 64; ++i) L.lc.bias[i] = b[i];
+    // row-chain kernel: the whole layer in one pass if it fits, else (3x3 only) 16 output channels per pass
+    L.chain_co = conv_chain_supports(CI, L.CO, k, d) ? L.CO : (k == 3 && conv_chain_supports(CI, 16, k, d) ? 16 : 0);
+    for (int co0 = 0; L.chain_co && co0 < L.CO; co0 += L.chain_co) {
+      const int n_real = std::max(0, std::min(L.chain_co, CO_real - co0));
+      std::vector<uint8_t> cp(conv_chain_packed_bytes(CI, L.chain_co, k));
+      conv_chain_pack_host(CI, L.chain_co, n_real, k, w + (size_t)co0 * CI * taps, cp.data(), c->dt == ACT_F16);
+      void* dev = nullptr;
+      DCK(nullptr, cudaMalloc(&dev, cp.size()));
+      L.wchain.push_back(dev);
+      DCK(nullptr, cudaMemcpy(dev, cp.data(), cp.size(), cudaMemcpyHostToDevice));
+      LayerConst lc{};
+      for (int i = 0; i < L.chain_co; ++i) lc.bias[i] = b[(size_t)co0 + i];
+      L.lc.push_back(lc);
     }
   }
   *used = (size_t)CO_real * CI * taps + CO_real;
@@ -146,8 +157,10 @@ smlm_status make_layer(dloc_ctx* c, GLayer& L, int CI, int CO_real, int k, int d
 
 void free_layer(GLayer& L) {
   if (L.wpack) cudaFree(L.wpack);
-  if (L.wchain) cudaFree(L.wchain);
-  L.wchain = nullptr;
+  for (void* p : L.wchain)
+    if (p) cudaFree(p);
+  L.wchain.clear();
+  L.lc.clear();
   if (L.w_direct) cudaFree(L.w_direct);
   if (L.bias) cudaFree(L.bias);
   L.wpack = nullptr;
@@ -231,10 +244,15 @@ smlm_status conv(dloc_ctx* c, const GLayer& L, const void* in, int in_ch, int ci
     ++c->tev_used;
     DCK(c, cudaEventRecord(e0, st));
   }
-  cudaError_t e;
-  if (c->use_umma && L.wchain && c->use_chain && a.ci_plane0 == 0 && !out_f32)
-    e = launch_conv_chain(c->dt == ACT_F16, a, L.wchain, L.lc, c->n_sm, st);
-  else
+  cudaError_t e = cudaSuccess;
+  if (c->use_umma && !L.wchain.empty() && c->use_chain && a.ci_plane0 == 0 && !out_f32) {
+    ConvGen p = a;
+    p.CO = L.chain_co;
+    for (size_t i = 0; i < L.wchain.size() && e == cudaSuccess; ++i) {
+      p.co_plane0 = a.co_plane0 + (int)i * L.chain_co / 8;
+      e = launch_conv_chain(c->dt == ACT_F16, p, L.wchain[i], L.lc[i], c->n_sm, st);
+    }
+  } else
     e = c->use_umma ? launch_conv_gen_umma(c->dt == ACT_F16, a, L.wpack, L.bias, c->n_sm, st)
                     : launch_conv_gen_direct(c->dt, a, L.w_direct, L.bias, st);
   if (e != cudaSuccess) return dfail(c, SMLM_ERR_CUDA, "conv_gen: %s", cudaGetErrorString(e));
