@@ -333,6 +333,8 @@ def main(argv=None):
     ap.add_argument("--conv-impl", default="auto", choices=["auto", "tcgen05", "direct"])
     ap.add_argument("--micro-batch", type=int, default=0)
     ap.add_argument("--fusion", default="auto", choices=["auto", "none", "all", "head", "pairs1"])
+    ap.add_argument("--stem", default="auto", choices=["auto", "tensor", "cuda"],
+                    help="K1 kernel: SMLM_STEM_AUTO / TENSOR (conv_chain.cu STEM variant) / CUDA_CORES (stem.cu)")
     ap.add_argument("--tile", type=int, default=-1, help="override the config's tile size (0: whole frames)")
     ap.add_argument("--tile-merge", default="auto", choices=["auto", "none", "row"],
                     help="row: one window per tile row (SMLM_TILE_MERGE_ROW); auto = row for a tiled config "
@@ -394,6 +396,7 @@ def main(argv=None):
     desc = P.desc_from_spec(cfg.net, tile=cfg.tile, micro_batch=args.micro_batch, conv_impl=conv_impl,
                             writeback_frames=cfg.writeback_batch,
                             tile_merge={"none": P.TILE_MERGE_NONE, "row": P.TILE_MERGE_ROW}[tile_merge],
+                            stem_impl={"auto": P.STEM_AUTO, "tensor": P.STEM_TENSOR, "cuda": P.STEM_CUDA_CORES}[args.stem],
                             fusion={"auto": P.FUSE_AUTO, "none": P.FUSE_NONE, "all": P.FUSE_ALL, "head": P.FUSE_HEAD, "pairs1": P.FUSE_PAIRS_1CTA}[args.fusion])
     loc = P.Localizer(desc, weights)
     cap = int(n_frames * max(4 * cfg.frames.emitters_per_frame, 1024))
@@ -547,8 +550,19 @@ def main(argv=None):
                                            "single_layer_launches": single_n, "pair_launches": pair_n,
                                            "share_of_step": conv_ms / ms_rf}}
     # K1 / K3: bytes moved per launch / CUDA-event time, against the
-    # measured HBM copy bandwidth (the maps they touch are L2-resident in this pipeline, so
-    # this is "bytes moved", not DRAM traffic).
+    # measured HBM copy bandwidth.  K1 is a pure WRITE stream (2 B in, 2C B out per pixel); a
+    # plain fill of device memory, measured here, is its real roof (profiles/stem_r2.md).
+    fill = torch.empty(1 << 30, dtype=torch.uint8, device="cuda")
+    fill_ms = 1e9
+    for _ in range(6):
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        f0.record()
+        fill.fill_(1)
+        f1.record()
+        torch.cuda.synchronize()
+        fill_ms = min(fill_ms, f0.elapsed_time(f1))
+    write_gbs = fill.numel() / (fill_ms * 1e-3) / 1e9
+    del fill
     io_kernels = {}
     if kt is not None:
         px = float(H) * W * n_frames * args.steps
@@ -561,6 +575,10 @@ def main(argv=None):
                 io_kernels[name] = {"achieved_GBs": gbs, "frac_of_hbm": gbs / float(peaks["hbm_gbs"]),
                                     "launches": k_n, "avg_launch_ms": k_ms / k_n,
                                     "share_of_step": k_ms / ms_rf}
+                if kind == P.KERNEL_STEM:
+                    io_kernels[name]["frac_of_write_stream_peak"] = gbs / write_gbs
+                    io_kernels[name]["write_stream_peak_GBs"] = write_gbs
+                    io_kernels[name]["write_stream_peak_source"] = "torch fill_ of 1 GiB, best of 6, this run"
     cpu = None
     if not args.no_cpu_baseline:
         # bounded sample: about 2e12 FLOP of oracle work (10-15 s on 16 host cores)
@@ -576,7 +594,7 @@ def main(argv=None):
         "config": {"workload": cfg.name, "frames_per_step": n_frames, "H": H, "W": W, "channels": C,
                    "layers": L, "head_channels": cfg.net.head_channels, "tile": cfg.tile, "tile_merge": tile_merge,
                    "precision": cfg.net.precision,
-                   "distinct_frames": int(len(fs.frames)), "conv_impl": args.conv_impl, "fusion": args.fusion,
+                   "distinct_frames": int(len(fs.frames)), "conv_impl": args.conv_impl, "fusion": args.fusion, "stem": args.stem,
                    "l2": "inputs larger than L2 (u16 stack + activation stream per step > 126 MB)",
                    "parallelism": f"replicas x{world}"},
         "emitters_per_s": world * emitters / (ms_max * 1e-3),

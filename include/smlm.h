@@ -42,7 +42,7 @@
 extern "C" {
 #endif
 
-#define SMLM_ABI_VERSION 3
+#define SMLM_ABI_VERSION 4
 #define SMLM_MAX_LAYERS 32
 
 typedef struct smlm_ctx smlm_ctx; /* opaque; owns device weights, activations, staging slots, events */
@@ -66,6 +66,19 @@ enum { SMLM_FP32 = 0, SMLM_BF16 = 1, SMLM_FP16 = 2 };
  *   ROW   the cores of one tile row share one window (core = tile rows x the whole frame
  *         width): their x halos are computed once instead of twice.  Same emitter list. */
 enum { SMLM_TILE_MERGE_NONE = 0, SMLM_TILE_MERGE_ROW = 1 };
+
+/* K1 (uint16 unpack + normalise + 3x3 stem) kernel choice.
+ *   AUTO          CUDA_CORES.  Both kernels are bound by the same thing - the write stream of a_0
+ *                 (2.5 TB/s in isolation, 2.3 TB/s in the step, against 3.9 TB/s for a plain fill of
+ *                 device memory: profiles/stem_r2.md) - and take the same time.
+ *   TENSOR        the stem on the tcgen05 tensor cores (conv_chain.cu, STEM variant; 16-bit precision,
+ *                 in_frames = 1): fp32 accuracy from three 16-bit pieces of every xhat and every weight,
+ *                 fp32 accumulation, bias through three constant-one input channels, ReLU in the
+ *                 conversion.  Half the issue slots of CUDA_CORES.  Differs from it only in summation
+ *                 order (~1 fp32 ulp before the rounding of a_0 to the storage type).
+ *   CUDA_CORES    stem.cu: one fp32 fmaf chain per channel, taps in (ky, kx) order (the only choice
+ *                 in fp32 precision and with in_frames = 3). */
+enum { SMLM_STEM_AUTO = 0, SMLM_STEM_TENSOR = 1, SMLM_STEM_CUDA_CORES = 2 };
 
 /* Trunk convolution kernel choice for SMLM_BF16 / SMLM_FP16 (fp32 mode always uses the CUDA-core kernel). */
 enum {
@@ -122,6 +135,7 @@ typedef struct {
                             normalised frames f-1, f, f+1 of the call, indices clamped to
                             [0, n_frames-1].  Not available through smlm_localize_ring. */
   int32_t tile_merge;    /* SMLM_TILE_MERGE_* */
+  int32_t stem_impl;     /* SMLM_STEM_* */
 } smlm_net_desc;
 
 /* Camera model.  Scalars are used where a map pointer is NULL.  Maps are [H][W] float32,

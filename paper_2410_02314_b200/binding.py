@@ -19,8 +19,9 @@ FP32, BF16, FP16 = 0, 1, 2
 TILE_MERGE_NONE, TILE_MERGE_ROW = 0, 1
 CONV_AUTO, CONV_TCGEN05, CONV_DIRECT = 0, 1, 2
 OK, ERR_INVALID_ARG, ERR_UNSUPPORTED_DEVICE, ERR_CUDA, ERR_OOM, ERR_OVERFLOW = 0, -1, -2, -3, -4, -5
-ABI_VERSION = 3
+ABI_VERSION = 4
 FUSE_AUTO, FUSE_NONE, FUSE_ALL, FUSE_HEAD, FUSE_PAIRS_1CTA = 0, 1, 2, 3, 4
+STEM_AUTO, STEM_TENSOR, STEM_CUDA_CORES = 0, 1, 2
 KERNEL_STEM, KERNEL_CONV, KERNEL_POST, KERNEL_CONV_PAIR = 0, 1, 2, 3
 
 EXPORTS = ["smlm_create", "smlm_localize", "smlm_check", "smlm_destroy", "smlm_last_error",
@@ -39,7 +40,7 @@ class NetDesc(C.Structure):
                 ("photon_scale", C.c_float), ("bg_scale", C.c_float), ("tile", C.c_int32),
                 ("micro_batch", C.c_int32), ("conv_impl", C.c_int32),
                 ("writeback_frames", C.c_int32), ("fusion", C.c_int32), ("in_frames", C.c_int32),
-                ("tile_merge", C.c_int32)]
+                ("tile_merge", C.c_int32), ("stem_impl", C.c_int32)]
 
 
 class CameraParams(C.Structure):
@@ -110,7 +111,7 @@ def make_desc(channels: int, dilations: Sequence[int], head_channels: int, preci
               z_scale_nm: float = 700.0, photon_scale: float = 1000.0, bg_scale: float = 100.0,
               tile: int = 0, micro_batch: int = 0, conv_impl: int = CONV_AUTO,
               writeback_frames: int = 0, fusion: int = FUSE_AUTO, in_frames: int = 1,
-              tile_merge: int = TILE_MERGE_NONE) -> NetDesc:
+              tile_merge: int = TILE_MERGE_NONE, stem_impl: int = 0) -> NetDesc:
     d = NetDesc()
     d.struct_size = C.sizeof(NetDesc)
     d.version = ABI_VERSION
@@ -128,6 +129,7 @@ def make_desc(channels: int, dilations: Sequence[int], head_channels: int, preci
     d.fusion = int(fusion)
     d.in_frames = int(in_frames)
     d.tile_merge = int(tile_merge)
+    d.stem_impl = int(stem_impl)
     return d
 
 

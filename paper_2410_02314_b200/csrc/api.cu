@@ -62,6 +62,9 @@ struct smlm_ctx {
   bool fuse_stem = false;  // desc.fusion == SMLM_FUSE_ALL: K1 inside the first layer's kernel
   bool fuse_pairs = true;  // AUTO / ALL / PAIRS_1CTA: layers (d, 2d) as one kernel (conv_pair.cu)
   bool pair_cg2 = true;    // ... with tcgen05 cta_group::2 where a row has an even number of segments
+  bool stem_tensor = false;  // K1 on the tensor cores (conv_chain.cu STEM variant)
+  void* w_stem_umma = nullptr;
+  LayerConst stem_lc{};
 
   uint16_t* slots = nullptr;  // kSlots x slot_elems
   size_t slot_elems = 0;
@@ -187,8 +190,12 @@ smlm_status run_trunk(smlm_ctx* c, const uint16_t* dev_frames, int frame_base, c
   smlm_status tr = SMLM_OK;
   if (!fuse_stem || trunk_dump) {  // (the trunk dump wants a_0 itself)
     if ((tr = time_begin(c, SMLM_KERNEL_STEM, st, &te)) != SMLM_OK) return tr;
-    CK(c, launch_stem(c->dt, dev_frames, frame_base, vs, s, np, c->w_stem, c->b_stem,
-                      c->d.stem_relu, c->act[0], st));
+    if (c->stem_tensor)
+      CK(c, launch_stem_umma(c->dt == ACT_F16, dev_frames, frame_base, vs, s, np, c->w_stem_umma, c->stem_lc,
+                             c->d.stem_relu, c->act[0], c->n_sm, st));
+    else
+      CK(c, launch_stem(c->dt, dev_frames, frame_base, vs, s, np, c->w_stem, c->b_stem,
+                        c->d.stem_relu, c->act[0], st));
     c->launches++;
     if ((tr = time_end(c, te, st)) != SMLM_OK) return tr;
     if (trunk_dump) {
@@ -380,6 +387,8 @@ smlm_status smlm_create(const smlm_net_desc* desc, const void* weights, smlm_ctx
     return fail(nullptr, SMLM_ERR_INVALID_ARG, "in_frames must be 1 or 3");
   if (desc->tile_merge != SMLM_TILE_MERGE_NONE && desc->tile_merge != SMLM_TILE_MERGE_ROW)
     return fail(nullptr, SMLM_ERR_INVALID_ARG, "bad tile_merge");
+  if (desc->stem_impl < SMLM_STEM_AUTO || desc->stem_impl > SMLM_STEM_CUDA_CORES)
+    return fail(nullptr, SMLM_ERR_INVALID_ARG, "bad stem_impl");
   if (desc->conv_impl < SMLM_CONV_AUTO || desc->conv_impl > SMLM_CONV_DIRECT)
     return fail(nullptr, SMLM_ERR_INVALID_ARG, "bad conv_impl");
   if (desc->precision == SMLM_FP32 && desc->conv_impl == SMLM_CONV_TCGEN05)
@@ -436,6 +445,19 @@ smlm_status smlm_create(const smlm_net_desc* desc, const void* weights, smlm_ctx
       for (int t = 0; t < 9; ++t)
         for (int co = 0; co < C; ++co) c->stem_args.w[t][co] = tmp[t * C + co];
     for (int co = 0; co < C; ++co) c->stem_args.b[co] = w[T9 * C + co];
+    {
+      const bool can = c->dt != ACT_F32 && c->in_frames == 1 && stem_umma_supports(C, 1);
+      if (desc->stem_impl == SMLM_STEM_TENSOR && !can)
+        return fail(nullptr, SMLM_ERR_INVALID_ARG, "SMLM_STEM_TENSOR needs 16-bit precision, in_frames = 1, channels 16/32/48/64");
+      c->stem_tensor = can && desc->stem_impl == SMLM_STEM_TENSOR;
+      if (c->stem_tensor) {
+        std::vector<uint8_t> sp(stem_umma_packed_bytes(C));
+        stem_umma_pack_host(C, tmp.data(), w + T9 * C, sp.data(), c->dt == ACT_F16);
+        CK(nullptr, cudaMalloc(&c->w_stem_umma, sp.size()));
+        CK(nullptr, cudaMemcpy(c->w_stem_umma, sp.data(), sp.size(), cudaMemcpyHostToDevice));
+        for (int co = 0; co < C; ++co) c->stem_lc.bias[co] = w[T9 * C + co];
+      }
+    }
     if ((st = upload(std::vector<float>(w + T9 * C, w + (T9 + 1) * C), &c->b_stem)) != SMLM_OK) return st;
     w += (T9 + 1) * C;
     c->layers.resize(L);
@@ -497,6 +519,7 @@ smlm_status smlm_create(const smlm_net_desc* desc, const void* weights, smlm_ctx
 void smlm_destroy(smlm_ctx* c) {
   if (!c) return;
   cudaDeviceSynchronize();
+  if (c->w_stem_umma) cudaFree(c->w_stem_umma);
   cudaFree(c->w_stem); cudaFree(c->b_stem); cudaFree(c->w_head); cudaFree(c->b_head);
   for (auto& L : c->layers) { cudaFree(L.w_direct); cudaFree(L.w_umma); cudaFree(L.bias); }
   cudaFree(c->act[0]); cudaFree(c->act[1]); cudaFree(c->logit); cudaFree(c->cand); cudaFree(c->slots);

@@ -15,6 +15,18 @@
 // the skip), so the epilogue never touches the stages.  Two lanes per CTA as in conv_umma.cu:
 // warps 0-3 / 4-7 epilogue of lane 0 / 1 (one TMEM lane quadrant each), 8 / 10 TMA producer,
 // 9 / 11 MMA issuer.  The layer is HBM-bound: 2 C_in + 2 C_out bytes per pixel.
+//
+// STEM variant (K1 of smlm.h on the tensor cores; BASELINE.json north_star (a)): uint16 unpack,
+// ((adu - offset) / gain) / norm_scale and the 3x3 stem convolution 1 -> C in one kernel that is
+// bound by its HBM WRITE (2 B in, 2C B out per pixel) instead of by fp32 FMA issue (stem.cu: 670
+// thread-instructions per pixel).  No map is read: the lane's producer warp computes the
+// operand row itself.  fp32 accuracy on 16-bit tensor cores by splitting: xhat = x_h + x_m + x_l
+// and w = w_h + w_m + w_l into three 16-bit pieces each (24 of fp32's 24 mantissa bits with
+// bf16), and letting six of the K = 16 input channels carry the pairings (x_h w_h), (x_h w_m),
+// (x_m w_h), (x_h w_l), (x_l w_h), (x_m w_m); the dropped ones are below 2^-24 relative.  The
+// products are exact in the fp32 accumulator, so a_0 differs from the fmaf chain of stem.cu
+// only in summation order (~1 fp32 ulp).  One MMA per horizontal tap and row: the tensor work
+// is nothing, the kernel streams.
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 #include <cuda_runtime.h>
@@ -31,6 +43,8 @@ namespace {
 using namespace ptx;
 
 constexpr int kThreads = 384;   // 12 warps
+constexpr int kStemThreads = 576;  // STEM: + 3 more operand-building warps per lane (warps 12-14 / 15-17)
+constexpr int kStemProd = 4;       // producer warps per lane in the STEM variant
 constexpr int kEpiWarps = 4;    // per lane
 constexpr int kTileM = 128;
 constexpr int kMaxStages = 4;
@@ -89,13 +103,53 @@ __host__ __device__ inline CSmem chain_smem(int CI, int CO, int kx_taps, int dx,
   return L;
 }
 
+// STEM: where the operand rows come from (the frames, not a map)
+struct StemSrc {
+  const uint16_t* frames;  // device; frame f of the call at frames + (f - frame_base) Hf Wf
+  int frame_base;
+  ViewSet vs;
+  NormParams np;
+};
+
+// max(v, 0) and the RNE rounding of two values in one conversion (low half = first argument)
+template <bool F16>
+__device__ __forceinline__ uint32_t pack2_relu(float lo, float hi) {
+  uint32_t d;
+  if (F16) asm("cvt.rn.relu.f16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
+  else asm("cvt.rn.relu.bf16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
+  return d;
+}
+
+// 16-bit pieces of v: v ~ h + m + l
+template <bool F16>
+__device__ __forceinline__ void split3(float v, uint32_t& h, uint32_t& m, uint32_t& l) {
+  if (F16) {
+    const __half a = __float2half_rn(v);
+    const float r1 = v - __half2float(a);
+    const __half b = __float2half_rn(r1);
+    const __half c = __float2half_rn(r1 - __half2float(b));
+    h = __half_as_ushort(a);
+    m = __half_as_ushort(b);
+    l = __half_as_ushort(c);
+  } else {
+    const __nv_bfloat16 a = __float2bfloat16_rn(v);
+    const float r1 = v - __bfloat162float(a);
+    const __nv_bfloat16 b = __float2bfloat16_rn(r1);
+    const __nv_bfloat16 c = __float2bfloat16_rn(r1 - __bfloat162float(b));
+    h = __bfloat16_as_ushort(a);
+    m = __bfloat16_as_ushort(b);
+    l = __bfloat16_as_ushort(c);
+  }
+}
+
 // KX = 3: 3x3 convolution.  KX = 1: 1x1 convolution (the transition of a dense block) run through
 // the same walk - one tap, no x halo, the weight rows of ky = 0 and ky = 2 are zero; the layer is
 // HBM-bound by a wide margin, so the idle two thirds of each MMA's N do not show.
-template <int CO, bool F16, int KX>
-__global__ void __launch_bounds__(kThreads, 1)
+template <int CO, bool F16, int KX, bool STEM>
+__global__ void __launch_bounds__(STEM ? kStemThreads : kThreads, 1)
     conv_chain_kernel(const uint8_t* __restrict__ in, uint8_t* __restrict__ out, CGeo geo,
-                      const uint8_t* __restrict__ wpack, int nstage, const __grid_constant__ LayerConst lc, int relu) {
+                      const uint8_t* __restrict__ wpack, int nstage, const __grid_constant__ LayerConst lc, int relu,
+                      const __grid_constant__ StemSrc ss) {
   extern __shared__ uint8_t smem_raw[];
   const int d = geo.d, dx = geo.dx, CI = geo.CI;
   const CSmem L = chain_smem(CI, CO, KX, dx, nstage);
@@ -113,12 +167,34 @@ __global__ void __launch_bounds__(kThreads, 1)
   auto acc_free_bar = [&](int ln) { return lane_bar(ln, 2 * kMaxStages + 1); };
   auto stage_addr = [&](int ln, int s) { return sbase + L.stage_off + (uint32_t)(ln * nstage + s) * L.stage_bytes; };
   volatile uint32_t* tmem_slot = reinterpret_cast<volatile uint32_t*>(smem + L.tmem_off);
+  const uint32_t plane_bytes_s = (uint32_t)(kTileM + 2 * dx) * 16u;  // one channel chunk of a stage
+  // does the step of window row `row` bring in a row?  A map row must lie inside the window; a
+  // STEM row inside the FRAME (smlm.h: xhat = 0 outside the frame - a window's neighbour rows
+  // are real pixels, as in stem.cu)
+  auto row_valid = [&](int wy0, int row) {
+    if (STEM) return row >= -1 && row <= geo.H && wy0 + row >= 0 && wy0 + row < ss.vs.Hf;
+    return row >= 0 && row < geo.H;
+  };
+  if (STEM) {
+    // the second K chunk (channels 8-15) of every stage is constant: channels 8, 9, 10 = 1 (they
+    // carry the three pieces of the bias through the centre tap), the rest 0
+    uint4* zs = reinterpret_cast<uint4*>(smem + L.stage_off);
+    const uint32_t one = F16 ? 0x3C00u : 0x3F80u;
+    const uint32_t per_stage = L.stage_bytes / 16u, per_plane = plane_bytes_s / 16u;
+    const uint32_t nz = 2u * nstage * per_stage;
+    for (uint32_t i = threadIdx.x; i < nz; i += kStemThreads) {
+      const uint32_t in_stage = i % per_stage;
+      const bool chunk1 = in_stage >= per_plane && in_stage < 2u * per_plane;
+      zs[i] = chunk1 ? make_uint4(one | (one << 16), one, 0u, 0u) : make_uint4(0u, 0u, 0u, 0u);
+    }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
 
   if (threadIdx.x == 0) {
     mbar_init(wbar, 1);
     for (int ln = 0; ln < 2; ++ln) {
       for (int s = 0; s < kMaxStages; ++s) {
-        mbar_init(full_bar(ln, s), 1);
+        mbar_init(full_bar(ln, s), STEM ? kStemProd : 1);  // the TMA transaction count, or the operand-building warps
         mbar_init(empty_bar(ln, s), 1);  // the MMA commit only: no residual, the epilogue never reads a stage
       }
       mbar_init(acc_full_bar(ln), 1);
@@ -141,9 +217,10 @@ __global__ void __launch_bounds__(kThreads, 1)
   const int nlanes = 2 * gridDim.x;
   const uint32_t plane = (uint32_t)(kTileM + 2 * dx) * 16u;
 
-  if (role == 0 || role == 2) {
-    // =========================== TMA producers
-    const int ln = role >> 1;
+  if (role == 0 || role == 2 || role >= 4) {
+    // =========================== TMA producers (STEM: the warps that build the operand rows)
+    const int ln = role >= 4 ? (role - 4) / (kStemProd - 1) : role >> 1;
+    const int sp = role >= 4 ? 1 + (role - 4) % (kStemProd - 1) : 0;  // STEM: which quarter of the positions
     if (role == 0 && elect_one()) {
       mbar_expect_tx(wbar, L.w_bytes);
       for (uint32_t off = 0; off < L.w_bytes; off += 16384u) {
@@ -161,6 +238,92 @@ __global__ void __launch_bounds__(kThreads, 1)
     CRun run;
     uint32_t st = 0, empty_par = 1;
     int last_x0 = -1, fills_left = 0;
+    if (STEM) {
+      // The warp builds the operand row of every valid step: 130 positions (x0 - 1 .. x0 + 128),
+      // lane l owns positions l, l + 32, ...  The raw values of the NEXT valid step are loaded
+      // before this step's arithmetic, so the global latency hides behind it.
+      constexpr int NP = 2;  // positions sp * 32 + lane, and (the two halo positions 128, 129) + 128
+      const size_t fpx = (size_t)ss.vs.Hf * ss.vs.Wf;
+      struct Raw {
+        float adu[NP], om[NP], gm[NP];
+        bool in[NP];
+      };
+      auto fetch = [&](int b, int x0, int row, Raw& r) {
+        const View v = view_of(ss.vs, b, geo.H, geo.W);
+        const uint16_t* frame = ss.frames + (size_t)(v.frame - ss.frame_base) * fpx;
+        const int fy = v.wy0 + row;
+#pragma unroll
+        for (int i = 0; i < NP; ++i) {
+          const int p = sp * 32 + lane + 128 * i;
+          const int fx = v.wx0 + x0 - 1 + p;
+          r.in[i] = p < kTileM + 2 && fx >= 0 && fx < ss.vs.Wf;
+          const size_t q = r.in[i] ? (size_t)fy * ss.vs.Wf + fx : 0;
+          r.adu[i] = r.in[i] ? (float)__ldg(frame + q) : 0.0f;
+          r.om[i] = (r.in[i] && ss.np.offset_map) ? __ldg(ss.np.offset_map + q) : ss.np.offset;
+          r.gm[i] = (r.in[i] && ss.np.offset_map) ? __ldg(ss.np.gain_map + q) : ss.np.gain;
+        }
+      };
+      // iterator over the valid steps of this lane, in walk order
+      bool have_run = false;
+      int j = 0, row = 0, wy0 = 0;
+      auto next_step = [&](int& b, int& x0, int& rrow) {
+        for (;;) {
+          if (!have_run) {
+            if (!runs.next(geo, run)) return false;
+            have_run = true;
+            j = 0;
+            row = run.r + (run.i0 - 1) * d;
+            wy0 = view_of(ss.vs, run.b, geo.H, geo.W).wy0;
+          }
+          while (j < run.n + 2) {
+            const int r0 = row;
+            ++j;
+            row += d;
+            if (row_valid(wy0, r0)) {
+              b = run.b;
+              x0 = run.x0;
+              rrow = r0;
+              return true;
+            }
+          }
+          have_run = false;
+        }
+      };
+      int b0, x00, r00;
+      bool have = next_step(b0, x00, r00);
+      Raw cur;
+      if (have) fetch(b0, x00, r00, cur);
+      while (have) {
+        int b1, x01, r01;
+        const bool have_next = next_step(b1, x01, r01);
+        Raw nxt;
+        if (have_next) fetch(b1, x01, r01, nxt);
+        mbar_wait(empty_bar(ln, (int)st), empty_par);
+        uint8_t* dst = smem + (stage_addr(ln, (int)st) - sbase);
+#pragma unroll
+        for (int i = 0; i < NP; ++i) {
+          const int p = sp * 32 + lane + 128 * i;
+          if (p >= kTileM + 2) continue;
+          uint4 o = make_uint4(0u, 0u, 0u, 0u);
+          if (cur.in[i]) {
+            const float xh = ((cur.adu[i] - cur.om[i]) / cur.gm[i]) / ss.np.norm_scale;  // the oracle's operation order (G5)
+            uint32_t h, m, l;
+            split3<F16>(xh, h, m, l);
+            o = make_uint4(h | (h << 16), m | (h << 16), l | (m << 16), 0u);  // (x_h, x_h, x_m, x_h, x_l, x_m, 0, 0)
+          }
+          *reinterpret_cast<uint4*>(dst + (size_t)p * 16u) = o;
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
+        if (lane == 0) mbar_arrive(full_bar(ln, (int)st));
+        if (++st == (uint32_t)nstage) {
+          st = 0;
+          empty_par ^= 1u;
+        }
+        cur = nxt;
+        have = have_next;
+      }
+    } else
     while (runs.next(geo, run)) {
       const int xl = run.x0 - dx, xr = run.x0 + kTileM + dx;
       const int lo = xl > 0 ? xl : 0, hi = xr < geo.W ? xr : geo.W;
@@ -215,8 +378,9 @@ __global__ void __launch_bounds__(kThreads, 1)
     uint32_t st = 0, full_par = 0, free_par = 0, m = 0;
     while (runs.next(geo, run)) {
       int row = run.r + (run.i0 - 1) * d;
+      const int wy0 = STEM ? view_of(ss.vs, run.b, geo.H, geo.W).wy0 : 0;
       for (int j = 0; j < run.n + 2; ++j, row += d) {
-        const bool in_valid = row >= 0 && row < geo.H;
+        const bool in_valid = row_valid(wy0, row);
         if (in_valid) mbar_wait(full_bar(ln, (int)st), full_par);
         mbar_wait(acc_free_bar(ln), free_par);
         free_par ^= 1u;
@@ -298,13 +462,21 @@ __global__ void __launch_bounds__(kThreads, 1)
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
               const int c0 = kk * 8 + 2 * i;
-              float v0 = __uint_as_float(acc[c0]) + lc.bias[c0];
-              float v1 = __uint_as_float(acc[c0 + 1]) + lc.bias[c0 + 1];
-              if (relu) {
-                v0 = fmaxf(v0, 0.0f);
-                v1 = fmaxf(v1, 0.0f);
+              if (STEM) {
+                // the bias came in through the MMA (three constant-one input channels), the ReLU
+                // rides on the conversion: two instructions per channel pair less in the one loop
+                // that sets the pace of this HBM-bound kernel
+                const float v0 = __uint_as_float(acc[c0]), v1 = __uint_as_float(acc[c0 + 1]);
+                ow[i] = relu ? pack2_relu<F16>(v0, v1) : pack2<F16>(v0, v1);
+              } else {
+                float v0 = __uint_as_float(acc[c0]) + lc.bias[c0];
+                float v1 = __uint_as_float(acc[c0 + 1]) + lc.bias[c0 + 1];
+                if (relu) {
+                  v0 = fmaxf(v0, 0.0f);
+                  v1 = fmaxf(v1, 0.0f);
+                }
+                ow[i] = pack2<F16>(v0, v1);
               }
-              ow[i] = pack2<F16>(v0, v1);
             }
             orow[(size_t)kk * plane_px] = make_uint4(ow[0], ow[1], ow[2], ow[3]);
           }
@@ -342,21 +514,21 @@ uint16_t bits16(float f, bool f16) {
   return (uint16_t)(u >> 16);
 }
 
-template <int CO, bool F16, int KX>
+template <int CO, bool F16, int KX, bool STEM>
 cudaError_t launch_t(const ConvGen& a, CGeo geo, const void* wpack, const LayerConst& lc, int nstage, int grid,
-                     size_t smem, cudaStream_t st) {
+                     size_t smem, const StemSrc& ss, cudaStream_t st) {
   static bool attr_done[kMaxDevices] = {};
   int dev = 0;
   cudaGetDevice(&dev);
   if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
   if (!attr_done[dev]) {
-    cudaError_t e = cudaFuncSetAttribute(conv_chain_kernel<CO, F16, KX>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    cudaError_t e = cudaFuncSetAttribute(conv_chain_kernel<CO, F16, KX, STEM>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) return e;
     attr_done[dev] = true;
   }
   cudaLaunchConfig_t cfg{};
   cfg.gridDim = dim3((unsigned)grid);
-  cfg.blockDim = dim3(kThreads);
+  cfg.blockDim = dim3(STEM ? kStemThreads : kThreads);
   cfg.dynamicSmemBytes = smem;
   cfg.stream = st;
   cudaLaunchAttribute attr[1];
@@ -364,8 +536,8 @@ cudaError_t launch_t(const ConvGen& a, CGeo geo, const void* wpack, const LayerC
   attr[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, conv_chain_kernel<CO, F16, KX>, (const uint8_t*)a.in, (uint8_t*)a.out, geo,
-                            (const uint8_t*)wpack, nstage, lc, a.relu);
+  return cudaLaunchKernelEx(&cfg, conv_chain_kernel<CO, F16, KX, STEM>, (const uint8_t*)a.in, (uint8_t*)a.out, geo,
+                            (const uint8_t*)wpack, nstage, lc, a.relu, ss);
 }
 
 }  // namespace
@@ -420,16 +592,108 @@ cudaError_t launch_conv_chain(bool f16, const ConvGen& a, const void* wpack, con
   const size_t smem = chain_smem(a.CI, a.CO, a.k, geo.dx, nstage).total + 1024;
   long long want = (geo.total + 23) / 24;
   const int grid = (int)(want < 1 ? 1 : (want > n_sm ? n_sm : want));
-#define SMLM_CHAIN_CASE(CC, KK)                                                              \
-  if (a.CO == CC && a.k == KK)                                                              \
-    return f16 ? launch_t<CC, true, KK>(a, geo, wpack, lc, nstage, grid, smem, st)          \
-               : launch_t<CC, false, KK>(a, geo, wpack, lc, nstage, grid, smem, st);
+  static const StemSrc ss0{};
+#define SMLM_CHAIN_CASE(CC, KK)                                                                     \
+  if (a.CO == CC && a.k == KK)                                                                     \
+    return f16 ? launch_t<CC, true, KK, false>(a, geo, wpack, lc, nstage, grid, smem, ss0, st)     \
+               : launch_t<CC, false, KK, false>(a, geo, wpack, lc, nstage, grid, smem, ss0, st);
   SMLM_CHAIN_CASE(16, 3)
   SMLM_CHAIN_CASE(32, 3)
   SMLM_CHAIN_CASE(16, 1)
   SMLM_CHAIN_CASE(32, 1)
   SMLM_CHAIN_CASE(48, 1)
 #undef SMLM_CHAIN_CASE
+  return cudaErrorInvalidValue;
+}
+
+// ---------------------------------------------------------------------------- K1 on the tensor cores
+bool stem_umma_supports(int C, int in_frames) {
+  return in_frames == 1 && (C == 16 || C == 32 || C == 48 || C == 64) && pick_chain_stages(16, C, 3, 1) > 0;
+}
+
+size_t stem_umma_packed_bytes(int C) { return conv_chain_packed_bytes(16, C, 3); }
+
+// w_stem [9][C] fp32 (tap ky * 3 + kx, channel) -> the chain kernel's image for C_in = 16: input
+// channel j of chunk 0 carries the weight piece that pairs with the x piece of the same j
+// (x_h w_h, x_h w_m, x_m w_h, x_h w_l, x_l w_h, x_m w_m); everything else zero.
+void stem_umma_pack_host(int C, const float* w_stem, const float* b_stem, void* dst, bool f16) {
+  static const int ky_seq[5] = {1, 0, 2, 1, 0};
+  static const int wpiece[8] = {0, 1, 0, 2, 0, 1, -1, -1};  // h, m, h, l, h, m
+  uint16_t* o = static_cast<uint16_t*>(dst);
+  auto val16 = [&](uint16_t bits) {
+    if (f16) return __half2float(__ushort_as_half(bits));
+    uint32_t u = (uint32_t)bits << 16;
+    float f;
+    std::memcpy(&f, &u, 4);
+    return f;
+  };
+  for (int kx = 0; kx < 3; ++kx)
+    for (int kc = 0; kc < 2; ++kc)
+      for (int n = 0; n < 5 * C; ++n) {
+        const int ky = ky_seq[n / C], co = n % C;
+        // chunk 0: the weight of the tap; chunk 1 (constant-one channels): the bias, at the centre tap only
+        const float w = kc == 0 ? w_stem[(size_t)(ky * 3 + kx) * C + co] : ((ky == 1 && kx == 1) ? b_stem[co] : 0.0f);
+        uint16_t piece[3];
+        piece[0] = bits16(w, f16);
+        const float r1 = w - val16(piece[0]);
+        piece[1] = bits16(r1, f16);
+        piece[2] = bits16(r1 - val16(piece[1]), f16);
+        for (int j = 0; j < 8; ++j) {
+          uint16_t v = 0;
+          if (kc == 0 && wpiece[j] >= 0) v = piece[wpiece[j]];
+          if (kc == 1 && j < 3) v = piece[j];
+          o[(((size_t)(kx * 2 + kc) * 5 * C) + n) * 8 + j] = v;
+        }
+      }
+}
+
+cudaError_t launch_stem_umma(bool f16, const uint16_t* frames, int frame_base, ViewSet vs, ActShape s, NormParams np,
+                             const void* wpack, const LayerConst& lc, int relu, void* act, int n_sm,
+                             cudaStream_t st) {
+  if (!stem_umma_supports(s.C, vs.in_frames <= 1 ? 1 : vs.in_frames)) return cudaErrorInvalidValue;
+  if (s.B <= 0) return cudaSuccess;
+  ConvGen a{};
+  a.in = nullptr;
+  a.out = act;
+  a.CI = 16;
+  a.CO = s.C;
+  a.B = s.B;
+  a.H = s.H;
+  a.W = s.W;
+  a.k = 3;
+  a.d = 1;
+  a.relu = relu;
+  CGeo geo;
+  geo.B = s.B;
+  geo.H = s.H;
+  geo.W = s.W;
+  geo.d = 1;
+  geo.dx = 1;
+  geo.nseg = (s.W + kTileM - 1) / kTileM;
+  geo.Lmax = s.H;
+  geo.total = (long long)s.B * geo.nseg * geo.Lmax;
+  geo.CI = 16;
+  geo.in_planes = 0;
+  geo.out_planes = (s.CT > 0 ? s.CT : s.C) / 8;
+  geo.co_plane0 = 0;
+  StemSrc ss;
+  ss.frames = frames;
+  ss.frame_base = frame_base;
+  ss.vs = vs;
+  ss.np = np;
+  const int nstage = pick_chain_stages(16, s.C, 3, 1);
+  const size_t smem = chain_smem(16, s.C, 3, 1, nstage).total + 1024;
+  long long want = (geo.total + 23) / 24;
+  const int grid = (int)(want < 1 ? 1 : (want > n_sm ? n_sm : want));
+#define SMLM_STEM_CASE(CC)                                                                       \
+  if (s.C == CC)                                                                                 \
+    return f16 ? launch_t<CC, true, 3, true>(a, geo, wpack, lc, nstage, grid, smem, ss, st)      \
+               : launch_t<CC, false, 3, true>(a, geo, wpack, lc, nstage, grid, smem, ss, st);
+  SMLM_STEM_CASE(16)
+  SMLM_STEM_CASE(32)
+  SMLM_STEM_CASE(48)
+  SMLM_STEM_CASE(64)
+#undef SMLM_STEM_CASE
   return cudaErrorInvalidValue;
 }
 

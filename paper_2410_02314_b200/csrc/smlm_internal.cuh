@@ -102,6 +102,15 @@ cudaError_t launch_stem(int dt, const uint16_t* frames, int frame_base, ViewSet 
                         NormParams np, const float* w_stem /*[in_frames * 9][C]*/, const float* b_stem,
                         int relu, void* act, cudaStream_t st);
 
+// K1 on the tensor cores (conv_chain.cu, STEM variant; 16-bit maps, in_frames = 1): the same
+// function as launch_stem with fp32 accuracy from 16-bit operand pieces; HBM-write-bound.
+struct LayerConst;
+bool stem_umma_supports(int C, int in_frames);
+size_t stem_umma_packed_bytes(int C);
+void stem_umma_pack_host(int C, const float* w_stem /*[9][C]*/, const float* b_stem /*[C]*/, void* dst, bool f16);
+cudaError_t launch_stem_umma(bool f16, const uint16_t* frames, int frame_base, ViewSet vs, ActShape s, NormParams np,
+                             const void* wpack, const LayerConst& lc, int relu, void* act, int n_sm, cudaStream_t st);
+
 // K2' reference trunk layer on CUDA cores (fp32 math; storage float, bf16 or fp16).
 // w: [9][C_in][C_out] float (already rounded to the storage type's values in the 16-bit modes).
 cudaError_t launch_conv_direct(int dt, const void* in, void* out, ActShape s, int dil,

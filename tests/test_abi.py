@@ -70,9 +70,10 @@ def test_struct_layout_matches_header():
 #include <stddef.h>
 #include "smlm.h"
 int main(void) {
-  printf("%zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu\n", sizeof(smlm_net_desc), offsetof(smlm_net_desc, dilations),
+  printf("%zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu %zu\n", sizeof(smlm_net_desc), offsetof(smlm_net_desc, dilations),
          offsetof(smlm_net_desc, head_channels), offsetof(smlm_net_desc, writeback_frames),
          offsetof(smlm_net_desc, fusion), offsetof(smlm_net_desc, in_frames), offsetof(smlm_net_desc, tile_merge),
+         offsetof(smlm_net_desc, stem_impl),
          sizeof(smlm_camera_params), offsetof(smlm_camera_params, gain_map), sizeof(smlm_emitter),
          offsetof(smlm_emitter, p));
   return 0;
@@ -86,7 +87,7 @@ int main(void) {
         got = [int(v) for v in subprocess.run([exe], capture_output=True, text=True, check=True).stdout.split()]
     N, Cam = binding.NetDesc, binding.CameraParams
     want = [C.sizeof(N), N.dilations.offset, N.head_channels.offset, N.writeback_frames.offset,
-            N.fusion.offset, N.in_frames.offset, N.tile_merge.offset, C.sizeof(Cam), Cam.gain_map.offset, binding.EMITTER_DTYPE.itemsize,
+            N.fusion.offset, N.in_frames.offset, N.tile_merge.offset, N.stem_impl.offset, C.sizeof(Cam), Cam.gain_map.offset, binding.EMITTER_DTYPE.itemsize,
             binding.EMITTER_DTYPE.fields["p"][1]]
     assert got == want
     assert binding.EMITTER_DTYPE.itemsize == 32

@@ -460,16 +460,53 @@ def test_fused_stem_and_heads_equal_unfused_bit_exact(C, nh, H, W, dil, tile):
     gm = np.clip(rng.normal(2.0, 0.1, size=(H, W)), 0.5, None).astype(np.float32)
     ck = dict(pixel_size_nm=100.0, offset=0.0, gain=1.0, offset_map=offm, gain_map=gm)
     kw = dict(conv_impl=P.CONV_TCGEN05)
+    # SMLM_FUSE_ALL computes a_0 with the fmaf chain of stem.cu inside the first layer's kernel, so its
+    # twin is the CUDA-core stem; the other modes share the default stem (tensor cores where it exists)
+    cc = dict(stem_impl=P.STEM_CUDA_CORES, **kw)
     if not tile:
-        ma, ta = G.gpu_forward_maps(spec, w, frames, ck, dump_trunk=True, fusion=P.FUSE_NONE, **kw)
+        ma, ta = G.gpu_forward_maps(spec, w, frames, ck, dump_trunk=True, fusion=P.FUSE_NONE, **cc)
         mb, tb = G.gpu_forward_maps(spec, w, frames, ck, dump_trunk=True, fusion=P.FUSE_ALL, **kw)
         assert np.array_equal(ta, tb) and np.array_equal(ma, mb)
     for thr in (0.5, 0.0):
-        a = G.gpu_localize(spec, w, frames, ck, thr, fusion=P.FUSE_NONE, tile=tile, **kw)
+        a = G.gpu_localize(spec, w, frames, ck, thr, fusion=P.FUSE_NONE, tile=tile, **cc)
         assert len(a) > 0 or H * W < 100
-        for fusion in (P.FUSE_AUTO, P.FUSE_ALL):
-            b = G.gpu_localize(spec, w, frames, ck, thr, fusion=fusion, tile=tile, **kw)
-            assert len(a) == len(b) and a.tobytes() == b.tobytes(), (thr, fusion)
+        b = G.gpu_localize(spec, w, frames, ck, thr, fusion=P.FUSE_ALL, tile=tile, **kw)
+        assert len(a) == len(b) and a.tobytes() == b.tobytes(), (thr, "all")
+        a = G.gpu_localize(spec, w, frames, ck, thr, fusion=P.FUSE_NONE, tile=tile, **kw)
+        b = G.gpu_localize(spec, w, frames, ck, thr, fusion=P.FUSE_AUTO, tile=tile, **kw)
+        assert len(a) == len(b) and a.tobytes() == b.tobytes(), (thr, "auto")
+
+
+# ------------------------------------------------------------------ K1 on the tensor cores vs the CUDA-core stem
+@pytest.mark.parametrize("C,prec,H,W,tile", [(48, "bf16", 70, 300, 0), (64, "bf16", 40, 129, 0), (16, "fp16", 33, 131, 0),
+                                             (32, "bf16", 1, 1, 0), (48, "bf16", 150, 173, 64)])
+def test_tensor_core_stem_equals_cuda_core_stem_to_rounding(C, prec, H, W, tile):
+    """SMLM_STEM_TENSOR (three 16-bit pieces of every xhat and weight, fp32 accumulation in TMEM)
+    against SMLM_STEM_CUDA_CORES (fp32 fmaf chain): a_0 is the same fp32 sum up to summation
+    order, so after the one rounding to the storage type the two maps agree except for rare
+    1-ulp flips - with per-pixel camera maps, ragged widths, 1x1 frames and tile windows."""
+    spec = NetSpec(C, (1, 2), 5, prec)
+    w = _rand_blob(spec, 900 + C + H, scale=(2.0 / (9 * C)) ** 0.5 * 0.6)
+    w[C * 10 + 2 * (C * C * 9 + C) + 5 * C] = 0.2
+    rng = np.random.default_rng(H * 77 + W)
+    frames = rng.integers(80, 6000, size=(3, H, W)).astype(np.uint16)
+    offm = rng.normal(100, 2, size=(H, W)).astype(np.float32)
+    gm = np.clip(rng.normal(2.0, 0.1, size=(H, W)), 0.5, None).astype(np.float32)
+    ck = dict(pixel_size_nm=100.0, offset=0.0, gain=1.0, offset_map=offm, gain_map=gm)
+    kw = dict(conv_impl=P.CONV_TCGEN05)
+    if not tile:
+        _, ta = G.gpu_forward_maps(spec, w, frames, ck, dump_trunk=True, stem_impl=P.STEM_CUDA_CORES, **kw)
+        _, tb = G.gpu_forward_maps(spec, w, frames, ck, dump_trunk=True, stem_impl=P.STEM_TENSOR, **kw)
+        a0, b0 = ta[:, 0].astype(np.float64), tb[:, 0].astype(np.float64)
+        ulp = 2.0 ** (-7 if prec == "bf16" else -10)         # one ulp of the storage type, relative, at the bottom of a binade
+        rel = np.abs(a0 - b0) / np.maximum(np.abs(a0), 1e-3)
+        assert rel.max() <= 1.01 * ulp, rel.max()                    # at most one ulp of the storage type
+        assert np.mean(a0 != b0) < 0.02, np.mean(a0 != b0)           # and rarely
+    a = G.gpu_localize(spec, w, frames, ck, 0.5, tile=tile, stem_impl=P.STEM_CUDA_CORES, **kw)
+    b = G.gpu_localize(spec, w, frames, ck, 0.5, tile=tile, stem_impl=P.STEM_TENSOR, **kw)
+    ka = {(int(f), int(q)) for f, q in zip(a["frame"], a["pix"])}
+    kb = {(int(f), int(q)) for f, q in zip(b["frame"], b["pix"])}
+    assert len(ka ^ kb) <= max(2, 0.02 * len(ka)), (len(ka), len(kb), len(ka ^ kb))
 
 
 # ------------------------------------------------------------------ layer pairs (conv_pair.cu) vs one kernel per layer
