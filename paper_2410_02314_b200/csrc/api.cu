@@ -174,8 +174,10 @@ smlm_status ensure_act(smlm_ctx* c, size_t bytes) {
 smlm_status run_trunk(smlm_ctx* c, const uint16_t* dev_frames, int frame_base, const ViewSet& vs,
                       ActShape s, const NormParams& np, cudaStream_t st, int* result_buf,
                       float* trunk_dump, size_t dump_view_stride, size_t dump_level_stride,
-                      cudaEvent_t after_stem, bool want_logit, float lthr, bool* have_logit) {
+                      cudaEvent_t after_stem, bool want_logit, float lthr, bool* have_logit,
+                      bool* heads_from_act = nullptr) {
   if (have_logit) *have_logit = false;
+  if (heads_from_act) *heads_from_act = false;
   const size_t nl = c->layers.size();
   // layers l, l+1 run as one kernel (conv_pair.cu) when their dilations are (d, 2d); pairs are
   // formed greedily from the first layer on (the trunk dump wants every level: no pairs then)
@@ -222,6 +224,7 @@ smlm_status run_trunk(smlm_ctx* c, const uint16_t* dev_frames, int frame_base, c
       cudaError_t e = launch_conv_pair(c->dt == ACT_F16, c->act[cur], c->act[cur ^ 1], s, L.dil, L.w_umma, L2.w_umma,
                                        L.lc, L2.lc, head ? &c->head_args : nullptr, c->pair_cg2, c->n_sm, st, err, sizeof err);
       if (head && have_logit) *have_logit = true;
+      if (head && heads_from_act) *heads_from_act = true;  // act[cur ^ 1] holds the last map at the candidates
       if (e != cudaSuccess) return fail(c, SMLM_ERR_CUDA, "conv_pair: %s %s", cudaGetErrorString(e), err);
       ++l;
     } else if (c->use_umma) {
@@ -782,13 +785,16 @@ smlm_status call_frames(Call& k, const uint16_t* frames, int64_t f_first, int64_
     for (size_t si = 0; si < sets.size(); ++si) {
       int res = 0;
       cudaEvent_t after_stem = (slot >= 0 && si + 1 == sets.size()) ? c->ev_consumed[slot] : nullptr;
-      bool have_logit = false;
+      bool have_logit = false, from_act = false;
       r = run_trunk(c, dev_frames, frame_base, sets[si].vs, sets[si].s, k.np, st, &res, nullptr, 0, 0,
-                    after_stem, true, k.hp.lthr, &have_logit);
+                    after_stem, true, k.hp.lthr, &have_logit, &from_act);
       if (r != SMLM_OK) return r;
       cudaEvent_t te = nullptr;
       if ((r = time_begin(c, SMLM_KERNEL_POST, st, &te)) != SMLM_OK) return r;
-      if (have_logit)
+      if (have_logit && from_act)
+        CK(c, launch_post_logits_act(c->dt, c->logit, c->act[res], sets[si].s, sets[si].vs, c->w_head, c->b_head, k.hp,
+                                     k.list, counter, k.capacity, st));
+      else if (have_logit)
         CK(c, launch_post_logits(c->logit, c->cand, sets[si].s, sets[si].vs, k.hp, k.list, counter, k.capacity, st));
       else
         CK(c, launch_head_post(c->dt, c->act[res], sets[si].s, sets[si].vs, c->w_head, c->b_head, k.hp,

@@ -90,7 +90,7 @@ struct PSmem {
   uint32_t wA_off, wB_off, w_bytes;   // per layer
   uint32_t stA_off, stA_bytes;        // input row segments of layer A (TMA)
   uint32_t stB_off, stB_bytes;        // `mid` row segments (written by A's epilogue)
-  uint32_t xch_off;                   // HEAD: float [128 px][8]
+  uint32_t xch_off;                   // HEAD: float [2][128 px][8]
   uint32_t bar_off, tmem_off, total;
 };
 
@@ -108,7 +108,7 @@ __host__ __device__ inline PSmem pair_smem(int C, int d, int nA, int nB, bool he
   L.stA_off = (2u * L.w_bytes + 127u) & ~127u;
   L.stB_off = L.stA_off + (uint32_t)nA * L.stA_bytes;
   L.xch_off = L.stB_off + (uint32_t)nB * L.stB_bytes;
-  L.bar_off = L.xch_off + (head ? kTileM * 8u * 4u : 0u);
+  L.bar_off = L.xch_off + (head ? 2u * kTileM * 8u * 4u : 0u);  // two step parities
   L.tmem_off = L.bar_off + 8u * kNumBars;
   L.total = L.tmem_off + 16u;
   return L;
@@ -140,15 +140,6 @@ __device__ __forceinline__ void wait_bar(uint32_t bar, uint32_t parity) {
     if (t0 == 0) t0 = t;
     else if (t - t0 > 20000000000ll) __trap();
   }
-}
-
-__device__ __forceinline__ unsigned long long pack2f(float lo, float hi) {
-  return ((unsigned long long)__float_as_uint(hi) << 32) | __float_as_uint(lo);
-}
-__device__ __forceinline__ unsigned long long ffma2(unsigned long long a, unsigned long long b, unsigned long long c) {
-  unsigned long long d;
-  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
-  return d;
 }
 
 // cta_group::2: one MMA over the CTA pair (ranks 2k, 2k+1 of the cluster = two adjacent
@@ -645,7 +636,7 @@ __global__ void __launch_bounds__(kThreads, 1)
       PRuns runs;
       runs.init(geo, cid, ncl);
       PRun run;
-      uint32_t slot0 = 2, slot1 = 2, par0 = 0, par1 = 0, bst = 0;
+      uint32_t slot0 = 2, slot1 = 2, par0 = 0, par1 = 0, bst = 0, xpar = 0;
       uint4 res_old[KH], res_mid[KH];
 #pragma unroll
       for (int k = 0; k < KH; ++k) res_old[k] = res_mid[k] = make_uint4(0u, 0u, 0u, 0u);
@@ -673,16 +664,18 @@ __global__ void __launch_bounds__(kThreads, 1)
           tc_fence_before();
           __syncwarp();
           if (lane == 0) arrive_accB_free(s);
-          // HEAD (K3 folded in, as conv_umma.cu): every head is the sum of two fmaf chains, one per
-          // channel half (head_post.cu evaluates the same two chains); heads are updated two at a
-          // time with fma.rn.f32x2 (two independent IEEE fp32 FMAs: the same bits as fmaf).
-          unsigned long long hq[3] = {0ull, 0ull, 0ull};  // (o_0, o_1), (o_2, o_3), (o_4, o_5)
+          // HEAD (last pair of the trunk): the epilogue evaluates the detection logit of every pixel
+          // - the sum of two fmaf chains, one per channel half, the same chains as head_post.cu,
+          // exchanged between the warp pair through shared memory - and stores the activations
+          // only where the logit exceeds the threshold: K3 (post_logits_act_kernel) evaluates the
+          // other heads there, for the survivors of the 3x3 test.  (All six heads in this
+          // epilogue cost 6 x 48 FMAs per pixel and made the HEAD launch 17-29 % slower than a
+          // plain one: profiles/conv_pair_r2.md.)
+          float hp0 = 0.0f;
+          uint32_t owv[HEAD ? KH : 1][4];
           auto post = [&](auto HALF) {
             constexpr int kHalf = decltype(HALF)::value;
-            if (HEAD && kHalf == 0) {
-#pragma unroll
-              for (int j = 0; j < 3; ++j) hq[j] = pack2f(ha.b[2 * j], ha.b[2 * j + 1]);
-            }
+            if (HEAD && kHalf == 0) hp0 = ha.b[0];
 #pragma unroll
             for (int kk = 0; kk < KH; ++kk) {
               constexpr int kc0 = kHalf * KH;
@@ -699,12 +692,9 @@ __global__ void __launch_bounds__(kThreads, 1)
                 if (HEAD) {
                   float a0, a1;
                   unpack2<F16>(ow[i], a0, a1);
-                  const unsigned long long aa0 = pack2f(a0, a0), aa1 = pack2f(a1, a1);
-#pragma unroll
-                  for (int j = 0; j < 3; ++j) hq[j] = ffma2(aa0, pack2f(ha.w[c0][2 * j], ha.w[c0][2 * j + 1]), hq[j]);
-#pragma unroll
-                  for (int j = 0; j < 3; ++j)
-                    hq[j] = ffma2(aa1, pack2f(ha.w[c0 + 1][2 * j], ha.w[c0 + 1][2 * j + 1]), hq[j]);
+                  hp0 = fmaf(a0, ha.w[c0][0], hp0);
+                  hp0 = fmaf(a1, ha.w[c0 + 1][0], hp0);
+                  owv[kk][i] = ow[i];
                 }
               }
               if (!HEAD) orow[(size_t)kk * plane_px] = make_uint4(ow[0], ow[1], ow[2], ow[3]);
@@ -713,32 +703,6 @@ __global__ void __launch_bounds__(kThreads, 1)
           if (store) {
             if (half == 0) post(std::integral_constant<int, 0>{});
             else post(std::integral_constant<int, 1>{});
-          }
-          if (HEAD && out_valid) {
-            float hp[6];
-#pragma unroll
-            for (int j = 0; j < 3; ++j) {
-              hp[2 * j] = __uint_as_float((uint32_t)hq[j]);
-              hp[2 * j + 1] = __uint_as_float((uint32_t)(hq[j] >> 32));
-            }
-            if (half == 1) {
-              *reinterpret_cast<float4*>(xch) = make_float4(hp[0], hp[1], hp[2], hp[3]);
-              *reinterpret_cast<float2*>(xch + 4) = make_float2(hp[4], hp[5]);
-            }
-            asm volatile("bar.sync %0, 64;" ::"r"(pair_bar) : "memory");
-            if (half == 0 && store) {
-              const float4 o03 = *reinterpret_cast<const float4*>(xch);
-              const float2 o45 = *reinterpret_cast<const float2*>(xch + 4);
-              const float lg = hp[0] + o03.x;
-              const size_t q = ((size_t)run.b * geo.H + (row - dB)) * geo.W + x;
-              ha.logit[q] = lg;
-              if (lg > ha.lthr) {
-                float4* cq = reinterpret_cast<float4*>(ha.cand) + q * 2;
-                cq[0] = make_float4(hp[1] + o03.y, hp[2] + o03.z, hp[3] + o03.w, hp[4] + o45.x);
-                cq[1] = make_float4(hp[5] + o45.y, 0.0f, 0.0f, 0.0f);
-              }
-            }
-            asm volatile("bar.sync %0, 64;" ::"r"(pair_bar) : "memory");
           }
           // residual bookkeeping: the output finished by the next step (other chain) has its
           // centre in the previous step's mid row, the one after that in this step's
@@ -759,6 +723,22 @@ __global__ void __launch_bounds__(kThreads, 1)
               if (has_right) mbar_arrive_cluster(eb_right + 8u * bst);
             }
             if (++bst == (uint32_t)nB) bst = 0;
+          }
+          // (the mid stage is released above, BEFORE the exchange: the barrier below must not delay it)
+          if (HEAD && out_valid) {
+            float* xb = xch + (xpar ? kTileM * 8 : 0);  // double-buffered by step: a warp may run one barrier ahead
+            xpar ^= 1u;
+            xb[half] = hp0;
+            asm volatile("bar.sync %0, 64;" ::"r"(pair_bar) : "memory");
+            const float lg = xb[0] + xb[1];  // (half 0's chain) + (half 1's chain), the same bits in both warps
+            if (store) {
+              if (half == 0) ha.logit[((size_t)run.b * geo.H + (row - dB)) * geo.W + x] = lg;
+              if (lg > ha.lthr) {
+#pragma unroll
+                for (int kk = 0; kk < KH; ++kk)
+                  orow[(size_t)kk * plane_px] = make_uint4(owv[kk][0], owv[kk][1], owv[kk][2], owv[kk][3]);
+              }
+            }
           }
           if (s) slot1 = slot1 == 2 ? 0u : slot1 + 1u;
           else slot0 = slot0 == 2 ? 0u : slot0 + 1u;

@@ -162,10 +162,42 @@ __global__ void __launch_bounds__(NT)
 constexpr int LW = 64, LH = 16;  // NT = 256 threads, four pixels each
 constexpr int LCAND = (LW / 2) * (LH / 2);  // no two detections are 8-adjacent
 
-__global__ void __launch_bounds__(NT, 4)
-    post_logits_kernel(const float* __restrict__ logit, const float* __restrict__ cand, ActShape s,
-                       ViewSet vs, HeadParams hp, smlm_emitter* __restrict__ out,
-                       unsigned long long* __restrict__ counter, unsigned long long capacity) {
+// Where a survivor's other heads (pre-activation) come from: the 32-byte candidate records of
+// conv_umma.cu's HEAD epilogue, or (conv_pair.cu) the last activation map, which that kernel
+// stores for above-threshold pixels only - evaluated here with the chains of ActSource.
+struct CandHeads {
+  const float* cand;
+  __device__ inline void get(const ActShape& s, const HeadParams& hp, int b, int y, int x, float& odx, float& ody,
+                             float& oz, float& oN, float& obg) const {
+    const float4* cq = reinterpret_cast<const float4*>(cand) + (((size_t)b * s.H + y) * s.W + x) * 2;
+    const float4 c0 = __ldg(cq), c1 = __ldg(cq + 1);
+    const bool six = hp.n_h == 6;
+    odx = c0.x;
+    ody = c0.y;
+    oz = c0.z;
+    oN = six ? c0.w : c0.z;
+    obg = six ? c1.x : c0.w;
+  }
+};
+template <typename T, int C>
+struct ActHeads {
+  ActSource<T, C> src;
+  __device__ inline void get(const ActShape&, const HeadParams& hp, int b, int y, int x, float& odx, float& ody,
+                             float& oz, float& oN, float& obg) const {
+    const int hN = hp.n_h == 6 ? 4 : 3;
+    odx = src.head(1, b, y, x);
+    ody = src.head(2, b, y, x);
+    oz = hp.n_h == 6 ? src.head(3, b, y, x) : 0.0f;
+    oN = src.head(hN, b, y, x);
+    obg = src.head(hN + 1, b, y, x);
+  }
+};
+
+template <typename Heads>
+__device__ __forceinline__ void post_logits_body(const float* __restrict__ logit, const Heads& heads, ActShape s,
+                                                 ViewSet vs, HeadParams hp, smlm_emitter* __restrict__ out,
+                                                 unsigned long long* __restrict__ counter,
+                                                 unsigned long long capacity) {
   __shared__ float lg[LH + 2][LW + 2];
   __shared__ int cnd[LCAND];
   __shared__ int ncand;
@@ -227,11 +259,10 @@ __global__ void __launch_bounds__(NT, 4)
   const int ly = i / LW, lx = i - ly * LW;
   const int y = y0 + ly, x = x0 + lx;
   const int fy = v.wy0 + y, fx = v.wx0 + x;
-  // candidate record: heads 1 .. n_h-1 (pre-activation) = (dx, dy, [z,] N, bg)
-  const float4* cq = reinterpret_cast<const float4*>(cand) + (((size_t)b * s.H + y) * s.W + x) * 2;
-  const float4 c0 = __ldg(cq), c1 = __ldg(cq + 1);
+  // heads 1 .. n_h-1 (pre-activation) = (dx, dy, [z,] N, bg)
   const bool six = hp.n_h == 6;
-  const float odx = c0.x, ody = c0.y, oz = c0.z, oN = six ? c0.w : c0.z, obg = six ? c1.x : c0.w;
+  float odx, ody, oz, oN, obg;
+  heads.get(s, hp, b, y, x, odx, ody, oz, oN, obg);
   smlm_emitter e;
   e.frame = v.frame;
   e.pix = fy * vs.Wf + fx;
@@ -245,6 +276,27 @@ __global__ void __launch_bounds__(NT, 4)
   const uint4* srcv = reinterpret_cast<const uint4*>(&e);
   dst[0] = srcv[0];
   dst[1] = srcv[1];
+}
+
+__global__ void __launch_bounds__(NT, 4)
+    post_logits_kernel(const float* __restrict__ logit, const float* __restrict__ cand, ActShape s,
+                       ViewSet vs, HeadParams hp, smlm_emitter* __restrict__ out,
+                       unsigned long long* __restrict__ counter, unsigned long long capacity) {
+  post_logits_body(logit, CandHeads{cand}, s, vs, hp, out, counter, capacity);
+}
+
+template <typename T, int C>
+__global__ void __launch_bounds__(NT, 4)
+    post_logits_act_kernel(const float* __restrict__ logit, const T* __restrict__ act, ActShape s, ViewSet vs,
+                           const float* __restrict__ w_head, const float* __restrict__ b_head, HeadParams hp,
+                           smlm_emitter* __restrict__ out, unsigned long long* __restrict__ counter,
+                           unsigned long long capacity) {
+  __shared__ float wh[6 * C];
+  __shared__ float bh[8];
+  for (int i = threadIdx.x; i < hp.n_h * C; i += NT) wh[i] = w_head[i];
+  if (threadIdx.x < hp.n_h) bh[threadIdx.x] = b_head[threadIdx.x];
+  __syncthreads();
+  post_logits_body(logit, ActHeads<T, C>{ActSource<T, C>{act, s, wh, bh}}, s, vs, hp, out, counter, capacity);
 }
 
 __global__ void __launch_bounds__(NT)
@@ -360,6 +412,28 @@ cudaError_t launch_post_logits(const float* logit, const float* cand, ActShape s
   dim3 grid((s.W + LW - 1) / LW, (s.H + LH - 1) / LH, s.B);
   post_logits_kernel<<<grid, NT, 0, st>>>(logit, cand, s, vs, hp, out, counter, capacity);
   return cudaGetLastError();
+}
+
+template <typename T, int C>
+cudaError_t post_logits_act_tc(const float* logit, const void* act, ActShape s, ViewSet vs, const float* w,
+                               const float* b, HeadParams hp, smlm_emitter* out, unsigned long long* counter,
+                               unsigned long long capacity, cudaStream_t st) {
+  dim3 grid((s.W + LW - 1) / LW, (s.H + LH - 1) / LH, s.B);
+  post_logits_act_kernel<T, C><<<grid, NT, 0, st>>>(logit, static_cast<const T*>(act), s, vs, w, b, hp, out, counter,
+                                                    capacity);
+  return cudaGetLastError();
+}
+
+cudaError_t launch_post_logits_act(int dt, const float* logit, const void* act, ActShape s, ViewSet vs,
+                                   const float* w_head, const float* b_head, HeadParams hp, smlm_emitter* out,
+                                   unsigned long long* counter, unsigned long long capacity, cudaStream_t st) {
+  if (s.B <= 0) return cudaSuccess;
+  if (dt == ACT_BF16) {
+    SMLM_DISPATCH_C(__nv_bfloat16, post_logits_act_tc, logit, act, s, vs, w_head, b_head, hp, out, counter, capacity, st)
+  } else if (dt == ACT_F16) {
+    SMLM_DISPATCH_C(__half, post_logits_act_tc, logit, act, s, vs, w_head, b_head, hp, out, counter, capacity, st)
+  }
+  return cudaErrorInvalidValue;
 }
 
 cudaError_t launch_head_maps(int dt, const void* act, ActShape s, const float* w_head,

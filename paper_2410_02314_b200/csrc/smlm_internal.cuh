@@ -159,7 +159,8 @@ cudaError_t launch_conv_umma(bool f16, const void* in, void* out, ActShape s, in
 
 // K2 pair (conv_pair.cu): layers l and l+1 with dilations (d, 2d) in one kernel; the map between
 // them stays in shared memory.  Bit-identical to two launch_conv_umma calls.  head != nullptr:
-// layer l+1 is the last one (HEAD variant, `out` is not written).  allow_cg2: rows with an even
+// layer l+1 is the last one (HEAD variant: head->logit gets the detection logit of every pixel,
+// `out` is written only where it exceeds head->lthr; head->cand is not used).  allow_cg2: rows with an even
 // number of segments use tcgen05 cta_group::2 (one M = 256 MMA per CTA pair).
 bool conv_pair_supports(int C, int dA, int dB, int W);
 cudaError_t launch_conv_pair(bool f16, const void* in, void* out, ActShape s, int dA, const void* wpackA,
@@ -177,6 +178,12 @@ cudaError_t launch_head_post(int dt, const void* act, ActShape s, ViewSet vs,
 cudaError_t launch_post_logits(const float* logit, const float* cand, ActShape s, ViewSet vs,
                                HeadParams hp, smlm_emitter* out, unsigned long long* counter,
                                unsigned long long capacity, cudaStream_t st);
+
+// K3 after the HEAD launch of conv_pair.cu: the detection logit from `logit`, the other heads
+// evaluated here from `act` - the last map, which that launch stored for above-threshold pixels only.
+cudaError_t launch_post_logits_act(int dt, const float* logit, const void* act, ActShape s, ViewSet vs,
+                                   const float* w_head, const float* b_head, HeadParams hp, smlm_emitter* out,
+                                   unsigned long long* counter, unsigned long long capacity, cudaStream_t st);
 
 // debug: heads only -> fp32 maps [B][n_h][H][W] (pre-activation)
 cudaError_t launch_head_maps(int dt, const void* act, ActShape s, const float* w_head,
