@@ -90,9 +90,10 @@ enum {
 /* Kernel fusion on the tcgen05 path ("post-processing is consolidated
  * within GPU memory to minimize data transfer").
  *   AUTO  HEAD + PAIRS:
- *         HEAD   the last trunk layer's epilogue evaluates the heads (K3 folded in): the final
- *                activation map is never stored; K3 reads a 4 B/px logit map and 32-byte records
- *                of the above-threshold pixels;
+ *         HEAD   the last trunk launch's epilogue evaluates the detection head of every pixel (a
+ *                4 B/px logit map) and, for above-threshold pixels only, either the other heads
+ *                (32-byte records) or the activations from which K3 evaluates them for the
+ *                survivors of the 3x3 test; the full final map is never stored;
  *         PAIRS  consecutive trunk layers with dilations (d, 2d) run as one kernel on a
  *                thread-block cluster; the map between them stays in shared memory (C <= 48,
  *                rows of at most 1024 pixels; other layers run one per kernel).  Rows with an
