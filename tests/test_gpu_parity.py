@@ -543,3 +543,31 @@ def test_layer_pairs_equal_unfused_bit_exact(C, nh, n, H, W, dil, tile):
         for fusion in (P.FUSE_AUTO, P.FUSE_PAIRS_1CTA):     # cta_group::2 where the row has an even number of segments / ::1
             b = G.gpu_localize(spec, w, frames, ck, thr, fusion=fusion, tile=tile, **kw)
             assert len(a) == len(b) and a.tobytes() == b.tobytes(), (thr, fusion)
+
+
+def test_layer_pairs_random_shapes_equal_unfused_bit_exact():
+    """Seeded random shapes through the pair kernel (both cta_group variants) against one kernel
+    per layer: widths on both sides of every segment boundary, heights around the dilations,
+    every supported channel count, every (d, 2d) pair, with and without a trailing single layer."""
+    rng = np.random.default_rng(20241002)
+    for case in range(14):
+        C = int(rng.choice([16, 32, 48]))
+        d = int(rng.choice([1, 2, 4, 8]))
+        dil = (d, 2 * d) + ((int(rng.choice([1, 2, 4])),) if rng.random() < 0.4 else ())
+        seg = int(rng.integers(1, 6))
+        W = int(np.clip(128 * seg + rng.integers(-3, 4), 1, 640))
+        H = int(rng.choice([1, 2, d, 2 * d + 1, 3 * d + 2, 40]))
+        n = int(rng.integers(1, 4))
+        spec = NetSpec(C, dil, int(rng.choice([5, 6])), "bf16")
+        w = _rand_blob(spec, 4000 + case, scale=(2.0 / (9 * C)) ** 0.5 * 0.6)
+        w[C * 10 + len(dil) * (C * C * 9 + C) + spec.head_channels * C] = 0.2
+        frames = rng.integers(80, 3000, size=(n, H, W)).astype(np.uint16)
+        ck = dict(pixel_size_nm=100.0, offset=100.0, gain=1.0)
+        kw = dict(conv_impl=P.CONV_TCGEN05)
+        ma = G.gpu_forward_maps(spec, w, frames, ck, fusion=P.FUSE_HEAD, **kw)
+        a = G.gpu_localize(spec, w, frames, ck, 0.5, fusion=P.FUSE_HEAD, **kw)
+        for fusion in (P.FUSE_AUTO, P.FUSE_PAIRS_1CTA):
+            mb = G.gpu_forward_maps(spec, w, frames, ck, fusion=fusion, **kw)
+            assert np.array_equal(ma, mb), (case, C, dil, H, W, fusion)
+            b = G.gpu_localize(spec, w, frames, ck, 0.5, fusion=fusion, **kw)
+            assert len(a) == len(b) and a.tobytes() == b.tobytes(), (case, C, dil, H, W, fusion)
