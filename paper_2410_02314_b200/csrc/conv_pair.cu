@@ -161,12 +161,6 @@ __device__ __forceinline__ void tc_commit2_mc(uint32_t bar, uint16_t mask) {
       "h"(mask)
       : "memory");
 }
-// relay "this CTA's stage is full" to the leader: the relaying warp has no stores of its own in
-// flight, so the cluster-scope release is cheap here
-__device__ __forceinline__ void mbar_arrive_cluster_release(uint32_t cbar) {
-  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cbar) : "memory");
-}
-
 template <int C, bool HEAD, bool F16, bool CG2>
 __global__ void __launch_bounds__(kThreads, 1)
     conv_pair_kernel(const __nv_bfloat16* __restrict__ in, __nv_bfloat16* __restrict__ out, PGeo geo,
