@@ -63,6 +63,8 @@ struct CGeo {
   int CI;                 // input channels (multiple of 16)
   int in_planes;          // planes per view of the input buffer
   int out_planes, co_plane0;
+  float* out_f32;         // != nullptr: planar fp32 maps [B][n_valid][H][W] instead (the head maps of dloc.h)
+  int n_valid;
 };
 
 struct CRun {
@@ -455,7 +457,17 @@ __global__ void __launch_bounds__(STEM ? kStemThreads : kThreads, 1)
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive(acc_free_bar(ln));
-        if (out_valid && x < geo.W) {
+        if (out_valid && x < geo.W && geo.out_f32) {
+          // head maps: pre-activation fp32 values, planar (a warp writes 32 consecutive pixels of one map)
+          float* o = geo.out_f32 + ((size_t)run.b * geo.n_valid * geo.H + (row - d)) * geo.W + x;
+#pragma unroll
+          for (int c = 0; c < CO; ++c)
+            if (c < geo.n_valid) {
+              float v = __uint_as_float(acc[c]) + (STEM ? 0.0f : lc.bias[c]);
+              if (relu) v = fmaxf(v, 0.0f);
+              o[(size_t)c * plane_px] = v;
+            }
+        } else if (out_valid && x < geo.W) {
 #pragma unroll
           for (int kk = 0; kk < CO / 8; ++kk) {
             uint32_t ow[4];
@@ -573,7 +585,7 @@ void conv_chain_pack_host(int CI, int CO, int CO_real, int k, const float* w, vo
 
 cudaError_t launch_conv_chain(bool f16, const ConvGen& a, const void* wpack, const LayerConst& lc, int n_sm,
                               cudaStream_t st) {
-  if (!conv_chain_supports(a.CI, a.CO, a.k, a.d) || a.out_f32 || a.ci_plane0 != 0) return cudaErrorInvalidValue;
+  if (!conv_chain_supports(a.CI, a.CO, a.k, a.d) || a.ci_plane0 != 0) return cudaErrorInvalidValue;
   if (a.B <= 0) return cudaSuccess;
   CGeo geo;
   geo.B = a.B;
@@ -587,6 +599,8 @@ cudaError_t launch_conv_chain(bool f16, const ConvGen& a, const void* wpack, con
   geo.CI = a.CI;
   geo.in_planes = a.in_planes;
   geo.out_planes = a.out_planes;
+  geo.out_f32 = a.out_f32;
+  geo.n_valid = a.n_valid;
   geo.co_plane0 = a.co_plane0;
   const int nstage = pick_chain_stages(a.CI, a.CO, a.k, a.d);
   const size_t smem = chain_smem(a.CI, a.CO, a.k, geo.dx, nstage).total + 1024;
@@ -675,6 +689,8 @@ cudaError_t launch_stem_umma(bool f16, const uint16_t* frames, int frame_base, V
   geo.CI = 16;
   geo.in_planes = 0;
   geo.out_planes = (s.CT > 0 ? s.CT : s.C) / 8;
+  geo.out_f32 = nullptr;
+  geo.n_valid = 0;
   geo.co_plane0 = 0;
   StemSrc ss;
   ss.frames = frames;

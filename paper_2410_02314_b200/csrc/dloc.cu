@@ -245,7 +245,7 @@ smlm_status conv(dloc_ctx* c, const GLayer& L, const void* in, int in_ch, int ci
     DCK(c, cudaEventRecord(e0, st));
   }
   cudaError_t e = cudaSuccess;
-  if (c->use_umma && !L.wchain.empty() && c->use_chain && a.ci_plane0 == 0 && !out_f32) {
+  if (c->use_umma && !L.wchain.empty() && c->use_chain && a.ci_plane0 == 0 && (!out_f32 || L.wchain.size() == 1)) {
     ConvGen p = a;
     p.CO = L.chain_co;
     for (size_t i = 0; i < L.wchain.size() && e == cudaSuccess; ++i) {
