@@ -57,6 +57,10 @@ def short_name(name: str) -> str:
     if m:
         return (f"conv_pair_kernel<{m.group(1)},{'HEAD' if t(m.group(2)) else '-'},{'f16' if t(m.group(3)) else '-'},"
                 f"{'cg2' if t(m.group(4)) else 'cg1'}>")
+    m = re.match(r"conv_chain_kernel<(\d+),\s*(?:\(bool\))?(\w+),\s*(?:\(int\))?(\d+),\s*(?:\(bool\))?(\w+)>", name)
+    if m:
+        return (f"conv_chain_kernel<{m.group(1)},{'f16' if t(m.group(2)) else '-'},{m.group(3)},"
+                f"{'STEM' if t(m.group(4)) else '-'}>")
     m = re.match(r"([\w:]+)(<.*?>)?\(", name)
     if m:
         return m.group(1) + (m.group(2) or "").replace("__nv_bfloat16", "bf16").replace("__half", "f16") \
