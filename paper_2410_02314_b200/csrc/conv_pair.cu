@@ -91,6 +91,7 @@ struct PSmem {
   uint32_t stA_off, stA_bytes;        // input row segments of layer A (TMA)
   uint32_t stB_off, stB_bytes;        // `mid` row segments (written by A's epilogue)
   uint32_t xch_off;                   // HEAD: float [2][128 px][8]
+  uint32_t scr_off;                   // HEAD: uint4 [C/16][256 threads]: the B epilogue's rounded outputs, parked
   uint32_t bar_off, tmem_off, total;
 };
 
@@ -108,7 +109,8 @@ __host__ __device__ inline PSmem pair_smem(int C, int d, int nA, int nB, bool he
   L.stA_off = (2u * L.w_bytes + 127u) & ~127u;
   L.stB_off = L.stA_off + (uint32_t)nA * L.stA_bytes;
   L.xch_off = L.stB_off + (uint32_t)nB * L.stB_bytes;
-  L.bar_off = L.xch_off + (head ? 2u * kTileM * 8u * 4u : 0u);  // two step parities
+  L.scr_off = L.xch_off + (head ? 2u * kTileM * 8u * 4u : 0u);  // two step parities
+  L.bar_off = L.scr_off + (head ? (uint32_t)(C / 16) * 256u * 16u : 0u);
   L.tmem_off = L.bar_off + 8u * kNumBars;
   L.total = L.tmem_off + 16u;
   return L;
@@ -665,8 +667,11 @@ __global__ void __launch_bounds__(kThreads, 1)
           // other heads there, for the survivors of the 3x3 test.  (All six heads in this
           // epilogue cost 6 x 48 FMAs per pixel and made the HEAD launch 17-29 % slower than a
           // plain one: profiles/conv_pair_r2.md.)
+          // The rounded outputs wait for the verdict in shared memory, not in registers: twelve
+          // more live registers made the compiler rematerialise addresses inside this loop and
+          // the HEAD launch 17 % slower than without the store (profiles/conv_pair_r2.md).
           float hp0 = 0.0f;
-          uint32_t owv[HEAD ? KH : 1][4];
+          uint4* scr = reinterpret_cast<uint4*>(smem + L.scr_off) + ((warp - kEpiWarps) * 32 + lane);
           auto post = [&](auto HALF) {
             constexpr int kHalf = decltype(HALF)::value;
             if (HEAD && kHalf == 0) hp0 = ha.b[0];
@@ -688,10 +693,10 @@ __global__ void __launch_bounds__(kThreads, 1)
                   unpack2<F16>(ow[i], a0, a1);
                   hp0 = fmaf(a0, ha.w[c0][0], hp0);
                   hp0 = fmaf(a1, ha.w[c0 + 1][0], hp0);
-                  owv[kk][i] = ow[i];
                 }
               }
               if (!HEAD) orow[(size_t)kk * plane_px] = make_uint4(ow[0], ow[1], ow[2], ow[3]);
+              else scr[kk * 256] = make_uint4(ow[0], ow[1], ow[2], ow[3]);
             }
           };
           if (store) {
@@ -729,8 +734,7 @@ __global__ void __launch_bounds__(kThreads, 1)
               if (half == 0) ha.logit[((size_t)run.b * geo.H + (row - dB)) * geo.W + x] = lg;
               if (lg > ha.lthr) {
 #pragma unroll
-                for (int kk = 0; kk < KH; ++kk)
-                  orow[(size_t)kk * plane_px] = make_uint4(owv[kk][0], owv[kk][1], owv[kk][2], owv[kk][3]);
+                for (int kk = 0; kk < KH; ++kk) orow[(size_t)kk * plane_px] = scr[kk * 256];
               }
             }
           }
