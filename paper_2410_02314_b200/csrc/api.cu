@@ -29,6 +29,8 @@ constexpr int kCounterWords = 2 + kSnapRing;
 
 thread_local std::string g_create_error;
 
+constexpr int kFirstParts = 4;
+
 struct Layer {
   float* w_direct = nullptr;  // [9][C][C] (tap, ci, co)
   void* w_umma = nullptr;     // packed bf16 image for conv_umma
@@ -70,6 +72,7 @@ struct smlm_ctx {
   size_t slot_elems = 0;
   bool slot_used[kSlots] = {false, false, false};
   cudaEvent_t ev_copied[kSlots]{}, ev_consumed[kSlots]{};
+  cudaEvent_t ev_part[kFirstParts]{};  // the first chunk of a call arrives in parts: K1 starts on the first one
   cudaEvent_t ev_start = nullptr, ev_batch = nullptr;
   cudaEvent_t ev_wb[kSnapRing]{};  // flush k records ev_wb[k % kSnapRing] on the write-back stream
   cudaStream_t copy_stream = nullptr, wb_stream = nullptr;
@@ -175,7 +178,7 @@ smlm_status run_trunk(smlm_ctx* c, const uint16_t* dev_frames, int frame_base, c
                       ActShape s, const NormParams& np, cudaStream_t st, int* result_buf,
                       float* trunk_dump, size_t dump_view_stride, size_t dump_level_stride,
                       cudaEvent_t after_stem, bool want_logit, float lthr, bool* have_logit,
-                      bool* heads_from_act = nullptr) {
+                      bool* heads_from_act = nullptr, int stem_parts = 1) {
   if (have_logit) *have_logit = false;
   if (heads_from_act) *heads_from_act = false;
   const size_t nl = c->layers.size();
@@ -191,15 +194,27 @@ smlm_status run_trunk(smlm_ctx* c, const uint16_t* dev_frames, int frame_base, c
   cudaEvent_t te = nullptr;
   smlm_status tr = SMLM_OK;
   if (!fuse_stem || trunk_dump) {  // (the trunk dump wants a_0 itself)
-    if ((tr = time_begin(c, SMLM_KERNEL_STEM, st, &te)) != SMLM_OK) return tr;
-    if (c->stem_tensor)
-      CK(c, launch_stem_umma(c->dt == ACT_F16, dev_frames, frame_base, vs, s, np, c->w_stem_umma, c->stem_lc,
-                             c->d.stem_relu, c->act[0], c->n_sm, st));
-    else
-      CK(c, launch_stem(c->dt, dev_frames, frame_base, vs, s, np, c->w_stem, c->b_stem,
-                        c->d.stem_relu, c->act[0], st));
-    c->launches++;
-    if ((tr = time_end(c, te, st)) != SMLM_OK) return tr;
+    // stem_parts > 1 (first chunk of a call from host memory, whole frames): the frames arrive
+    // in that many H2D copies (ev_part); K1 runs per part and starts as soon as the first one is
+    // there, so only a quarter of the first copy is exposed
+    for (int q = 0; q < stem_parts; ++q) {
+      const int v0 = (int)((long long)s.B * q / stem_parts), v1 = (int)((long long)s.B * (q + 1) / stem_parts);
+      if (v1 <= v0) continue;
+      if (stem_parts > 1) CK(c, cudaStreamWaitEvent(st, c->ev_part[q], 0));
+      ViewSet vq = vs;
+      vq.frame0 = vs.frame0 + v0;
+      ActShape sq = s;
+      sq.B = v1 - v0;
+      void* aq = static_cast<char*>(c->act[0]) + (size_t)v0 * s.C * s.H * s.W * (c->bf16 ? 2 : 4);
+      if ((tr = time_begin(c, SMLM_KERNEL_STEM, st, &te)) != SMLM_OK) return tr;
+      if (c->stem_tensor)
+        CK(c, launch_stem_umma(c->dt == ACT_F16, dev_frames, frame_base, vq, sq, np, c->w_stem_umma, c->stem_lc,
+                               c->d.stem_relu, aq, c->n_sm, st));
+      else
+        CK(c, launch_stem(c->dt, dev_frames, frame_base, vq, sq, np, c->w_stem, c->b_stem, c->d.stem_relu, aq, st));
+      c->launches++;
+      if ((tr = time_end(c, te, st)) != SMLM_OK) return tr;
+    }
     if (trunk_dump) {
       CK(c, launch_dump_act(c->dt, c->act[0], s, trunk_dump, dump_view_stride, st));
       c->launches++;
@@ -500,6 +515,9 @@ smlm_status smlm_create(const smlm_net_desc* desc, const void* weights, smlm_ctx
       CK(nullptr, cudaEventCreateWithFlags(&c->ev_copied[i], cudaEventDisableTiming));
       CK(nullptr, cudaEventCreateWithFlags(&c->ev_consumed[i], cudaEventDisableTiming));
     }
+    for (int i = 0; i < kFirstParts; ++i) {
+      CK(nullptr, cudaEventCreateWithFlags(&c->ev_part[i], cudaEventDisableTiming));
+    }
     CK(nullptr, cudaEventCreateWithFlags(&c->ev_start, cudaEventDisableTiming));
     CK(nullptr, cudaEventCreateWithFlags(&c->ev_batch, cudaEventDisableTiming));
     for (int i = 0; i < kSnapRing; ++i)
@@ -532,6 +550,9 @@ void smlm_destroy(smlm_ctx* c) {
   for (int i = 0; i < kSlots; ++i) {
     if (c->ev_copied[i]) cudaEventDestroy(c->ev_copied[i]);
     if (c->ev_consumed[i]) cudaEventDestroy(c->ev_consumed[i]);
+  }
+  for (int i = 0; i < kFirstParts; ++i) {
+    if (c->ev_part[i]) cudaEventDestroy(c->ev_part[i]);
   }
   if (c->ev_start) cudaEventDestroy(c->ev_start);
   if (c->ev_batch) cudaEventDestroy(c->ev_batch);
@@ -739,7 +760,7 @@ smlm_status call_frames(Call& k, const uint16_t* frames, int64_t f_first, int64_
     const int nf = (int)std::min<int64_t>(F, f_first + n - f0);
     const uint16_t* dev_frames = frames;
     int frame_base = (int)f_first;
-    int slot = -1;
+    int slot = -1, parts = 1;
     if (host_frames) {
       // P1: the preload ring.  Copy chunk k into slot k % kSlots on the copy stream as soon
       // as the stem of chunk k - kSlots has consumed it; compute waits for the copy only.
@@ -753,10 +774,17 @@ smlm_status call_frames(Call& k, const uint16_t* frames, int64_t f_first, int64_
         c0 = std::max<int64_t>(f0 - 1, f_first);
         c1 = std::min<int64_t>(f0 + nf + 1, f_first + n);
       }
-      CK(c, cudaMemcpyAsync(dst, frames + (size_t)(c0 - f_first) * frame_elems, (size_t)(c1 - c0) * frame_elems * 2,
-                            cudaMemcpyHostToDevice, c->copy_stream));
+      // the first chunk of a call has nothing to hide behind: it travels in kFirstParts copies and
+      // K1 starts on the first (run_trunk, stem_parts)
+      parts = (k.chunk == 0 && !k.tiled && c->in_frames == 1 && !c->fuse_stem && nf >= 16 * kFirstParts) ? kFirstParts : 1;
+      for (int q = 0; q < parts; ++q) {
+        const int64_t a = c0 + (c1 - c0) * q / parts, b = c0 + (c1 - c0) * (q + 1) / parts;
+        CK(c, cudaMemcpyAsync(dst + (size_t)(a - c0) * frame_elems, frames + (size_t)(a - f_first) * frame_elems,
+                              (size_t)(b - a) * frame_elems * 2, cudaMemcpyHostToDevice, c->copy_stream));
+        if (parts > 1) CK(c, cudaEventRecord(c->ev_part[q], c->copy_stream));
+      }
       CK(c, cudaEventRecord(c->ev_copied[slot], c->copy_stream));
-      CK(c, cudaStreamWaitEvent(st, c->ev_copied[slot], 0));
+      if (parts == 1) CK(c, cudaStreamWaitEvent(st, c->ev_copied[slot], 0));
       c->slot_used[slot] = true;
       dev_frames = dst;
       frame_base = (int)c0;
@@ -787,7 +815,7 @@ smlm_status call_frames(Call& k, const uint16_t* frames, int64_t f_first, int64_
       cudaEvent_t after_stem = (slot >= 0 && si + 1 == sets.size()) ? c->ev_consumed[slot] : nullptr;
       bool have_logit = false, from_act = false;
       r = run_trunk(c, dev_frames, frame_base, sets[si].vs, sets[si].s, k.np, st, &res, nullptr, 0, 0,
-                    after_stem, true, k.hp.lthr, &have_logit, &from_act);
+                    after_stem, true, k.hp.lthr, &have_logit, &from_act, parts);
       if (r != SMLM_OK) return r;
       cudaEvent_t te = nullptr;
       if ((r = time_begin(c, SMLM_KERNEL_POST, st, &te)) != SMLM_OK) return r;
