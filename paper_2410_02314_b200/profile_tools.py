@@ -11,6 +11,11 @@ hot path; bench.py only READS profiles/traffic_r2.json).
 
     # per-kernel totals of an `ncu --metrics gpu__time_duration.sum --csv` launch list, markdown
     python -m paper_2410_02314_b200.profile_tools launches launches.csv
+
+    # device timeline of ONE end-to-end step (pinned frames in, pinned list out) from CUPTI via
+    # torch.profiler: every H2D copy and kernel with start / end, and how much of the copy time
+    # runs under a kernel (needs a GPU; markdown)
+    python -m paper_2410_02314_b200.profile_tools timeline --config 1 > profiles/timeline_r2.md
 """
 from __future__ import annotations
 
@@ -198,6 +203,74 @@ def cmd_launches(args):
     return 0
 
 
+def cmd_timeline(args):
+    """One smlm_localize call with the frames in pinned host memory and the list in pinned host
+    memory, traced by CUPTI (torch.profiler).  Not a timing run: the profiler adds overhead."""
+    import numpy as np
+    import torch
+    from torch.profiler import ProfilerActivity, profile
+    root = os.path.dirname(HERE)
+    if root not in sys.path:
+        sys.path.insert(0, root)
+    import paper_2410_02314_b200 as P
+    from smlm_synth import get_config, make_frames, make_weights
+    cfg = get_config(args.config)
+    n = args.frames or cfg.frames.n_frames
+    fs = make_frames(cfg, min(64, n))
+    frames = np.ascontiguousarray(np.concatenate([fs.frames] * (-(-n // len(fs.frames))))[:n])
+    loc = P.Localizer(P.desc_from_spec(cfg.net, tile=cfg.tile, writeback_frames=cfg.writeback_batch), make_weights(cfg))
+    H, W = frames.shape[1:]
+    cap = int(min(n * ((H + 1) // 2) * ((W + 1) // 2), n * max(4 * cfg.frames.emitters_per_frame, 1024)))
+    om = torch.from_numpy(fs.offset_map).cuda() if fs.offset_map is not None else None
+    gm = torch.from_numpy(fs.gain_map).cuda() if fs.gain_map is not None else None
+    cam = loc.camera(fs.pixel_size_nm, fs.offset, fs.gain, om, gm)
+    fh = torch.from_numpy(frames).pin_memory()
+    oh = torch.zeros(cap * 32, dtype=torch.uint8).pin_memory()
+    st = torch.cuda.Stream()
+    for _ in range(3):
+        loc.localize(fh, cam, cfg.threshold, oh, cap, stream=st)
+    torch.cuda.synchronize()
+    with profile(activities=[ProfilerActivity.CUDA]) as prof:
+        loc.localize(fh, cam, cfg.threshold, oh, cap, stream=st)
+        torch.cuda.synchronize()
+    ev = sorted((e.time_range.start, e.time_range.end, short_name(e.name) if "smlm" in e.name else e.name)
+                for e in prof.events() if e.device_type == torch.autograd.DeviceType.CUDA)
+    t0 = ev[0][0]
+    ev = [(a - t0, b - t0, nm) for a, b, nm in ev]
+    copies = [(a, b) for a, b, nm in ev if nm.startswith("Memcpy HtoD")]
+    kernels = sorted((a, b) for a, b, nm in ev if not nm.startswith("Mem"))
+    merged = []                      # union of the kernel intervals
+    for a, b in kernels:
+        if merged and a <= merged[-1][1]:
+            merged[-1][1] = max(merged[-1][1], b)
+        else:
+            merged.append([a, b])
+    def under(a, b):
+        return sum(max(0.0, min(b, y) - max(a, x)) for x, y in merged)
+    copy_us = sum(b - a for a, b in copies)
+    hidden = sum(under(a, b) for a, b in copies)
+    end = max(b for _, b, _ in ev)
+    busy = sum(y - x for x, y in merged)
+    print(f"# Device timeline of one end-to-end step (cfg {args.config}, {n} frames), round 2\n")
+    print(f"Command: `python -m paper_2410_02314_b200.profile_tools timeline --config {args.config}"
+          + (f" --frames {args.frames}" if args.frames else "") + "` (CUPTI activity records through `torch.profiler`; one "
+          "`smlm_localize` call with the frames in pinned host memory and the emitter list in pinned host memory, after "
+          "three warm-up calls).  The profiler adds overhead: this is a picture of the overlap, not a timing.\n")
+    print(f"* step on the device: {end / 1e3:.2f} ms; kernels busy {busy / 1e3:.2f} ms ({100 * busy / end:.1f} %)")
+    print(f"* H2D copies: {len(copies)}, {copy_us / 1e3:.2f} ms in total, {100 * hidden / max(copy_us, 1e-9):.1f} % of it under a "
+          f"running kernel; first kernel starts at {kernels[0][0]:.0f} us")
+    print(f"* consecutive trunk launches overlap by programmatic dependent launch: the next kernel's start precedes "
+          f"the previous kernel's end\n")
+    print("| start us | end us | activity |")
+    print("|---|---|---|")
+    for a, b, nm in ev[:args.rows]:
+        print(f"| {a:.1f} | {b:.1f} | `{nm[:90]}` |")
+    if len(ev) > args.rows:
+        print(f"| ... | ... | {len(ev) - args.rows} more activities |")
+    loc.close()
+    return 0
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
     sub = ap.add_subparsers(dest="cmd", required=True)
@@ -217,6 +290,11 @@ def main(argv=None):
     l = sub.add_parser("launches")
     l.add_argument("csv")
     l.set_defaults(fn=cmd_launches)
+    tl = sub.add_parser("timeline")
+    tl.add_argument("--config", type=int, default=1)
+    tl.add_argument("--frames", type=int, default=0)
+    tl.add_argument("--rows", type=int, default=48)
+    tl.set_defaults(fn=cmd_timeline)
     args = ap.parse_args(argv)
     return args.fn(args)
 
