@@ -193,3 +193,41 @@ def test_dloc_pipeline_host_ring_micro_batches_three_frames_and_edges():
         with pytest.raises(P.SmlmError) as ei:
             P.DlocLocalizer(P.dloc_desc_from_spec(spec, **kw), w)
         assert ei.value.status == P.ERR_INVALID_ARG
+
+
+def test_dloc_full_size_in_bench_launch_shape_sampled_against_oracle():
+    """The shape bench.py --net dloc times: the default DilatedLoc spec in bf16 on 256 x 256 frames,
+    default launch sets (64 frames: one full set + a tail), pinned host frames in, pinned host
+    list out.  The stack cycles 2 distinct frames, so (1) frames 0 and 65 - one in each launch
+    set - are compared element by element with the oracle (head maps through the activations,
+    2e-2), (2) every frame's map and emitter records must equal, bit by bit, those of the first
+    occurrence of the same distinct frame (position in a launch set must not matter: the chain
+    kernel's lane ranges start and end mid-chain), (3) frame 0's emitters go through the gate."""
+    spec = DlocSpec(precision="bf16")
+    w = dloc_he_normal_blob(spec, 3, head_gain=0.5)
+    base = _frames(2, 256, 256, 31)
+    n = 66
+    frames = np.ascontiguousarray(np.concatenate([base] * (n // 2)))
+    ck = dict(pixel_size_nm=100.0, offset=100.0, gain=1.0)
+    cam = O.make_camera(**ck)
+    o = D.forward_maps(D.net_from_spec(spec), w, base, cam)
+    og = _gpu_maps(spec, w, frames, ck)
+    for f in range(2, n):
+        assert np.array_equal(og[f], og[f % 2]), f
+    gs = _spec_for_gate(spec)
+    for f in (0, 65):
+        err = G.head_errors(gs, o[f % 2:f % 2 + 1, :6], og[f:f + 1, :6])
+        assert err.max() < 2e-2, (f, err)
+    thr = 0.5
+    em, found, status, _ = _gpu_localize(spec, w, frames, ck, thr, host_frames=True, host_out=True)
+    assert status == P.OK and found == len(em) and found > 100
+    key = lambda e: (int(e["pix"]), float(e["x_nm"]), float(e["y_nm"]), float(e["p"]), float(e["sx_nm"]))
+    per = {}
+    for e in em:
+        per.setdefault(int(e["frame"]), []).append(key(e))
+    for f in range(2, n):
+        assert sorted(per.get(f, [])) == sorted(per.get(f % 2, [])), f
+    em_o = D.postprocess(spec, o[:1], cam, thr)
+    em0 = em[em["frame"] == 0]
+    st = G.parity_gate(gs, o[:1, :6], em_o, em0, thr, 2e-2, 100.0, 256, 256, dp_measured=G.p_error(o[:1], og[:1]), o_gpu=og[:1])
+    G.record("dloc_full_size_256", gate=st, frames=n, emitters=int(found))
