@@ -356,7 +356,9 @@ def selftest_spawn(args, cfg):
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=40)
+    ap.add_argument("--steps", type=int, default=0,
+                    help="timed steps; default: 40 for cfg 0 / 1 (1.3 s, averages over the dips of the power governor), "
+                         "5 / 3 / 4 for cfg 2 / 3 / 4, 5 for --net dloc")
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1)
@@ -385,6 +387,8 @@ def main(argv=None):
                     help="CPU only: exercise the --gpus N spawn path, the frame sharding and the max-over-ranks "
                          "reduction over gloo with synthetic per-rank timings")
     args = ap.parse_args(argv)
+    if args.steps <= 0:
+        args.steps = 5 if args.net == "dloc" else {2: 5, 3: 3, 4: 4}.get(args.config, 40)
     cfg = get_config(args.config)
     if args.tile >= 0 or args.precision:
         import dataclasses
