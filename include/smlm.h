@@ -264,6 +264,72 @@ smlm_status smlm_debug_postprocess(smlm_ctx* ctx, const float* maps, int64_t n_f
                                    int32_t W, const smlm_camera_params* camera, float threshold,
                                    smlm_emitter* out_emitters, int64_t* out_count, void* cuda_stream);
 
+/*
+ * smlm_postprocess_static: post-processing for callers that cannot allocate GPU memory.
+ *
+ * Who this is for.  All calls above work on an smlm_ctx, and a ctx allocates: smlm_create calls
+ * cudaMalloc, and smlm_localize / smlm_debug_postprocess call it again when a frame size or a
+ * capacity grows.  Some programs cannot have that happen under them:
+ *   - a live acquisition loop, where cudaMalloc / cudaFree would stall the whole device (both wait
+ *     for running work) while the camera's next frames are being copied in;
+ *   - a plug-in or custom operator inside a host application that reserved the GPU's memory for
+ *     its own pool and only hands out buffers - a cudaMalloc from inside it can simply fail;
+ *   - a process that must do all its allocation at start-up.
+ * This one call needs no ctx and calls no cudaMalloc, cudaFree, cudaMallocHost or any library
+ * routine that allocates.  The caller passes the maps and the output list; the bookkeeping of the
+ * compaction lives in a fixed array of SMLM_POST_STATIC_SCRATCH_BYTES (1 MiB) that is part of the
+ * library's device code: every GPU on which the library is used holds that 1 MiB from the moment
+ * its code is loaded there until the process exits.
+ *
+ * What it computes: the same rule as smlm_debug_postprocess (threshold on sigmoid(o_p), 3x3 local
+ * maximum with the lower-index tie rule, decode of the other heads; formulas at the top of this
+ * file) on caller-supplied pre-activation maps.  Same records, but in a FIXED order: by frame,
+ * then by 32 x 64 pixel tile (tile rows top to bottom, tiles left to right), then row-major
+ * inside the tile.  Two calls on the same input give byte-identical lists.
+ *
+ *   maps         DEVICE float32 [n_frames][head_channels][H][W], pre-activation head outputs o.
+ *   params       HOST struct, read during the call.
+ *   threshold    as in smlm_localize.
+ *   out_emitters DEVICE (or pinned host) array of `capacity` records, 16-byte aligned; may be NULL
+ *                when capacity == 0 (count only).  Of more than `capacity` detections the first
+ *                `capacity` in the order above are stored.
+ *   out_count    DEVICE (or pinned host) int64 the GPU can write: number of detections found (may
+ *                exceed capacity).  Valid once the stream has finished.  Unlike smlm_localize this
+ *                is not a pageable host pointer: forwarding to one would need a host allocation.
+ *   cuda_stream  a cudaStream_t (NULL = legacy default stream); the call only enqueues three kernels.
+ *
+ * Size limit: ceil(H/32) * ceil(W/64) * n_frames <= SMLM_POST_STATIC_MAX_TILES (262 080 tiles:
+ * 8 190 frames of 256 x 256, 2 047 of 512 x 512, 127 of 2048 x 2048).  A larger call is refused
+ * with SMLM_ERR_INVALID_ARG and a message that names the limit; split it by frames.
+ *
+ * First call on a device: looks up the device address of the scratch array (cudaGetSymbolAddress,
+ * with that device current - the current device of the calling thread is the one used) and keeps
+ * it for later calls.  That lookup may make the CUDA runtime load the library's device code on
+ * that GPU, so make the first call on each device during start-up, before any stream capture
+ * begins.  The lookup and all argument checks are thread-safe.
+ *
+ * Sharing: all calls on one device use the same array.  Nothing needs clearing between calls
+ * (each call overwrites every word before it reads it), but calls whose kernels can run at the
+ * same time on one GPU - different streams, or several host threads - race on it and produce
+ * wrong lists.  Keep calls on one device in one stream, or order them with events.
+ *
+ * Errors (synchronous): INVALID_ARG (NULL, sizes, the limit above, head_channels not 5 / 6),
+ * UNSUPPORTED_DEVICE (current device is not sm_100), CUDA.  smlm_postprocess_static_error returns
+ * the message of the last failed call on the calling thread (valid until that thread's next call).
+ */
+#define SMLM_POST_STATIC_SCRATCH_BYTES 1048576
+#define SMLM_POST_STATIC_MAX_TILES 262080 /* (SCRATCH_BYTES - 256) / 4 */
+typedef struct {
+  int32_t head_channels; /* 5: p,dx,dy,N,bg    6: p,dx,dy,z,N,bg */
+  float xy_scale, z_scale_nm, photon_scale, bg_scale; /* as in smlm_net_desc */
+  float pixel_size_nm;                                /* as in smlm_camera_params */
+} smlm_post_params;
+smlm_status smlm_postprocess_static(const float* maps, int64_t n_frames, int32_t H, int32_t W,
+                                    const smlm_post_params* params, float threshold,
+                                    smlm_emitter* out_emitters, int64_t capacity, int64_t* out_count,
+                                    void* cuda_stream);
+const char* smlm_postprocess_static_error(void);
+
 #ifdef __cplusplus
 }
 #endif

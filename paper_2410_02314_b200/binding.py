@@ -28,8 +28,10 @@ EXPORTS = ["smlm_create", "smlm_localize", "smlm_check", "smlm_destroy", "smlm_l
            "smlm_launch_count", "smlm_kernel_timing", "smlm_kernel_time_ms",
            "smlm_debug_forward_maps", "smlm_debug_postprocess",
            "smlm_ring_open", "smlm_localize_ring", "smlm_ring_acquire", "smlm_ring_release",
-           "smlm_ring_close"]
+           "smlm_ring_close", "smlm_postprocess_static", "smlm_postprocess_static_error"]
 RING_PAGEABLE = 1
+POST_STATIC_SCRATCH_BYTES = 1048576
+POST_STATIC_MAX_TILES = 262080
 
 
 class NetDesc(C.Structure):
@@ -41,6 +43,11 @@ class NetDesc(C.Structure):
                 ("micro_batch", C.c_int32), ("conv_impl", C.c_int32),
                 ("writeback_frames", C.c_int32), ("fusion", C.c_int32), ("in_frames", C.c_int32),
                 ("tile_merge", C.c_int32), ("stem_impl", C.c_int32)]
+
+
+class PostParams(C.Structure):
+    _fields_ = [("head_channels", C.c_int32), ("xy_scale", C.c_float), ("z_scale_nm", C.c_float),
+                ("photon_scale", C.c_float), ("bg_scale", C.c_float), ("pixel_size_nm", C.c_float)]
 
 
 class CameraParams(C.Structure):
@@ -102,6 +109,10 @@ def lib():
         L.smlm_ring_release.argtypes = [vp, i64]
         L.smlm_ring_close.restype = None
         L.smlm_ring_close.argtypes = [vp]
+        L.smlm_postprocess_static.restype = C.c_int
+        L.smlm_postprocess_static.argtypes = [vp, i64, i32, i32, C.POINTER(PostParams), f32, vp, i64, vp, vp]
+        L.smlm_postprocess_static_error.restype = C.c_char_p
+        L.smlm_postprocess_static_error.argtypes = []
         _LIB = L
     return _LIB
 
@@ -318,6 +329,29 @@ class Ring:
             self.close()
         except Exception:
             pass
+
+
+def postprocess_static(maps, head_channels: int, threshold: float, out_emitters, capacity: int, out_count,
+                       xy_scale: float = 0.5, z_scale_nm: float = 700.0, photon_scale: float = 1000.0,
+                       bg_scale: float = 100.0, pixel_size_nm: float = 100.0, stream=None,
+                       shape: Optional[Sequence[int]] = None) -> None:
+    """smlm_postprocess_static: post-processing without a ctx and without any GPU allocation
+    (for callers that cannot call cudaMalloc: see include/smlm.h).  maps: cuda float32
+    [n][head_channels][H][W] (or a raw address plus `shape` = (n, H, W)); out_emitters: cuda
+    buffer of capacity * 32 bytes; out_count: cuda int64 tensor of one element, written by the
+    GPU.  Enqueues only; raises SmlmError with the library's message on a refused call."""
+    if shape is None:
+        n, nh, H, W = (int(v) for v in maps.shape)
+        if nh != head_channels:
+            raise ValueError("maps.shape[1] != head_channels")
+    else:
+        n, H, W = (int(v) for v in shape)
+    pp = PostParams(int(head_channels), float(xy_scale), float(z_scale_nm), float(photon_scale),
+                    float(bg_scale), float(pixel_size_nm))
+    st = lib().smlm_postprocess_static(_ptr(maps), n, H, W, C.byref(pp), float(threshold), _ptr(out_emitters),
+                                       int(capacity), _ptr(out_count), _stream_handle(stream))
+    if st != OK:
+        raise SmlmError(st, (lib().smlm_postprocess_static_error() or b"").decode())
 
 
 def emitters_to_numpy(buf, count: int) -> np.ndarray:
