@@ -213,7 +213,13 @@ smlm_status smlm_check(smlm_ctx* ctx);
  *   smlm_ring_acquire / smlm_ring_release: the consumer side by hand (tests, custom loops):
  *     acquire blocks until the next chunk is in memory (*n_frames = 0 at the end of the file),
  *     release(first_frame) lets the readers refill its slot.
- *   smlm_ring_close: stops the readers, frees the ring.  NULL is allowed.
+ *   smlm_ring_rewind: start over at the first chunk (what smlm_localize_ring does on entry), also
+ *     after a pass that was abandoned part-way.  Blocks until every chunk handed out so far has
+ *     been released - release what you acquired first - and until reads in flight have ended.
+ *     Not to be called concurrently with acquire / release / smlm_localize_ring on the same ring.
+ *   smlm_ring_close: stops the readers, frees the ring.  NULL is allowed.  GPU work of an earlier
+ *     smlm_localize_ring on this ring must have finished (synchronise its stream first): that
+ *     work hands slots back to the ring from stream callbacks.
  */
 typedef struct smlm_ring smlm_ring;
 enum { SMLM_RING_PAGEABLE = 1 };
@@ -226,6 +232,7 @@ smlm_status smlm_localize_ring(smlm_ctx* ctx, smlm_ring* ring, const smlm_camera
 smlm_status smlm_ring_acquire(smlm_ring* ring, const uint16_t** frames, int64_t* n_frames,
                               int64_t* first_frame);
 smlm_status smlm_ring_release(smlm_ring* ring, int64_t first_frame);
+smlm_status smlm_ring_rewind(smlm_ring* ring);
 void smlm_ring_close(smlm_ring* ring);
 
 /* Synchronise, free everything the ctx owns.  NULL is allowed. */

@@ -28,7 +28,7 @@ EXPORTS = ["smlm_create", "smlm_localize", "smlm_check", "smlm_destroy", "smlm_l
            "smlm_launch_count", "smlm_kernel_timing", "smlm_kernel_time_ms",
            "smlm_debug_forward_maps", "smlm_debug_postprocess",
            "smlm_ring_open", "smlm_localize_ring", "smlm_ring_acquire", "smlm_ring_release",
-           "smlm_ring_close", "smlm_postprocess_static", "smlm_postprocess_static_error"]
+           "smlm_ring_close", "smlm_ring_rewind", "smlm_postprocess_static", "smlm_postprocess_static_error"]
 RING_PAGEABLE = 1
 POST_STATIC_SCRATCH_BYTES = 1048576
 POST_STATIC_MAX_TILES = 262080
@@ -107,6 +107,8 @@ def lib():
         L.smlm_ring_acquire.argtypes = [vp, C.POINTER(vp), C.POINTER(i64), C.POINTER(i64)]
         L.smlm_ring_release.restype = C.c_int
         L.smlm_ring_release.argtypes = [vp, i64]
+        L.smlm_ring_rewind.restype = C.c_int
+        L.smlm_ring_rewind.argtypes = [vp]
         L.smlm_ring_close.restype = None
         L.smlm_ring_close.argtypes = [vp]
         L.smlm_postprocess_static.restype = C.c_int
@@ -312,6 +314,12 @@ class Ring:
         st = lib().smlm_ring_release(self._h, int(first_frame))
         if st != OK:
             raise SmlmError(st, "smlm_ring_release")
+
+    def rewind(self):
+        """Start over at the first chunk (every acquired chunk must have been released)."""
+        st = lib().smlm_ring_rewind(self._h)
+        if st != OK:
+            raise SmlmError(st, "smlm_ring_rewind")
 
     def close(self):
         if self._h:

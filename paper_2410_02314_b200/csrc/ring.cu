@@ -21,14 +21,13 @@ void reader_main(smlm_ring* r) {
     int64_t k, g;
     {
       std::unique_lock<std::mutex> lk(r->mu);
+      // parked while the file is exhausted, and for the WHOLE of a rewind: an assignment taken
+      // between the rewind's generation bump and its reset of next_chunk / free_from would carry
+      // the new generation with an old chunk index and be read twice
+      r->cv.wait(lk, [&] { return r->stop || (!r->rewinding && r->next_chunk.load() < r->n_chunks); });
       if (r->stop) return;
       k = r->next_chunk.load();
       g = r->gen;
-      if (k >= r->n_chunks) {
-        // wait for a rewind or for the end
-        r->cv.wait(lk, [&] { return r->stop || r->gen != g || r->next_chunk.load() < r->n_chunks; });
-        continue;
-      }
       r->next_chunk.store(k + 1);
       const int s = (int)(k % r->n_slots);
       r->cv.wait(lk, [&] { return r->stop || r->gen != g || r->free_from[s] == k; });
@@ -97,12 +96,14 @@ void ring_release_chunk(smlm_ring* r, int64_t k) {
 // pass's copies still read the slots, and a late release of old chunk k would otherwise free
 // the slot that holds new chunk k - the host then waits for that chunk forever), void the
 // readers' pending assignments (generation bump) and wait for reads in flight, so that no
-// stale reader writes into a slot of the new pass.
+// stale reader writes into a slot of the new pass.  The mutex is released inside those waits:
+// `rewinding` keeps the readers parked until next_chunk / free_from / loaded are reset.
 void ring_rewind(smlm_ring* r) {
   {
     std::unique_lock<std::mutex> lk(r->mu);
     if (!r->touched) return;
     r->cv.wait(lk, [&] { return r->stop || r->outstanding == 0; });
+    r->rewinding = true;  // readers take no assignment until the reset below is complete
     ++r->gen;
     r->cv.notify_all();
     r->cv.wait(lk, [&] { return r->stop || r->active_reads == 0; });
@@ -113,6 +114,7 @@ void ring_rewind(smlm_ring* r) {
     r->next_chunk.store(0);
     r->next_acquire = 0;
     r->touched = false;
+    r->rewinding = false;
   }
   r->cv.notify_all();
 }
@@ -207,6 +209,13 @@ smlm_status smlm_ring_acquire(smlm_ring* r, const uint16_t** frames, int64_t* n_
     ++r->by_hand;
   }
   return SMLM_OK;
+}
+
+smlm_status smlm_ring_rewind(smlm_ring* r) {
+  if (!r) return SMLM_ERR_INVALID_ARG;
+  smlm::ring_rewind(r);
+  std::lock_guard<std::mutex> lk(r->mu);
+  return r->stop ? SMLM_ERR_INVALID_ARG : SMLM_OK;  // a read error stopped the ring
 }
 
 smlm_status smlm_ring_release(smlm_ring* r, int64_t first_frame) {

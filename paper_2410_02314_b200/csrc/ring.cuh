@@ -31,6 +31,7 @@ struct smlm_ring {
   int64_t next_acquire = 0;
   int64_t gen = 0;       // bumped by a rewind: readers drop the chunk they were assigned before it
   int active_reads = 0;  // readers inside pread
+  bool rewinding = false;  // a rewind is between its generation bump and its reset: readers stay parked
   bool touched = false;  // a chunk has been handed out since the last rewind
   int64_t outstanding = 0;  // chunks handed out and not yet released (a rewind waits for them)
   int64_t by_hand = 0;      // ... of which through smlm_ring_acquire

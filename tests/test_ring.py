@@ -117,3 +117,33 @@ def test_localize_ring_back_to_back_calls_without_sync(tmp_path):
         for b, c in zip(bufs, cnts):
             em = P.emitters_to_numpy(b, c.value)
             assert len(em) == len(ref) and em.tobytes() == ref.tobytes()
+
+
+def test_rewind_of_a_partly_consumed_ring_delivers_every_chunk_once(tmp_path):
+    """A pass abandoned part-way (chunks taken and released by hand, then a rewind): the readers
+    hold assignments for later chunks and wait for slots.  None of those claims may survive the
+    rewind - a survivor would read its chunk a second time into a slot of the new pass (wrong
+    frames, or a consumer that waits forever).  8 chunks, 2 slots, 3 readers, many repeats."""
+    rng = np.random.default_rng(5)
+    n, chunk, H, W = 8 * 3, 3, 5, 7
+    frames = rng.integers(0, 65536, size=(n, H, W)).astype(np.uint16)
+    path = _write(str(tmp_path), frames)
+    with P.Ring(path, n, H, W, chunk, n_slots=2, n_threads=3, pageable=True) as ring:
+        for it in range(400):
+            for _ in range((2, 0, 5, 1, 8, 3)[it % 6]):          # abandon the pass after this many chunks
+                arr, first = ring.acquire()
+                if arr is None:
+                    break
+                ring.release(first)
+            ring.rewind()
+            seen = 0
+            while True:
+                arr, first = ring.acquire()
+                if arr is None:
+                    break
+                assert first == seen, (it, first, seen)
+                assert np.array_equal(arr, frames[first:first + arr.shape[0]]), (it, first)
+                seen += arr.shape[0]
+                ring.release(first)
+            assert seen == n
+            ring.rewind()
