@@ -29,6 +29,9 @@ from smlm_synth import get_config, make_frames, make_weights  # noqa: E402
 METRIC = "frames_per_s_256x256"
 UNIT = "frames/s"
 DISTINCT_FRAMES = 128       # generated once, cycled to the config's frame count (throughput is data-independent)
+# /opt/skills/guides/B200_PROFILING.md, "Peaks and the roofline denominators": "FALLBACK, only if that file
+# is absent ...: 6.65 TB/s and 1.59 PFLOP/s ... (1.59 is the burst figure; sustained it settles near 1.4 PFLOP/s)".
+# A line computed from these says peak_source "fallback".
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
 
 
@@ -202,6 +205,21 @@ def dloc_flop_per_px(spec):
     return f
 
 
+def dloc_bytes_per_px(spec, elt=2):
+    """Algorithmic HBM bytes of the timed convolution launches per full-resolution pixel: every
+    launch reads its input channels and writes its output channels once (a
+    dense-block layer re-reads the whole concatenation so far), 16-bit storage; enc1 / dec1 at 1/4 of
+    the pixels, enc2 at 1/16; the heads write fp32 planes.  Stem, pool and upsample kernels are not
+    among the timed launches."""
+    b = 0.0
+    for name, co, ci, k in spec.layers():
+        if name == "stem":
+            continue
+        scale = {"enc1": 0.25, "dec1": 0.25, "enc2": 1.0 / 16}.get(name, 1.0)
+        b += (ci * elt + co * (4 if name == "head" else elt)) * scale
+    return b
+
+
 def run_dloc(args, cfg):
     """The paper's own topology through dloc_localize: same step, timing and JSON contract as
     the headline path (one step = one call over the whole stack; value device-resident, e2e
@@ -268,12 +286,30 @@ def run_dloc(args, cfg):
     achieved = conv_flop / (conv_ms * 1e-3) / 1e12 if conv_ms > 0 else None
     roofline = None
     if achieved is not None:
-        roofline = {"bound": "tensor" if spec.precision != "fp32" and args.conv_impl != "direct" else "alu",
-                    "kernel": "conv_gen_umma_kernel (every convolution of the net except stem and heads)",
-                    "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                    "frac_of_burst": achieved / float(peaks["bf16_tflops"]), "traffic": None,
-                    "traffic_source": "no ncu --set full capture of this path",
-                    "peak_source": f"{peak_kind} bf16_tflops_sustained (kernels timed inside a long step)",
+        # which kernels ran the timed launches (dloc.cu: conv_impl AUTO = the row-chain kernel for every
+        # convolution but dec1, whose 288 input channels go through the generic implicit GEMM)
+        kernels = {"auto": "conv_chain_kernel (dense-block layers, 1x1 transitions, enc1, enc2, dec0, heads) + "
+                           "conv_gen_umma_kernel (dec1)",
+                   "tcgen05": "conv_gen_umma_kernel (every convolution but the stem)",
+                   "direct": "conv_gen_direct_kernel (every convolution but the stem; CUDA cores)"}[args.conv_impl]
+        tensor = {"achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                  "frac_of_burst": achieved / float(peaks["bf16_tflops"]),
+                  "peak_source": f"{peak_kind} bf16_tflops_sustained (kernels timed inside a long step)"}
+        gbs = dloc_bytes_per_px(spec, 4 if spec.precision == "fp32" else 2) * H * W * n_frames * args.steps \
+            / (conv_ms * 1e-3) / 1e9
+        hbm = {"achieved": gbs, "peak": float(peaks["hbm_gbs"]), "unit": "GB/s", "frac": gbs / float(peaks["hbm_gbs"]),
+               "peak_source": f"{peak_kind} hbm_gbs (copy bandwidth)",
+               "bytes_per_px": dloc_bytes_per_px(spec, 4 if spec.precision == "fp32" else 2)}
+        # the binding roof is the one the launches sit closer to: the dense-block launches move
+        # 1 024 B/px per block and run at 88-100 % of the copy bandwidth
+        if args.conv_impl == "direct" or spec.precision == "fp32":
+            lead, bound = hbm if hbm["frac"] > 0.5 else tensor, "hbm" if hbm["frac"] > 0.5 else "alu"
+        else:
+            lead, bound = (hbm, "hbm") if hbm["frac"] >= tensor["frac"] else (tensor, "tensor")
+        roofline = {"bound": bound, "kernel": kernels, **{k: lead[k] for k in ("achieved", "peak", "unit", "frac", "peak_source")},
+                    "traffic": None, "traffic_source": "no ncu --set full capture of the whole launch set "
+                                                       "(profiles/ holds one of the dense-block chain kernel)",
+                    "against_tensor_peak": tensor, "against_hbm_peak": hbm,
                     "launches": conv_n, "avg_launch_ms": conv_ms / max(conv_n, 1), "share_of_step": conv_ms / ms_rf}
     cpu = None
     if not args.no_cpu_baseline:
@@ -289,7 +325,7 @@ def run_dloc(args, cfg):
                "sample": f"first {ns} frame(s), {dt:.1f} s (oracle/dloc_oracle.c)", "emitters_per_s": len(em) / dt}
     line = {"metric": METRIC, "value": n_frames * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": 1,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": {"bf16": "bf16"}.get(spec.precision, "f32"),
+            "scaling": "weak", "vs_baseline": None, "dtype": {"bf16": "bf16", "fp16": "f16"}.get(spec.precision, "f32"),
             "data": "synthetic",
             "config": {"workload": f"dloc_c{spec.c0}g{spec.growth}_b{spec.n_blocks}_on_{cfg.name}", "frames_per_step": n_frames,
                        "H": H, "W": W, "c0": spec.c0, "growth": spec.growth, "n_blocks": spec.n_blocks,
@@ -510,11 +546,14 @@ def main(argv=None):
             barrier()
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record(stream)
+            disk_counts = []      # kept until the barrier: the library writes them asynchronously
             for _ in range(args.steps):
-                loc.localize_ring(ring, cam, cfg.threshold, out_host, cap, stream=stream)
+                disk_counts.append(loc.localize_ring(ring, cam, cfg.threshold, out_host, cap, stream=stream))
             e1.record(stream)
             barrier()
             ms_disk = e0.elapsed_time(e1)
+            if loc.check() != P.OK or any(int(c.value) != int(disk_counts[0].value) for c in disk_counts):
+                raise SystemExit(f"--disk: smlm_check {loc.check()} / counts differ between passes")
         os.remove(path)
         disk = {"value": n_frames * args.steps / (ms_disk * 1e-3), "unit": UNIT, "ms_per_step": ms_disk / args.steps,
                 "file_bytes": int(frames.nbytes), "chunk_frames": chunk, "ring_slots": slots, "reader_threads": threads,

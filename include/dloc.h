@@ -91,8 +91,14 @@ typedef struct {
 smlm_status dloc_create(const dloc_net_desc* desc, const void* weights, dloc_ctx** out_ctx);
 
 /* The whole path for n frames of H x W (H, W >= 4): stem, DCD blocks, U-Net, heads, detection,
- * decode, compaction.  *out_count in: capacity, out: emitters found (after stream sync).
- * Asynchronous on `cuda_stream`.  Order of the list unspecified. */
+ * decode, compaction.  *out_count in: capacity, out: emitters found; written from a host callback
+ * ordered on the stream, so the int64 must stay allocated until the stream has finished the call.
+ * Order of the list unspecified.
+ * Asynchronous on `cuda_stream` when out_emitters is DEVICE memory.  With a PINNED HOST list the
+ * call waits (cudaStreamSynchronize) for its own kernels before it returns: the list is compacted
+ * on the device and copied out in one piece once the count is known, a copy that is not
+ * overlapped with compute (smlm_localize's chunked write-back is not implemented for this net);
+ * when the capacity grows it also reallocates the device list behind a device-wide sync. */
 smlm_status dloc_localize(dloc_ctx* ctx, const uint16_t* frames_u16, int64_t n_frames, int32_t H, int32_t W,
                           const smlm_camera_params* camera_params, float threshold, dloc_emitter* out_emitters,
                           int64_t* out_count, void* cuda_stream);

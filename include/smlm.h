@@ -179,7 +179,9 @@ smlm_status smlm_create(const smlm_net_desc* desc, const void* weights, smlm_ctx
  *                records is unspecified (atomic compaction); compare as a set.
  *   out_count    HOST pointer.  In: capacity of out_emitters in records.  Out: number of
  *                emitters found (may exceed the capacity; only the first `capacity` in arrival
- *                order are stored).  Written asynchronously: valid after the stream finished.
+ *                order are stored).  Written asynchronously, from a host callback ordered on the
+ *                stream: the int64 must stay allocated until the stream has finished the call (do
+ *                not pass the address of a temporary), and it is valid from then on.
  *   cuda_stream  a cudaStream_t (NULL = legacy default stream).  The call only enqueues work;
  *                it is ordered after earlier work on that stream; results are valid once the
  *                stream has been synchronised.

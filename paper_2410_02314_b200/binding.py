@@ -183,6 +183,10 @@ class Localizer:
     def __init__(self, desc: NetDesc, weights: np.ndarray):
         self._h = C.c_void_p()
         self.desc = desc
+        # out_count words of calls that may still be in flight: the library writes them from a
+        # stream-ordered host callback after the call returned, so they must outlive a caller
+        # that drops the returned object.  Released by check() / close(), which follow a sync.
+        self._counts_in_flight = []
         w = np.ascontiguousarray(weights, dtype="<f4")
         Cc, L, nh = desc.channels, desc.n_layers, desc.head_channels
         IF = 3 if desc.in_frames == 3 else 1
@@ -219,6 +223,7 @@ class Localizer:
         if count is None:
             count = C.c_int64()
         count.value = int(capacity)
+        self._counts_in_flight.append(count)
         st = lib().smlm_localize(self._h, _ptr(frames), n, H, W, C.byref(cam), float(threshold),
                                  _ptr(out_emitters), C.byref(count), _stream_handle(stream))
         self._check(st)
@@ -230,13 +235,17 @@ class Localizer:
         if count is None:
             count = C.c_int64()
         count.value = int(capacity)
+        self._counts_in_flight.append(count)
         st = lib().smlm_localize_ring(self._h, ring._h, C.byref(cam), float(threshold),
                                       _ptr(out_emitters), C.byref(count), _stream_handle(stream))
         self._check(st)
         return count
 
     def check(self) -> int:
-        return lib().smlm_check(self._h)
+        """smlm_check; call it after the stream of the last localize has been synchronised."""
+        st = lib().smlm_check(self._h)
+        self._counts_in_flight.clear()
+        return st
 
     def launch_count(self) -> int:
         return int(lib().smlm_launch_count(self._h))
@@ -261,6 +270,7 @@ class Localizer:
                     stream=None) -> C.c_int64:
         n, nh, H, W = (int(v) for v in maps.shape)
         count = C.c_int64(int(capacity))
+        self._counts_in_flight.append(count)
         st = lib().smlm_debug_postprocess(self._h, _ptr(maps), n, H, W, C.byref(cam),
                                           float(threshold), _ptr(out_emitters), C.byref(count),
                                           _stream_handle(stream))
@@ -269,8 +279,9 @@ class Localizer:
 
     def close(self):
         if self._h:
-            lib().smlm_destroy(self._h)
+            lib().smlm_destroy(self._h)          # synchronises: no callback is pending afterwards
             self._h = C.c_void_p()
+            self._counts_in_flight.clear()
 
     def __del__(self):
         try:

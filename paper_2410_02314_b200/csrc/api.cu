@@ -948,7 +948,11 @@ smlm_status smlm_debug_forward_maps(smlm_ctx* c, const uint16_t* frames, int64_t
   uint16_t* tmp = nullptr;
   if (fk == PTR_HOST_PINNED && n > 0) {
     CK(c, cudaMalloc(&tmp, (size_t)n * px * 2));
-    CK(c, cudaMemcpyAsync(tmp, frames, (size_t)n * px * 2, cudaMemcpyHostToDevice, st));
+    cudaError_t e = cudaMemcpyAsync(tmp, frames, (size_t)n * px * 2, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) {
+      cudaFree(tmp);
+      return fail(c, SMLM_ERR_CUDA, "cudaMemcpyAsync(frames): %s", cudaGetErrorString(e));
+    }
     frames = tmp;
   }
   for (int64_t f0 = 0; f0 < n; f0 += mb) {

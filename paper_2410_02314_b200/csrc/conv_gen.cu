@@ -254,8 +254,9 @@ __global__ void __launch_bounds__(128)
     conv_gen_direct_kernel(const ConvGen a, const float* __restrict__ w /*[k*k][CI][CO]*/,
                            const float* __restrict__ bias) {
   extern __shared__ float ws[];  // [CI][16]
-  const int x = blockIdx.x * 128 + threadIdx.x;
-  const int y = blockIdx.y % a.H, b = blockIdx.y / a.H;
+  // grid.x runs over (view, row): B * H may exceed the 65535 limit of grid.y / grid.z
+  const int x = blockIdx.y * 128 + threadIdx.x;
+  const int y = blockIdx.x % a.H, b = blockIdx.x / a.H;
   const int co0 = blockIdx.z * 16;
   const int r = a.k / 2;
   float acc[16];
@@ -527,7 +528,7 @@ cudaError_t launch_conv_gen_umma(bool f16, const ConvGen& a, const void* wpack, 
 
 cudaError_t launch_conv_gen_direct(int dt, const ConvGen& a, const float* w, const float* bias, cudaStream_t st) {
   if (a.B <= 0) return cudaSuccess;
-  dim3 grid((a.W + 127) / 128, a.B * a.H, a.CO / 16);
+  dim3 grid(a.B * a.H, (a.W + 127) / 128, a.CO / 16);
   const size_t smem = (size_t)a.CI * 16 * sizeof(float);
   if (dt == ACT_BF16) conv_gen_direct_kernel<__nv_bfloat16><<<grid, 128, smem, st>>>(a, w, bias);
   else if (dt == ACT_F16) conv_gen_direct_kernel<__half><<<grid, 128, smem, st>>>(a, w, bias);

@@ -26,6 +26,7 @@
 //
 // Warps: 0-7 epilogue of A, 8-15 epilogue of B (warp pair (q, q+4) = TMEM lane quadrant q,
 // channel halves), 16 TMA producer, 17 MMA issuer of A, 18 MMA issuer of B (+ TMEM allocation).
+#include <algorithm>
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 #include <cuda_runtime.h>
@@ -870,7 +871,13 @@ cudaError_t launch_conv_pair(bool f16, const void* in, void* out, ActShape s, in
   int nA = 0, nB = 0;
   const bool cg2 = pair_uses_cg2(geo.nseg, allow_cg2);
   pick_pair_stages(s.C, dA, head != nullptr, cg2, &nA, &nB);
-  const size_t smem = pair_smem(s.C, dA, nA, nB, head != nullptr, cg2).total + 1024;
+  // One CTA per SM, whatever C: every CTA allocates all 512 TMEM columns with a blocking
+  // tcgen05.alloc, so two co-resident CTAs of different clusters, each waiting for cluster peers
+  // queued behind the other's allocation, would deadlock.  __launch_bounds__(608, 1) does not
+  // forbid a second CTA; the small-C instantiations need little shared memory and few registers.
+  // Asking for more than half of an SM's 228 KB does (and makes the cluster-occupancy figure
+  // cached per cluster size in launch_pair_t independent of d and of the stage counts).
+  const size_t smem = std::max<size_t>(pair_smem(s.C, dA, nA, nB, head != nullptr, cg2).total + 1024, 116 * 1024);
 #define SMLM_PAIR_CASE(CC)                                                                                          \
   case CC:                                                                                                          \
     return cg2 ? launch_pair_c<CC, true>(f16, in, out, geo, wpackA, wpackB, lcA, lcB, nA, nB, smem, head, n_sm, st)  \

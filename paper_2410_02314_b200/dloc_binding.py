@@ -97,6 +97,7 @@ class DlocLocalizer:
         self._h = C.c_void_p()
         self.desc = desc
         w = np.ascontiguousarray(weights, dtype="<f4")
+        self._counts_in_flight = []
         st = dlib().dloc_create(C.byref(desc), w.ctypes.data, C.byref(self._h))
         if st != B.OK:
             raise B.SmlmError(st, (dlib().dloc_last_error(None) or b"").decode())
@@ -122,6 +123,7 @@ class DlocLocalizer:
         if count is None:
             count = C.c_int64()
         count.value = int(capacity)
+        self._counts_in_flight.append(count)     # written by a stream callback after the call returned
         st = dlib().dloc_localize(self._h, B._ptr(frames), n, H, W, C.byref(cam), float(threshold),
                                   B._ptr(out_emitters), C.byref(count), B._stream_handle(stream))
         self._check(st)
@@ -133,7 +135,10 @@ class DlocLocalizer:
                                                    B._ptr(dump), B._stream_handle(stream)))
 
     def check(self) -> int:
-        return dlib().dloc_check(self._h)
+        """dloc_check; call it after the stream of the last localize has been synchronised."""
+        st = dlib().dloc_check(self._h)
+        self._counts_in_flight.clear()
+        return st
 
     def launch_count(self) -> int:
         return int(dlib().dloc_launch_count(self._h))
@@ -150,6 +155,7 @@ class DlocLocalizer:
         if self._h:
             dlib().dloc_destroy(self._h)
             self._h = C.c_void_p()
+            self._counts_in_flight.clear()
 
     def __del__(self):
         try:

@@ -518,7 +518,9 @@ def test_tensor_core_stem_equals_cuda_core_stem_to_rounding(C, prec, H, W, tile)
     (48, 5, 2, 3, 17, (4, 8), 0),                    # H < d
     (48, 5, 1, 40, 1025, (1, 2), 0),                 # 9 segments: not a pair, must fall back
     (48, 5, 2, 300, 300, (4, 8, 1, 2, 4), 96),       # tiles (windows of 96 + halo), a single layer after the pairs
-    (32, 5, 70, 24, 200, (1, 2, 4, 8), 0)])          # more views than clusters x rows: several runs per cluster
+    (32, 5, 70, 24, 200, (1, 2, 4, 8), 0),           # more views than clusters x rows: several runs per cluster
+    (16, 5, 48, 40, 300, (1, 2, 4, 8), 0),           # a full wave of 3-CTA clusters at C = 16 (one CTA per SM: TMEM)
+    (32, 6, 40, 48, 512, (2, 4), 0)])                # a full wave of 4-CTA clusters (cta_group::2) at C = 32
 def test_layer_pairs_equal_unfused_bit_exact(C, nh, n, H, W, dil, tile):
     """SMLM_FUSE_AUTO runs layers with dilations (d, 2d) as one kernel on a thread-block cluster
     (the map between them stays in shared memory, x halos exchanged through distributed shared
