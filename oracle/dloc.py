@@ -66,8 +66,32 @@ def lib():
         L.dloc_oracle_sigmas.restype = C.c_int
         L.dloc_oracle_sigmas.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_int64,
                                          C.c_double, C.c_double, C.c_double, C.c_double, C.c_void_p]
+        L.dloc_oracle_maxpool2.restype = C.c_int
+        L.dloc_oracle_maxpool2.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p]
+        L.dloc_oracle_upsample2.restype = C.c_int
+        L.dloc_oracle_upsample2.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_void_p]
         _LIB = L
     return _LIB
+
+
+def maxpool2(x: np.ndarray) -> np.ndarray:
+    """The oracle's 2 x 2 / stride 2 / floor max pooling (reading D4) of a planar [c][H][W] map."""
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    c, H, W = x.shape
+    out = np.empty((c, H // 2, W // 2), np.float64)
+    if lib().dloc_oracle_maxpool2(x.ctypes.data, c, H, W, out.ctypes.data) != 0:
+        raise ValueError("dloc_oracle_maxpool2: bad argument")
+    return out
+
+
+def upsample2(x: np.ndarray, Ho: int, Wo: int) -> np.ndarray:
+    """The oracle's nearest-neighbour x 2 up-sampling to exactly Ho x Wo (reading D5)."""
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    c, H, W = x.shape
+    out = np.empty((c, int(Ho), int(Wo)), np.float64)
+    if lib().dloc_oracle_upsample2(x.ctypes.data, c, H, W, int(Ho), int(Wo), out.ctypes.data) != 0:
+        raise ValueError("dloc_oracle_upsample2: bad argument")
+    return out
 
 
 def make_net(c0: int, growth: int, n_blocks: int = 4, dilations: Sequence[int] = (2, 4, 8, 16),

@@ -125,6 +125,19 @@ static void upsample2(const double *in, int c, int H, int W, int Ho, int Wo, dou
       }
 }
 
+/* Test hooks: the two resampling rules on their own, so that tests/test_dloc_oracle_pins.py can
+ * pin them to a library routine and to hand-written cases (they add no arithmetic). */
+int dloc_oracle_maxpool2(const double *in, int c, int H, int W, double *out) {
+  if (!in || !out || c < 1 || H < 2 || W < 2) return -1;
+  maxpool2(in, c, H, W, out);
+  return 0;
+}
+int dloc_oracle_upsample2(const double *in, int c, int H, int W, int Ho, int Wo, double *out) {
+  if (!in || !out || c < 1 || H < 1 || W < 1 || Ho < 1 || Wo < 1) return -1;
+  upsample2(in, c, H, W, Ho, Wo, out);
+  return 0;
+}
+
 /*
  * Forward pass for n frames of H x W uint16 (H, W >= 4).  out_maps [n][10][H][W]: the
  * PRE-activation head outputs.  dump (may be NULL) receives, per frame, the feature maps in

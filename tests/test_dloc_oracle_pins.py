@@ -59,8 +59,11 @@ def _torch_forward(spec, blob, frames, offset=100.0, gain=1.0):
     e0 = f
     e1 = F.relu(F.conv2d(F.max_pool2d(e0, 2), *P["enc1"], padding=1))
     e2 = F.relu(F.conv2d(F.max_pool2d(e1, 2), *P["enc2"], padding=1))
-    up = lambda t, size: t[:, :, torch.clamp(torch.arange(size[0]) // 2, max=t.shape[2] - 1)][
-        :, :, :, torch.clamp(torch.arange(size[1]) // 2, max=t.shape[3] - 1)]
+    def up(t, size):
+        # library routines only: nearest x 2, then the finer map's odd last row / column (if any)
+        # by replicating the edge (reading D5)
+        u = F.interpolate(t, scale_factor=2, mode="nearest")
+        return F.pad(u, (0, size[1] - u.shape[3], 0, size[0] - u.shape[2]), mode="replicate")
     m1 = F.relu(F.conv2d(torch.cat([up(e2, e1.shape[2:]), e1], 1), *P["dec1"], padding=1))
     m0 = F.relu(F.conv2d(torch.cat([up(m1, e0.shape[2:]), e0], 1), *P["dec0"], padding=1))
     dump.update(e1=e1, e2=e2, m1=m1, m0=m0)
@@ -117,9 +120,48 @@ def test_dense_connection_by_brute_force_scatter():
     assert np.max(np.abs(t - dump[0]["block0"])) < 1e-10
 
 
-def test_pool_upsample_and_uncertainty_by_hand():
-    # a net whose stem copies the input and whose blocks / U-Net can be followed by hand is
-    # overkill; pin the two resampling rules through torch (above) and the decode here.
+def test_upsample2_against_interpolate_and_by_hand():
+    """Reading D5 ("two-stage U-Net"; P:192 item 2): nearest neighbour x 2 to exactly the finer
+    map's size.  Even sizes: torch's nearest interpolation.  Odd target: written out by hand."""
+    import torch
+    import torch.nn.functional as F
+    rng = np.random.default_rng(3)
+    for c, H, W in ((1, 1, 1), (3, 4, 6), (2, 5, 3)):
+        x = rng.normal(size=(c, H, W))
+        ref = F.interpolate(torch.from_numpy(x)[None], scale_factor=2, mode="nearest")[0].numpy()
+        assert np.array_equal(D.upsample2(x, 2 * H, 2 * W), ref)
+    x = np.array([[[1., 2., 3.], [4., 5., 6.], [7., 8., 9.]]])
+    want = np.array([[1, 1, 2, 2, 3, 3, 3],
+                     [1, 1, 2, 2, 3, 3, 3],
+                     [4, 4, 5, 5, 6, 6, 6],
+                     [4, 4, 5, 5, 6, 6, 6],
+                     [7, 7, 8, 8, 9, 9, 9],
+                     [7, 7, 8, 8, 9, 9, 9],
+                     [7, 7, 8, 8, 9, 9, 9]], dtype=np.float64)
+    assert np.array_equal(D.upsample2(x, 7, 7)[0], want)
+    assert np.array_equal(D.upsample2(x, 6, 7)[0], want[:6]) and np.array_equal(D.upsample2(x, 7, 6)[0], want[:, :6])
+    two = np.stack([x[0], -x[0].T])                       # channels stay apart, rows are not columns
+    got = D.upsample2(two, 7, 7)
+    assert np.array_equal(got[0], want) and np.array_equal(got[1], -want.T)
+
+
+def test_maxpool2_against_max_pool2d_and_by_hand_on_an_odd_map():
+    """Reading D4: 2 x 2 max pooling, stride 2, floor - the trailing odd row / column is dropped."""
+    import torch
+    import torch.nn.functional as F
+    rng = np.random.default_rng(4)
+    for c, H, W in ((1, 2, 2), (3, 6, 8), (2, 7, 5), (2, 4, 9)):
+        x = rng.normal(size=(c, H, W))
+        assert np.array_equal(D.maxpool2(x), F.max_pool2d(torch.from_numpy(x)[None], 2)[0].numpy())
+    x = np.array([[[1, 9, 2, 3, 50],
+                   [4, 5, 8, 7, 51],
+                   [-1, -2, -3, -4, 52],
+                   [-8, -7, -6, -5, 53],
+                   [60, 61, 62, 63, 64]]], dtype=np.float64)
+    assert np.array_equal(D.maxpool2(x)[0], np.array([[9., 8.], [-1., -3.]]))   # row 4 / column 4 never read
+
+
+def test_uncertainty_decode_by_hand():
     spec = DlocSpec(c0=8, growth=4)
     o = np.zeros((1, 10, 4, 4))
     o[0, 0] = -5.0
