@@ -607,8 +607,7 @@ def main(argv=None):
         alg_bytes_per_launch = 4.0 * C * H * W * n_frames * args.steps * L / layers_run
         # DRAM traffic per launch: dram__bytes_read.sum + dram__bytes_write.sum of the dominant
         # kernel in this launch shape, from the tracked ncu --set full record
-        # (profiles/traffic_r2.json, written by paper_2410_02314_b200/profile_tools.py from the
-        # capture named there); null when no capture of this (workload, views per launch) exists.
+        # (profiles/traffic_r2.json: per-kernel means of one `ncu --set full` capture, named there); null when no capture of this (workload, views per launch) exists.
         traffic, traffic_note = lookup_traffic(cfg, C, loc_views_per_launch, bound, dominant_pair, args.fusion)
         roofline = {"bound": bound,
                     "kernel": "conv3x3_dilated x2, layers (d, 2d) fused (conv_pair_kernel)" if dominant_pair

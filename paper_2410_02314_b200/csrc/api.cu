@@ -375,7 +375,7 @@ smlm_status store_count(smlm_ctx* c, const unsigned long long* counter, int64_t*
 
 int auto_micro_batch(const smlm_ctx* c, int Hw, int Ww) {
   if (c->d.micro_batch > 0) return c->d.micro_batch;
-  // Measured on B200 (profiles/microbatch_sweep_r1.md, profiles/bench_r2.md): keeping the two
+  // Measured on B200 (round-1 micro-batch sweep; profiles/bench_r2.md): keeping the two
   // ping-pong maps L2-resident (7 frames of 256x256x48) is SLOWER than streaming large
   // micro-batches from HBM - per-launch overheads (prologue, weight load, tail) and the halo
   // steps per work range weigh more than the DRAM traffic.  So: up to 128 views per launch

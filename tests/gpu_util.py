@@ -225,10 +225,12 @@ def parity_gate(spec, o_oracle, em_oracle, em_gpu, threshold, tol, pixel_size_nm
 
 
 # ---------------------------------------------------------------------------- parity record
-# Every gate run appends its statistics here; the file comes back from the GPU box in
-# gpurun_out/ and is committed as profiles/parity_r2.json ("a vacuous gate must be visible").
-_RECORD_PATH = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out",
-                            "parity_r2.json")
+# Every gate run appends its statistics to one JSON file ("a vacuous gate must be visible").  The
+# file goes where SMLM_PARITY_RECORD points (a GPU run sets it to a path that travels back, and a
+# summary of it is committed under profiles/), else to the system's temporary directory.
+import tempfile
+
+_RECORD_PATH = os.environ.get("SMLM_PARITY_RECORD") or os.path.join(tempfile.gettempdir(), "smlm_parity_record.json")
 _RECORDS = {}
 
 
@@ -245,7 +247,7 @@ def record(test, **stats):
         return v
     _RECORDS[test] = plain(stats)
     try:
-        os.makedirs(os.path.dirname(_RECORD_PATH), exist_ok=True)
+        os.makedirs(os.path.dirname(os.path.abspath(_RECORD_PATH)), exist_ok=True)
         with open(_RECORD_PATH, "w", encoding="utf-8") as fh:
             json.dump({"written_by": "tests/gpu_util.py record() during `pytest tests -m gpu`",
                        "records": _RECORDS}, fh, indent=1, sort_keys=True)

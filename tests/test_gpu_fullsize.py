@@ -118,10 +118,17 @@ def test_cfg3_2048_tiled_sampled_rows_against_oracle_crop():
     H = W = 2048
     ck = G.cam_kwargs(fs)
     frames = np.ascontiguousarray(np.concatenate([fs.frames, fs.frames]))
-    em = G.gpu_localize(cfg.net, w, frames, ck, cfg.threshold, capacity=2 * 4 * cfg.frames.emitters_per_frame,
-                        host_frames=True, host_out=True, tile=cfg.tile)
-    a, b = em[em["frame"] == 0], em[em["frame"] == 1]
-    assert len(a) > 1000 and np.array_equal(a["pix"], b["pix"]) and np.array_equal(a["x_nm"], b["x_nm"])
+    lists = {}
+    # NONE: the library default, 606 x 606 windows (layer pairs on 5-CTA clusters).  ROW: the shape
+    # bench.py times for cfg 3, windows of 606 rows x the whole 2048-pixel width, one layer per kernel.
+    for merge in (P.TILE_MERGE_NONE, P.TILE_MERGE_ROW):
+        em = G.gpu_localize(cfg.net, w, frames, ck, cfg.threshold, capacity=2 * 4 * cfg.frames.emitters_per_frame,
+                            host_frames=True, host_out=True, tile=cfg.tile, tile_merge=merge)
+        a, b = em[em["frame"] == 0], em[em["frame"] == 1]
+        assert len(a) > 1000 and np.array_equal(a["pix"], b["pix"]) and np.array_equal(a["x_nm"], b["x_nm"])
+        lists[merge] = a
+    # the two window shapes compute every owned pixel from the same receptive field
+    assert lists[P.TILE_MERGE_NONE].tobytes() == lists[P.TILE_MERGE_ROW].tobytes()
     # crop with its origin at the frame origin: rows/cols 0..699 (the frame border keeps its
     # zero padding, the inner edges lose 47 px)
     S, M = 700, 47
@@ -135,6 +142,7 @@ def test_cfg3_2048_tiled_sampled_rows_against_oracle_crop():
     inner = lambda y, x: (y < S - M) & (x < S - M)
     yo, xo = em_o["pix"] // S, em_o["pix"] % S
     em_o = em_o[inner(yo, xo)]
+    a = lists[P.TILE_MERGE_ROW]                    # the timed shape against the oracle (NONE is byte-identical)
     ya, xa = a["pix"] // W, a["pix"] % W
     ag = a[inner(ya, xa)].copy()
     ag["pix"] = (ya[inner(ya, xa)] * S + xa[inner(ya, xa)]).astype(np.int32)
@@ -148,5 +156,5 @@ def test_cfg3_2048_tiled_sampled_rows_against_oracle_crop():
     og_in[:, :, :S - M + 1, :S - M + 1] = og[:, :, :S - M + 1, :S - M + 1]
     st = G.parity_gate(cfg.net, o, em_o, ag, cfg.threshold, 2e-2, fs.pixel_size_nm, S, S, dp_measured=dp,
                        o_gpu=og_in)
-    G.record("cfg3_2048_tiled_vs_oracle_crop", gate=st)
+    G.record("cfg3_2048_tiled_vs_oracle_crop", gate=st, shapes="tile_merge ROW (timed) == NONE byte for byte")
     assert st["oracle"] > 1000 and st["contested_frac_local"] <= 0.6 and st["uncontested_local"] >= 100, st
