@@ -405,6 +405,9 @@ def main(argv=None):
     ap.add_argument("--frames", type=int, default=0, help="override the number of frames per step")
     ap.add_argument("--conv-impl", default="auto", choices=["auto", "tcgen05", "direct"])
     ap.add_argument("--micro-batch", type=int, default=0)
+    ap.add_argument("--weights", default="lc", choices=["lc", "st"],
+                    help="synthetic weight set: lc = random He-normal net (smooth p-map, ~29 %% of the pixels above the "
+                         "threshold), st = surrogate for trained weights (sharp p-map peaks, a few %% above the threshold)")
     ap.add_argument("--fusion", default="auto", choices=["auto", "none", "all", "head", "pairs1"])
     ap.add_argument("--stem", default="auto", choices=["auto", "tensor", "cuda"],
                     help="K1 kernel: SMLM_STEM_AUTO / TENSOR (conv_chain.cu STEM variant) / CUDA_CORES (stem.cu)")
@@ -464,7 +467,7 @@ def main(argv=None):
         lo, hi = shard_frames(n_frames, rank, world)
         n_frames = hi - lo
     fs, frames = workload(cfg, n_frames)
-    weights = make_weights(cfg)
+    weights = make_weights(cfg, args.weights)
     H, W = frames.shape[1:]
     conv_impl = {"auto": P.CONV_AUTO, "tcgen05": P.CONV_TCGEN05, "direct": P.CONV_DIRECT}[args.conv_impl]
     tile_merge = args.tile_merge if args.tile_merge != "auto" else ("row" if cfg.tile else "none")
@@ -671,7 +674,7 @@ def main(argv=None):
         "dtype": {"bf16": "bf16", "fp16": "f16"}.get(cfg.net.precision, "f32"), "data": "synthetic",
         "config": {"workload": cfg.name, "frames_per_step": n_frames, "H": H, "W": W, "channels": C,
                    "layers": L, "head_channels": cfg.net.head_channels, "tile": cfg.tile, "tile_merge": tile_merge,
-                   "precision": cfg.net.precision,
+                   "precision": cfg.net.precision, "weights": args.weights,
                    "distinct_frames": int(len(fs.frames)), "conv_impl": args.conv_impl, "fusion": args.fusion, "stem": args.stem,
                    "l2": "inputs larger than L2 (u16 stack + activation stream per step > 126 MB)",
                    "parallelism": f"replicas x{world}"},

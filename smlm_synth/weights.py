@@ -20,6 +20,16 @@ Flavours (readings G12, G13 of SURVEY.md 8(c), restated in DESIGN.md):
              (never from the CUDA path).  Low-contrast set used in bf16 mode.
   "hc"       same with a high-contrast p-head (logit std 3) - the strong index test, run
              through the library's fp32 mode.
+  "st"       surrogate for TRAINED weights ("the probability of a
+             fluorescent molecule" peaks at single pixels): hand-set signal channels inside the
+             random net, so that the p-map has sharp peaks at the emitters and ~1 % of the
+             pixels exceed the threshold, as a trained DilatedLoc would give, instead of the
+             smooth map of random weights.  Stem channel 0 is a zero-mean matched filter for the
+             sigma = 1.3 px PSF, channels 1-4 are +x / -x / +y / -y gradient filters; the trunk
+             rows that write into these five channels are scaled by `ST_TRUNK_LEAK`; the p-head
+             reads channel 0 only (x kappa, + b_p from calibration.json, oracle statistics), the
+             dx / dy heads read the gradient channels, the other rows are the random ones x 0.3.
+             Everything else (the other stem filters, the trunk) is the seeded He-normal draw.
 The library never sees flavours: it receives the final blob.
 """
 from __future__ import annotations
@@ -98,6 +108,41 @@ def apply_recipe(net: NetSpec, blob: np.ndarray, g_res: float, row_gain, kappa: 
     return out.astype(np.float32)
 
 
+ST_SIGNAL_GAIN = 4.0     # scale of the five hand-set stem filters
+ST_TRUNK_LEAK = 0.05     # trunk rows writing into the signal channels: residual additions stay small
+ST_XY_GAIN = 2.0         # dx / dy head gain on the gradient channels
+
+
+def st_base_blob(net: NetSpec, seed: int, g_res: float, sigma_px: float = 1.3) -> np.ndarray:
+    """The "st" flavour before calibration (p-head = channel 0 with gain 1 and zero bias)."""
+    out = he_normal_blob(net, seed).astype(np.float64)
+    off = blob_offsets(net)
+    C, L, nh, IF = net.channels, net.n_layers, net.head_channels, net.in_frames
+    k = np.arange(-1, 2, dtype=np.float64)
+    g = np.exp(-(k[:, None] ** 2 + k[None, :] ** 2) / (2.0 * sigma_px ** 2))
+    mf = g - g.mean()
+    mf /= np.sqrt((mf ** 2).sum())
+    gx = np.outer([1.0, 2.0, 1.0], [-1.0, 0.0, 1.0]) / 8.0          # [ky][kx]: rises to the right
+    stem = out[off["stem_w"]:off["stem_w"] + C * IF * 9].reshape(C, IF, 3, 3)
+    stem[:5] = 0.0
+    c = IF // 2                                                        # the frame itself (3-frame context: centre)
+    for ch, f in enumerate((mf, gx, -gx, gx.T, -gx.T)):
+        stem[ch, c] = ST_SIGNAL_GAIN * f
+    for l in range(L):
+        w = out[off[f"w{l}"]:off[f"w{l}"] + C * C * 9].reshape(C, C, 3, 3)
+        w *= g_res
+        w[:5] *= ST_TRUNK_LEAK
+    head = out[off["head_w"]:off["head_w"] + nh * C].reshape(nh, C)
+    head[0] = 0.0
+    head[0, 0] = 1.0
+    head[1] = 0.0
+    head[1, 1], head[1, 2] = ST_XY_GAIN, -ST_XY_GAIN
+    head[2] = 0.0
+    head[2, 3], head[2, 4] = ST_XY_GAIN, -ST_XY_GAIN
+    head[3:] *= 0.3
+    return out.astype(np.float32)
+
+
 def make_weights(cfg: Config, flavour: Optional[str] = None, seed: Optional[int] = None,
                  calibration: Optional[dict] = None) -> np.ndarray:
     """Final fp32 blob for `cfg`.  `flavour` defaults to "literal" for cfg 0, "lc" otherwise."""
@@ -110,11 +155,19 @@ def make_weights(cfg: Config, flavour: Optional[str] = None, seed: Optional[int]
         return blob
     if flavour == "base":          # g_res only; what the calibration script starts from
         return apply_recipe(net, blob, cfg.g_res, [1.0] * net.head_channels, 1.0, 0.0)
+    if flavour == "st_base":
+        return st_base_blob(net, seed, cfg.g_res, cfg.frames.sigma_px)
     cal = load_calibration() if calibration is None else calibration
     key = calibration_key(cfg, flavour, seed)
     if key not in cal:
         raise KeyError(f"no calibration entry {key!r}; run tests/golden/make_calibration.py")
     e = cal[key]
+    if flavour == "st":
+        out = st_base_blob(net, seed, cfg.g_res, cfg.frames.sigma_px).astype(np.float64)
+        off = blob_offsets(net)
+        out[off["head_w"]:off["head_w"] + net.channels] *= float(e["kappa"])
+        out[off["head_b"]] = float(e["b_p"])
+        return out.astype(np.float32)
     return apply_recipe(net, blob, cfg.g_res, e["row_gain"], e["kappa"], e["b_p"])
 
 

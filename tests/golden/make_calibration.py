@@ -14,6 +14,16 @@ are INPUT choices: the library and the oracle both just receive the final blob.
   row_gain  "lc": p 1, dx/dy 0.6, z 0.3, N/bg 0.3 (sized so that bf16 residual-stream
          rounding stays inside the 2e-2 map tolerance);  "hc": all 1
 
+"st" flavour (smlm_synth/weights.py: hand-set signal channels, the surrogate for trained
+weights): the p-head reads channel 0 of the final map, a_L[0].
+  b_p    as above, from the order statistic of the oracle's local maxima of a_L[0]
+  kappa  ST_KAPPA_CUT / cut, cut = that order statistic.  An input choice sized for the bf16 map
+         tolerance: a bf16 residual stream rounds a_l[0] once per layer (2^-9 relative each, up to
+         ~1.6 % after the stem and 12 layers at the worst pixel of a frame), and the p-map error
+         at the threshold is ~ 0.25 * kappa * cut * that.  ST_KAPPA_CUT = 2 keeps it near 1e-2,
+         inside the 2e-2 tolerance, and keeps the p-map out of saturation at the emitters (a
+         saturated peak and its neighbours differ by less than their bf16 error)
+
 Run from the repo root:  python tests/golden/make_calibration.py
 """
 import json
@@ -69,6 +79,47 @@ def calibrate(cfg_index, flavour):
     return calibration_key(cfg, flavour, cfg.weight_seed), entry
 
 
+ST_KAPPA_CUT = 2.0
+
+
+def calibrate_st(cfg_index):
+    cfg = get_config(cfg_index)
+    K = CAL_FRAMES[cfg_index]
+    fs = make_frames(cfg, K)
+    w = make_weights(cfg, "st_base")
+    net = O.net_from_spec(cfg.net)
+    cam = O.make_camera(fs.pixel_size_nm, fs.offset, fs.gain, fs.offset_map, fs.gain_map)
+    o = O.forward_maps(net, w, fs.frames, cam)
+    a0 = o[:, 0]                                                   # = a_L[0]: gain 1, bias 0
+    maxima = O.postprocess(net, o, cam, 0.0)
+    H, W = fs.frames.shape[1:]
+    v = np.sort(a0.reshape(K, -1)[maxima["frame"], maxima["pix"]])[::-1]
+    n_max = len(v) / K
+    target = min(cfg.frames.emitters_per_frame, int(0.8 * n_max))
+    k = int(target * K)
+    cut = 0.5 * (v[k - 1] + v[k])
+    kappa = ST_KAPPA_CUT / cut
+    lthr = math.log(cfg.threshold / (1 - cfg.threshold))
+    b_p = float(lthr - kappa * cut)
+    entry = {"kappa": float(kappa), "b_p": b_p}
+    key = calibration_key(cfg, "st", cfg.weight_seed)
+    wf = make_weights(cfg, "st", calibration={key: entry})
+    of = O.forward_maps(net, wf, fs.frames, cam)
+    em = O.postprocess(net, of, cam, cfg.threshold)
+    hit = 0                                                        # detections within 1 px of a simulated emitter
+    for f in range(K):
+        t, s = fs.truth[f], em[em["frame"] == f]
+        d = np.hypot((s["pix"] % W)[:, None] - t[None, :, 0], (s["pix"] // W)[:, None] - t[None, :, 1])
+        hit += int((d.min(axis=1) < 1.0).sum())
+    p = 1.0 / (1.0 + np.exp(-of[:, 0]))
+    entry["stats"] = {"calibration_frames": K, "cut": float(cut), "local_maxima_per_frame": n_max,
+                      "target_per_frame": target, "oracle_detections_per_frame": len(em) / K,
+                      "within_1px_of_a_simulated_emitter": hit / max(len(em), 1),
+                      "pixels_above_threshold": float((p > cfg.threshold).mean()),
+                      "median_detection_logit": float(np.median(np.log(em["p"] / (1 - em["p"] + 1e-300))))}
+    return key, entry
+
+
 def main():
     cal = {"_note": "written by tests/golden/make_calibration.py from oracle/ statistics only"}
     for ci in (1, 2, 4):
@@ -76,8 +127,11 @@ def main():
             key, e = calibrate(ci, flavour)
             cal[key] = e
             print(key, json.dumps(e["stats"]))
+        key, e = calibrate_st(ci)
+        cal[key] = e
+        print(key, json.dumps(e["stats"]))
     # cfg 3 runs the cfg-1 architecture on the same emitter density: it reuses cfg 1's weights
-    for flavour in ("lc", "hc"):
+    for flavour in ("lc", "hc", "st"):
         src = cal[calibration_key(get_config(1), flavour, get_config(1).weight_seed)]
         cal[calibration_key(get_config(3), flavour, get_config(3).weight_seed)] = dict(src, alias_of="cfg1")
     with open(OUT, "w", encoding="utf-8") as fh:

@@ -86,13 +86,13 @@ def test_cfg4_stream_10000_frames_writeback_256_sampled_against_oracle():
     cfg = get_config(4)
     n, k = cfg.frames.n_frames, 8
     fs, frames = _stack(cfg, n, k)
-    w = make_weights(cfg)
+    w = make_weights(cfg, "st")        # sharp p-map peaks (reading G28): the index gate covers >= 85 % of the detections
     cap = int(n * 1.5 * cfg.frames.emitters_per_frame)
     em = G.gpu_localize(cfg.net, w, frames, G.cam_kwargs(fs), cfg.threshold, capacity=cap,
                         host_frames=True, host_out=True, writeback_frames=cfg.writeback_batch)
     em = _check_cycle_and_adjacency(em, n, k, 256)
     _oracle_gate("cfg4_stream_10000_frames", cfg, w, fs, em, (0, 255, 256, 2559, 9999), 2e-2, 256, 256,
-                 max_contested=0.75)
+                 max_contested=0.15)
 
 
 def test_cfg2_512x512_six_heads_sampled_against_oracle():

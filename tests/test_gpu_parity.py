@@ -183,7 +183,8 @@ def _bf16_maps_and_gate(name, cfg, fs, w, impl, H, W, max_contested, check_tol=T
                        dp_measured=dp, check_tol=check_tol, o_gpu=og)
     impl_name = {P.CONV_DIRECT: "direct", P.CONV_TCGEN05: "tcgen05"}[impl]
     G.record(f"{name}_bf16_{impl_name}", gate=st, head_max_err=err, frames=len(fs.frames), H=H, W=W)
-    assert st["contested_frac_local"] <= max_contested, st
+    if max_contested is not None:
+        assert st["contested_frac_local"] <= max_contested, st
     assert st["uncontested_local"] >= 100, st
     return st
 
@@ -215,9 +216,23 @@ def test_cfg2_crop_bf16_six_heads(impl):
 
 @pytest.mark.parametrize("impl", BF16_IMPLS)
 def test_cfg4_dense_bf16(impl):
+    """cfg 4 with the random `lc` weights: map parity, and the index gate outside the contested set.
+    No cap on the contested fraction here (it is recorded: ~0.6 on this smooth p-map, DESIGN.md
+    reading G28); the bounded index gate of cfg 4 is test_st_weights_bf16_index_gate."""
     cfg = get_config(4)
-    # 4 emitters / um^2: the smooth p-map has more near-ties between neighbours than cfg 1
-    _bf16_maps_and_gate("cfg4", cfg, make_frames(cfg, 1), make_weights(cfg, "lc"), impl, 256, 256, 0.75)
+    _bf16_maps_and_gate("cfg4", cfg, make_frames(cfg, 1), make_weights(cfg, "lc"), impl, 256, 256, None)
+
+
+@pytest.mark.parametrize("impl", BF16_IMPLS)
+@pytest.mark.parametrize("ci", [1, 4])
+def test_st_weights_bf16_index_gate(ci, impl):
+    """The surrogate-trained weight set (smlm_synth "st", reading G28: sharp p-map peaks at the
+    emitters, as P:61 describes the trained net's output) through the bf16 kernels: maps within
+    2e-2, and the index gate must compare most detections bit-exactly - at most 15 % of the
+    oracle's detections may lie in the contested set built from the measured local error."""
+    cfg = get_config(ci)
+    st = _bf16_maps_and_gate(f"cfg{ci}st", cfg, make_frames(cfg, 2), make_weights(cfg, "st"), impl, 256, 256, 0.15)
+    assert st["oracle"] > 0.9 * 2 * min(cfg.frames.emitters_per_frame, 2621)
 
 
 # ------------------------------------------------------------------ maps in the launch shape bench.py times
