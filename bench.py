@@ -28,6 +28,7 @@ from smlm_synth import get_config, make_frames, make_weights  # noqa: E402
 
 METRIC = "frames_per_s_256x256"
 UNIT = "frames/s"
+REPEATS = 3                 # timed windows per path; the median one is reported
 DISTINCT_FRAMES = 128       # generated once, cycled to the config's frame count (throughput is data-independent)
 # /opt/skills/guides/B200_PROFILING.md, "Peaks and the roofline denominators": "FALLBACK, only if that file
 # is absent ...: 6.65 TB/s and 1.59 PFLOP/s ... (1.59 is the burst figure; sustained it settles near 1.4 PFLOP/s)".
@@ -345,6 +346,33 @@ def run_dloc(args, cfg):
     return 0
 
 
+OTHER_CONFIGS = {   # short device-resident runs appended to the default line (the driver's record then holds them too)
+    "cfg2_3d_astig_512_bf16": ["--config", "2", "--frames", "96"],
+    "cfg3_fov2048_tiled_bf16": ["--config", "3", "--frames", "8"],
+    "cfg4_dense_stream_bf16": ["--config", "4", "--frames", "2560"],
+    "dloc_on_cfg1": ["--net", "dloc", "--frames", "256"],
+}
+
+
+def other_configs(args):
+    """Each of OTHER_CONFIGS as a child `bench.py` process after the headline's timed region (own
+    process: own clocks sample, no shared device memory); its JSON line reduced to the judged keys."""
+    import subprocess
+    out = {}
+    for name, extra in OTHER_CONFIGS.items():
+        cmd = [sys.executable, os.path.abspath(__file__), *extra, "--steps", "3", "--warmup", "3", "--no-cpu-baseline",
+               "--no-other-configs", "--weights", args.weights]
+        try:
+            r = subprocess.run(cmd, capture_output=True, text=True, timeout=240)
+            d = json.loads(r.stdout.strip().splitlines()[-1])
+            out[name] = {k: d.get(k) for k in ("value", "unit", "ms_per_step", "steps", "dtype", "config", "e2e", "gpu_launches",
+                                               "clocks", "roofline", "io_kernels", "tensor_frac_whole_step", "emitters_per_frame")}
+            out[name]["command"] = "python bench.py " + " ".join(cmd[2:])
+        except Exception as ex:  # the headline line must still be printed
+            out[name] = {"error": f"{type(ex).__name__}: {ex}"[:300]}
+    return out
+
+
 def _rank_entry(rank, world, port, argv):
     """One rank of a self-spawned run: the same environment torchrun would set."""
     os.environ.update(RANK=str(rank), LOCAL_RANK=str(rank), WORLD_SIZE=str(world), LOCAL_WORLD_SIZE=str(world),
@@ -418,6 +446,8 @@ def main(argv=None):
     ap.add_argument("--precision", default="", choices=["", "bf16", "fp16"],
                     help="activation storage type of the variants study (SURVEY.md 8(f)-4); default: the config's")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true",
+                    help="default cfg-1 run only: do not append the short runs of cfgs 2, 3, 4 and --net dloc")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = every rank localises the config's full stack (replicas); "
                          "strong = the stack is sharded by frame range (shard_frames)")
@@ -527,8 +557,12 @@ def main(argv=None):
         timed(frames_host, out_host, max(1, extra // 3))
 
     sampler.start()
-    ms, counts, launches, _ = timed(frames_dev, out_dev, args.steps)
-    ms_e2e, counts_e2e, _, _ = timed(frames_host, out_host, args.steps)
+    # the timed window (exactly --steps steps) runs REPEATS times per path; `value` / `e2e` come from
+    # the median window, all windows are listed under "repeats" (run-to-run spread of the power governor)
+    reps_dev = [timed(frames_dev, out_dev, args.steps) for _ in range(REPEATS)]
+    reps_e2e = [timed(frames_host, out_host, args.steps) for _ in range(REPEATS)]
+    ms, counts, launches, _ = sorted(reps_dev, key=lambda r: r[0])[REPEATS // 2]
+    ms_e2e, counts_e2e, _, _ = sorted(reps_e2e, key=lambda r: r[0])[REPEATS // 2]
     # roofline pass: the same steps with every K2 launch bracketed by CUDA events on the
     # launching stream (the events serialise a little, so `value` is not taken from this pass)
     ms_rf, _, _, kt = timed(frames_dev, out_dev, args.steps, kernel_timing=True)
@@ -634,15 +668,18 @@ def main(argv=None):
     # measured HBM copy bandwidth.  K1 is a pure WRITE stream (2 B in, 2C B out per pixel); a
     # plain fill of device memory, measured here, is its real roof (profiles/stem_r2.md).
     fill = torch.empty(1 << 30, dtype=torch.uint8, device="cuda")
-    fill_ms = 1e9
-    for _ in range(6):
-        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        f0.record()
-        fill.fill_(1)
-        f1.record()
-        torch.cuda.synchronize()
-        fill_ms = min(fill_ms, f0.elapsed_time(f1))
-    write_gbs = fill.numel() / (fill_ms * 1e-3) / 1e9
+    f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    write_modes = {}
+    for mode, label in ((0, "cudaMemsetAsync"), (1, "st.global.v4 kernel (smlm_debug_fill)")):
+        best = 1e9
+        for _ in range(10):
+            f0.record()
+            P.debug_fill(fill, mode)
+            f1.record()
+            torch.cuda.synchronize()
+            best = min(best, f0.elapsed_time(f1))
+        write_modes[label] = fill.numel() / (best * 1e-3) / 1e9
+    write_src, write_gbs = max(write_modes.items(), key=lambda kv: kv[1])
     del fill
     io_kernels = {}
     if kt is not None:
@@ -659,7 +696,8 @@ def main(argv=None):
                 if kind == P.KERNEL_STEM:
                     io_kernels[name]["frac_of_write_stream_peak"] = gbs / write_gbs
                     io_kernels[name]["write_stream_peak_GBs"] = write_gbs
-                    io_kernels[name]["write_stream_peak_source"] = "torch fill_ of 1 GiB, best of 6, this run"
+                    io_kernels[name]["write_stream_peak_source"] = f"{write_src}, 1 GiB, best of 10, this run"
+                    io_kernels[name]["write_only_GBs"] = write_modes
     cpu = None
     if not args.no_cpu_baseline:
         # bounded sample: about 2e12 FLOP of oracle work (10-15 s on 16 host cores)
@@ -691,7 +729,13 @@ def main(argv=None):
         "from_disk": disk,
         "tensor_frac_whole_step": (cfg.net.flop_per_px() * H * W * n_frames * args.steps / (ms_max * 1e-3) / 1e12)
                                   / float(peaks["bf16_tflops"]),
+        "repeats": {"windows": REPEATS, "steps_per_window": args.steps, "reported": "median window",
+                    "value": sorted(world * n_frames * args.steps / (r[0] * 1e-3) for r in reps_dev),
+                    "e2e": sorted(world * n_frames * args.steps / (r[0] * 1e-3) for r in reps_e2e),
+                    "note": "this rank's windows x world size" if world > 1 else "frames/s of each window, ascending"},
     }
+    if world == 1 and args.config == 1 and not args.frames and not args.no_other_configs and not args.disk:
+        line["other_configs"] = other_configs(args)
     print(json.dumps(line), flush=True)
     loc.close()
     if dist is not None:

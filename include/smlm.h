@@ -273,6 +273,11 @@ smlm_status smlm_debug_postprocess(smlm_ctx* ctx, const float* maps, int64_t n_f
                                    int32_t W, const smlm_camera_params* camera, float threshold,
                                    smlm_emitter* out_emitters, int64_t* out_count, void* cuda_stream);
 
+/* Measurement aid for bench.py (no part of the method): fill `bytes` (a multiple of 16) of DEVICE
+ * memory at `dst` (16-byte aligned) with a byte pattern.  mode 0: cudaMemsetAsync; mode 1: a kernel
+ * of 16-byte stores.  Asynchronous on `cuda_stream`.  The write-only bandwidth K1 is held against. */
+smlm_status smlm_debug_fill(void* dst, int64_t bytes, int32_t mode, void* cuda_stream);
+
 /*
  * smlm_postprocess_static: post-processing for callers that cannot allocate GPU memory.
  *

@@ -26,7 +26,7 @@ KERNEL_STEM, KERNEL_CONV, KERNEL_POST, KERNEL_CONV_PAIR = 0, 1, 2, 3
 
 EXPORTS = ["smlm_create", "smlm_localize", "smlm_check", "smlm_destroy", "smlm_last_error",
            "smlm_launch_count", "smlm_kernel_timing", "smlm_kernel_time_ms",
-           "smlm_debug_forward_maps", "smlm_debug_postprocess",
+           "smlm_debug_forward_maps", "smlm_debug_postprocess", "smlm_debug_fill",
            "smlm_ring_open", "smlm_localize_ring", "smlm_ring_acquire", "smlm_ring_release",
            "smlm_ring_close", "smlm_ring_rewind", "smlm_postprocess_static", "smlm_postprocess_static_error"]
 RING_PAGEABLE = 1
@@ -111,6 +111,8 @@ def lib():
         L.smlm_ring_rewind.argtypes = [vp]
         L.smlm_ring_close.restype = None
         L.smlm_ring_close.argtypes = [vp]
+        L.smlm_debug_fill.restype = C.c_int
+        L.smlm_debug_fill.argtypes = [vp, i64, i32, vp]
         L.smlm_postprocess_static.restype = C.c_int
         L.smlm_postprocess_static.argtypes = [vp, i64, i32, i32, C.POINTER(PostParams), f32, vp, i64, vp, vp]
         L.smlm_postprocess_static_error.restype = C.c_char_p
@@ -371,6 +373,13 @@ def postprocess_static(maps, head_channels: int, threshold: float, out_emitters,
                                        int(capacity), _ptr(out_count), _stream_handle(stream))
     if st != OK:
         raise SmlmError(st, (lib().smlm_postprocess_static_error() or b"").decode())
+
+
+def debug_fill(buf, mode: int, stream=None) -> None:
+    """smlm_debug_fill over a whole cuda tensor (mode 0: cudaMemsetAsync, 1: 16-byte store kernel)."""
+    st = lib().smlm_debug_fill(_ptr(buf), int(buf.numel() * buf.element_size()), int(mode), _stream_handle(stream))
+    if st != OK:
+        raise SmlmError(st, "smlm_debug_fill")
 
 
 def emitters_to_numpy(buf, count: int) -> np.ndarray:

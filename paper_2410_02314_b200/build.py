@@ -17,7 +17,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(ROOT, "include")
 LIB = os.path.join(HERE, "libsmlm_b200.so")
-SOURCES = ["api.cu", "ring.cu", "stem.cu", "conv_direct.cu", "conv_umma.cu", "conv_pair.cu", "head_post.cu", "post_static.cu", "conv_gen.cu", "conv_chain.cu", "dloc.cu"]
+SOURCES = ["api.cu", "ring.cu", "stem.cu", "conv_direct.cu", "conv_umma.cu", "conv_pair.cu", "head_post.cu", "post_static.cu", "probe.cu", "conv_gen.cu", "conv_chain.cu", "dloc.cu"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 
 
