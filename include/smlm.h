@@ -68,9 +68,10 @@ enum { SMLM_FP32 = 0, SMLM_BF16 = 1, SMLM_FP16 = 2 };
 enum { SMLM_TILE_MERGE_NONE = 0, SMLM_TILE_MERGE_ROW = 1 };
 
 /* K1 (uint16 unpack + normalise + 3x3 stem) kernel choice.
- *   AUTO          CUDA_CORES.  Both kernels are bound by the same thing - the write stream of a_0
- *                 (2.5 TB/s in isolation, 2.3 TB/s in the step, against 3.9 TB/s for a plain fill of
- *                 device memory: profiles/stem_r2.md) - and take the same time.
+ *   AUTO          CUDA_CORES.  Both kernels take the same time on cfg 1 (2.2 TB/s of a_0 written inside
+ *                 the step).  That is 0.41 of the write-only bandwidth of this GPU (5.4 TB/s, 16-byte
+ *                 stores, measured by bench.py in the same run: profiles/bench_r3.md), so neither is at
+ *                 its roof: the way the a_0 chunks are stored, not the arithmetic, sets the pace.
  *   TENSOR        the stem on the tcgen05 tensor cores (conv_chain.cu, STEM variant; 16-bit precision,
  *                 in_frames = 1): fp32 accuracy from three 16-bit pieces of every xhat and every weight,
  *                 fp32 accumulation, bias through three constant-one input channels, ReLU in the
